@@ -1,0 +1,611 @@
+"""Pins of the float64 oracle against what the paper and the mathematics fix.
+
+None of these re-type the oracle's formulas: they are closed forms, conservation laws, special cases that
+reduce to library routines (scipy Rotation, numpy matrix powers), published known-answer vectors, and brute force.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.spatial.transform import Rotation
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+M_, G_ = 0.027, 9.81
+J_ = np.array([1.395e-5, 1.395e-5, 2.173e-5])
+KF, KM = 3.16e-10, 7.94e-12
+W_HOVER = math.sqrt(M_ * G_ / (4 * KF))
+
+
+def gold(fname):
+    out = {}
+    for line in open(os.path.join(GOLD, fname)):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, *v = line.split()
+        out[k] = np.array([float(t) for t in v])
+    return out
+
+
+def fp_state(p=(0, 0, 1), q=(0, 0, 0, 1), v=(0, 0, 0), w=(0, 0, 0), rpm=(W_HOVER,) * 4):
+    return np.concatenate([p, q, v, w, rpm]).astype(np.float64).reshape(17, 1)
+
+
+def ab_state(p=(0, 0, 1), psi=(0, 0, 0), v=(0, 0, 0), dpsi=(0, 0, 0), f=M_ * G_):
+    return np.concatenate([p, psi, v, dpsi, [f]]).astype(np.float64).reshape(13, 1)
+
+
+def rotor_sim(cfo, integrator, overrides=None, model=0):
+    ov = dict(integrator=integrator, iface=cfo.IF_ROTOR if model == 0 else cfo.IF_ATTITUDE)
+    ov.update(overrides or {})
+    sim = cfo.OracleSim(1, 1, model, ov)
+    sim.reset(0)
+    return sim
+
+
+def cmd1(vals, K=1):
+    return np.tile(np.asarray(vals, dtype=np.float32).reshape(1, 1, 4), (K, 1, 1))
+
+
+# ---------------------------------------------------------------------------------- P1 free fall
+@pytest.mark.parametrize("integ", [0, 1])
+def test_p1_free_fall(cfo, integ):
+    sim = rotor_sim(cfo, integ)
+    sim.set_full(state=fp_state(p=(0.3, -0.2, 5.0), rpm=(0,) * 4), step_counter=0)
+    n, h = 500, 1e-3
+    rec = sim.step(cmd1([0, 0, 0, 0]), n, cmd_hold=n, record_every=1)
+    k = np.arange(1, n + 1)
+    if integ == 0:   # forward Euler: z_k = z0 - g h^2 k(k-1)/2, v_k = -g h k
+        z = 5.0 - G_ * h * h * k * (k - 1) / 2
+    else:            # RK4 is exact on a parabola: z0 - g t^2 / 2 (north_star)
+        z = 5.0 - G_ * (k * h) ** 2 / 2
+    np.testing.assert_allclose(rec[:, 2, 0], z, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(rec[:, 9, 0], -G_ * h * k, rtol=1e-13)
+    np.testing.assert_allclose(rec[:, 0, 0], 0.3, atol=1e-15)
+    np.testing.assert_allclose(rec[:, 3:7, 0], np.tile([0, 0, 0, 1.0], (n, 1)), atol=1e-15)
+
+
+# ---------------------------------------------------------------------------------- P2 hover equilibrium
+@pytest.mark.parametrize("integ", [0, 1])
+def test_p2_hover_equilibrium(cfo, integ):
+    assert abs(4 * KF * W_HOVER ** 2 - M_ * G_) < 1e-15
+    W = 14476.0                                   # float32-exact rotor command; mass chosen so 4 k_f W^2 = m g
+    sim = rotor_sim(cfo, integ, dict(mass=4 * KF * W * W / G_))
+    x0 = fp_state(rpm=(W,) * 4)
+    sim.set_full(state=x0, step_counter=0)
+    sim.step(cmd1([W] * 4), 1000, cmd_hold=1000)
+    x = sim.get_state()
+    np.testing.assert_allclose(x[:13, 0], x0[:13, 0], atol=1e-11)
+    np.testing.assert_allclose(x[13:, 0], W, rtol=0, atol=0)
+
+
+def test_p2_controller_returns_hover_speed(cfo):
+    p = cfo.make_params(0)
+    eR, iR, tau, rpm = cfo.attitude_tick(p, [0, 0, 0, 1], [0, 0, 0], [0, 0, 0, M_ * G_], [0, 0, 0])
+    np.testing.assert_allclose(eR, 0, atol=1e-16)
+    np.testing.assert_allclose(tau, 0, atol=1e-20)
+    np.testing.assert_allclose(rpm, W_HOVER, rtol=1e-14)
+    assert abs(W_HOVER - gold("worked_step.txt")["omega_hover"][0]) < 1e-6
+
+
+# ---------------------------------------------------------------------------------- P3 / P4 torque-free body
+TORQUE_FREE = dict(kf=[0, 0, 0], km=[0, 0, 0], g=0.0)
+
+
+def test_p3_precession_closed_form(cfo):
+    sim = rotor_sim(cfo, 1, TORQUE_FREE)
+    w0 = np.array([3.0, -2.0, 10.0])
+    sim.set_full(state=fp_state(w=w0), step_counter=0)
+    sim.step(cmd1([W_HOVER] * 4), 1000, cmd_hold=1000)
+    w = sim.get_state()[10:13, 0]
+    lam = (J_[2] - J_[0]) / J_[0] * w0[2]          # Euler's equations with Jx = Jy: (wx + i wy) rotates at lam
+    z = (w0[0] + 1j * w0[1]) * np.exp(1j * lam * 1.0)
+    np.testing.assert_allclose(w, [z.real, z.imag, 10.0], atol=5e-10)
+    g = gold("closed_forms.txt")
+    assert abs(lam - g["precession_lambda"][0]) < 1e-11
+    np.testing.assert_allclose(w, g["precession_w_1s"], atol=5e-10)
+
+
+def _world_L(x, Jp=0.0):
+    q, w, rpm = x[3:7], x[10:13], x[13:17]
+    S = (rpm[0] - rpm[1] + rpm[2] - rpm[3]) * 2 * math.pi / 60
+    Lb = J_ * w + np.array([0, 0, Jp * S])
+    return Rotation.from_quat(q).apply(Lb)
+
+
+def test_p4_conservation_and_p5_unit_norm(cfo):
+    sim = rotor_sim(cfo, 1, TORQUE_FREE)
+    sim.set_full(state=fp_state(q=Rotation.from_rotvec([0.3, -0.2, 0.5]).as_quat(), w=(3, -2, 10)), step_counter=0)
+    x0 = sim.get_state()[:, 0]
+    rec = sim.step(cmd1([W_HOVER] * 4), 1000, cmd_hold=1000, record_every=1)
+    L0, E0 = _world_L(x0), 0.5 * np.sum(J_ * x0[10:13] ** 2)
+    for k in (0, 99, 499, 999):
+        x = rec[k, :, 0]
+        np.testing.assert_allclose(_world_L(x), L0, rtol=0, atol=1e-9 * np.linalg.norm(L0))
+        assert abs(0.5 * np.sum(J_ * x[10:13] ** 2) - E0) < 1e-10 * E0
+    np.testing.assert_allclose(np.linalg.norm(rec[:, 3:7, 0], axis=1), 1.0, atol=2e-16)     # P5
+
+
+def test_p4_gyro_reading_conserves_total_angular_momentum(cfo):
+    """Eq. (5) as read in DESIGN.md R2: body + rotor angular momentum R(q)(J w + Jp S e_z) is constant while
+    the rotors spin up (dS != 0) and the body tumbles.  The as-printed signs would break this."""
+    Jp = 2.0e-8
+    sim = rotor_sim(cfo, 1, dict(TORQUE_FREE, Jp=Jp))
+    x0 = fp_state(q=Rotation.from_rotvec([0.1, 0.4, -0.3]).as_quat(), w=(2, 1, -3), rpm=(9000, 15000, 11000, 14000))
+    sim.set_full(state=x0, step_counter=0)
+    rec = sim.step(cmd1([20000, 5000, 18000, 7000]), 300, cmd_hold=300, record_every=1)
+    L0 = _world_L(x0[:, 0], Jp)
+    assert abs((rec[-1, 13, 0] - rec[-1, 14, 0]) - (9000 - 15000)) > 1000     # S really changed
+    for k in (0, 50, 299):
+        np.testing.assert_allclose(_world_L(rec[k, :, 0], Jp), L0, rtol=0, atol=2e-9 * np.linalg.norm(L0))
+
+
+# ---------------------------------------------------------------------------------- P6 quaternion kinematics
+def test_p6_constant_yaw_rate_closed_form(cfo):
+    sim = rotor_sim(cfo, 1, TORQUE_FREE)
+    wz = 2.0
+    sim.set_full(state=fp_state(w=(0, 0, wz)), step_counter=0)
+    rec = sim.step(cmd1([W_HOVER] * 4), 1000, cmd_hold=1000, record_every=100)
+    for k in range(10):
+        t = (k + 1) * 0.1
+        np.testing.assert_allclose(rec[k, 3:7, 0], [0, 0, math.sin(wz * t / 2), math.cos(wz * t / 2)], atol=1e-12)
+
+
+def test_quaternion_rate_matches_exponential_map(cfo):
+    """Eq. (2) via an independent route: (q (x) exp(w d/2) - q)/d from scipy's rotation composition."""
+    sim = rotor_sim(cfo, 0, dict(TORQUE_FREE, f_phys=1e6, f_att=1e6, f_pos=1e6))
+    rot = Rotation.from_rotvec([0.7, -0.4, 1.1])
+    w = np.array([1.5, -2.5, 0.8])
+    q0 = rot.as_quat()
+    sim.set_full(state=fp_state(q=q0, w=w), step_counter=0)
+    sim.step(cmd1([W_HOVER] * 4), 1)
+    d = 1e-6
+    q_exact = (rot * Rotation.from_rotvec(w * d)).as_quat()
+    if np.dot(q_exact, q0) < 0:
+        q_exact = -q_exact
+    np.testing.assert_allclose(sim.get_state()[3:7, 0], q_exact, atol=1e-11)
+
+
+# ---------------------------------------------------------------------------------- P7 / P11 first-order lags
+def test_p7_motor_lag_factors(cfo):
+    g = gold("closed_forms.txt")["lag_factors"]
+    z = 1e-3 / 0.03
+    fac = {0: 1 - z, 1: 1 - z + z ** 2 / 2 - z ** 3 / 6 + z ** 4 / 24}
+    assert abs(fac[0] - g[0]) < 1e-10 and abs(fac[1] - g[1]) < 1e-10 and abs(math.exp(-z) - g[2]) < 1e-10
+    for integ in (0, 1):
+        sim = rotor_sim(cfo, integ)
+        sim.set_full(state=fp_state(rpm=(10000, 12000, 16000, 20000)), step_counter=0)
+        k = 60
+        sim.step(cmd1([15000] * 4), k, cmd_hold=k)
+        rpm = sim.get_state()[13:, 0]
+        want = 15000 + (np.array([10000, 12000, 16000, 20000]) - 15000) * fac[integ] ** k
+        np.testing.assert_allclose(rpm, want, rtol=1e-13)
+        if integ == 1:   # and RK4 tracks the exact exponential to O(h^4)
+            np.testing.assert_allclose(rpm, 15000 + (np.array([10000, 12000, 16000, 20000]) - 15000) * math.exp(-k * z), rtol=1e-8)
+
+
+def test_eq6_asymmetric_branch_and_equilibrium(cfo):
+    """Eq. (6): the commanded speed is the unique equilibrium; acceleration / deceleration use their own coefficients."""
+    ov = dict(cv_up=40.0, cv_dn=10.0, cd_up=1e-4, cd_dn=3e-4, f_phys=1e5, f_att=1e5, f_pos=1e5)
+    sim = rotor_sim(cfo, 0, ov)
+    W0 = np.array([10000.0, 12000.0, 15000.0, 20000.0])
+    sim.set_full(state=fp_state(rpm=W0), step_counter=0)
+    sim.step(cmd1([15000] * 4), 1)
+    rate = (sim.get_state()[13:, 0] - W0) * 1e5
+    e = 15000 - W0
+    want = np.where(e >= 0, 40.0 * e + 1e-4 * (15000 ** 2 - W0 ** 2), 10.0 * e + 3e-4 * (15000 ** 2 - W0 ** 2))
+    np.testing.assert_allclose(rate, want, rtol=1e-9, atol=1e-6)
+    assert rate[2] == 0.0
+
+
+def test_p11_thrust_lag(cfo):
+    sim = rotor_sim(cfo, 0, model=1)
+    sim.set_full(state=ab_state(f=0.1), step_counter=0)
+    k, z = 80, 0.002 / 0.03
+    fc = float(np.float32(0.3))                   # the command buffer is float32 by contract
+    sim.step(cmd1([0, 0, 0, fc]), k, cmd_hold=k)
+    assert abs(sim.get_state()[12, 0] - (fc + (0.1 - fc) * (1 - z) ** k)) < 1e-15
+
+
+# ---------------------------------------------------------------------------------- P8 mixer round trip
+def test_p8_mixer_inverts_mixing_matrix(cfo):
+    p = cfo.make_params(0)
+    rng = np.random.default_rng(0)
+    for _ in range(20):
+        q = Rotation.from_rotvec(rng.uniform(-0.3, 0.3, 3)).as_quat()
+        w = rng.uniform(-1, 1, 3)
+        cmd = [*rng.uniform(-0.2, 0.2, 2), rng.uniform(-0.1, 0.1), rng.uniform(0.2, 0.35)]
+        eR, iR, tau, rpm = cfo.attitude_tick(p, q, w, cmd, [0, 0, 0])
+        assert rpm.min() > 1.0 and rpm.max() < 21699.0           # nothing clipped
+        F, tau_back = cfo.mix(p, rpm)
+        assert abs(F - cmd[3]) < 1e-14
+        np.testing.assert_allclose(tau_back, tau, rtol=1e-9, atol=1e-16)
+    # yaw-only torque changes no thrust sum and no roll/pitch torque
+    F0, t0 = cfo.mix(p, [W_HOVER] * 4)
+    d = 500.0
+    rpm = np.sqrt(W_HOVER ** 2 + d * np.array([-1, 1, -1, 1]) * 1e4)
+    F1, t1 = cfo.mix(p, rpm)
+    assert abs(F1 - F0) < 1e-15 and abs(t1[0]) < 1e-17 and abs(t1[1]) < 1e-17 and t1[2] > 0
+
+
+def test_mixing_matrix_geometry(cfo):
+    """C1 by geometry: torque of rotor k = r_k x f_k e_z with r on the X at arm/sqrt(2); yaw = -spin * k_m W^2."""
+    p = cfo.make_params(0)
+    lever = 0.046 / math.sqrt(2)
+    pos = lever * np.array([[1, -1, 0], [-1, -1, 0], [-1, 1, 0], [1, 1, 0]], dtype=float)
+    spin = np.array([1, -1, 1, -1])
+    rpm = np.array([11000.0, 13000.0, 17000.0, 19000.0])
+    F, tau = cfo.mix(p, rpm)
+    f = KF * rpm ** 2
+    want = sum(np.cross(pos[k], [0, 0, f[k]]) for k in range(4)) + np.array([0, 0, -(spin * KM * rpm ** 2).sum()])
+    assert abs(F - f.sum()) < 1e-15
+    np.testing.assert_allclose(tau, want, rtol=1e-12, atol=1e-18)
+
+
+# ---------------------------------------------------------------------------------- P9 tilted thrust parabola
+def test_p9_constant_tilted_thrust(cfo):
+    sim = rotor_sim(cfo, 1)
+    rot = Rotation.from_euler("xyz", [0.3, -0.2, 0.4])
+    W = 16000.0
+    sim.set_full(state=fp_state(p=(1, 2, 3), q=rot.as_quat(), v=(0.5, 0, -0.1), rpm=(W,) * 4), step_counter=0)
+    n = 400
+    sim.step(cmd1([W] * 4), n, cmd_hold=n)
+    t = n * 1e-3
+    acc = rot.apply([0, 0, 4 * KF * W * W / M_]) - np.array([0, 0, G_])
+    x = sim.get_state()[:, 0]
+    np.testing.assert_allclose(x[0:3], np.array([1, 2, 3]) + np.array([0.5, 0, -0.1]) * t + 0.5 * acc * t * t, atol=1e-12)
+    np.testing.assert_allclose(x[7:10], np.array([0.5, 0, -0.1]) + acc * t, atol=1e-12)
+    np.testing.assert_allclose(x[3:7], rot.as_quat() * np.sign(rot.as_quat()[3]), atol=1e-15)
+
+
+# ---------------------------------------------------------------------------------- P10 / P12 abstracted model
+def test_p10_eq10_linear_recurrence(cfo):
+    a, b, c, h, u, k = -130.0, -16.0, 130.0, 0.002, 0.2, 100
+    A = np.array([[1, h], [a * h, 1 + b * h]])
+    B = np.array([0, c * h])
+    Ak = np.linalg.matrix_power(A, k)
+    want = (np.eye(2) - Ak) @ np.linalg.solve(np.eye(2) - A, B * u)
+    np.testing.assert_allclose(want, gold("closed_forms.txt")["eq10_k100"], atol=1e-9)
+    sim = rotor_sim(cfo, 0, model=1)
+    sim.set_full(state=ab_state(), step_counter=0)
+    cm = np.float32(u)     # the command buffer is float32 by contract
+    want32 = (np.eye(2) - Ak) @ np.linalg.solve(np.eye(2) - A, B * float(cm))
+    sim.step(cmd1([cm, -cm, 0.5 * cm, M_ * G_]), k, cmd_hold=k)
+    x = sim.get_state()[:, 0]
+    np.testing.assert_allclose([x[3], x[9]], want32, rtol=1e-12)
+    np.testing.assert_allclose([x[4], x[10]], -want32, rtol=1e-12)
+    np.testing.assert_allclose([x[5], x[11]], 0.5 * want32, rtol=1e-12)
+
+
+def test_p12_abstracted_stationary_and_free_fall(cfo):
+    sim = rotor_sim(cfo, 0, model=1)
+    mg32 = float(np.float32(M_ * G_))
+    sim.set_full(state=ab_state(f=mg32), step_counter=0)
+    sim.step(cmd1([0, 0, 0, mg32]), 200, cmd_hold=200)
+    x = sim.get_state()[:, 0]
+    np.testing.assert_allclose(x[:3], [0, 0, 1 + 0.5 * (mg32 / M_ - G_) * 0.4 * 0.4 * (199 / 200)], atol=1e-12)
+    np.testing.assert_allclose(x[3:6], 0, atol=0)
+    # free fall with f = 0 (Euler ordering as P1)
+    sim.set_full(state=ab_state(f=0.0), step_counter=0)
+    sim.step(cmd1([0, 0, 0, 0]), 100, cmd_hold=100)
+    x = sim.get_state()[:, 0]
+    assert abs(x[2] - (1 - G_ * 0.002 ** 2 * 100 * 99 / 2)) < 1e-13 and abs(x[8] + G_ * 0.2) < 1e-13
+
+
+def test_abstracted_thrust_direction_is_rz_ry_rx(cfo):
+    """Eq. (8) with reading R13: R = Rz Ry Rx -> scipy 'xyz' extrinsic.  One Euler step of v from rest."""
+    sim = rotor_sim(cfo, 0, dict(f_phys=1e4, f_att=1e4, f_pos=1e4), model=1)
+    psi = (0.3, -0.4, 0.9)
+    f = 0.31
+    sim.set_full(state=ab_state(psi=psi, f=f), step_counter=0)
+    sim.step(cmd1([0, 0, 0, f]), 1)
+    acc = sim.get_state()[6:9, 0] * 1e4
+    want = Rotation.from_euler("xyz", psi).apply([0, 0, f / M_]) - [0, 0, G_]
+    np.testing.assert_allclose(acc, want, rtol=1e-10, atol=1e-9)
+
+
+def test_body_drag_opposes_velocity_in_body_frame(cfo):
+    """f_a = Ca * v_body, rotated to world; checked against scipy for both models."""
+    Ca = [-0.01, -0.02, -0.03]
+    rot = Rotation.from_euler("xyz", [0.2, 0.3, -0.5])
+    v = np.array([1.0, -2.0, 0.5])
+    want_drag = rot.apply(np.array(Ca) * rot.inv().apply(v)) / M_
+    for model in (0, 1):
+        sim = rotor_sim(cfo, 0, dict(Ca=Ca, f_phys=1e5, f_att=1e5, f_pos=1e5), model=model)
+        if model == 0:
+            sim.set_full(state=fp_state(q=rot.as_quat(), v=v), step_counter=0)
+            sim.step(cmd1([W_HOVER] * 4), 1)
+            acc = (sim.get_state()[7:10, 0] - v) * 1e5
+        else:
+            sim.set_full(state=ab_state(psi=(0.2, 0.3, -0.5), v=v), step_counter=0)
+            sim.step(cmd1([0, 0, 0, M_ * G_]), 1)
+            acc = (sim.get_state()[6:9, 0] - v) * 1e5
+        thrust = rot.apply([0, 0, G_ if model == 0 else float(np.float32(M_ * G_)) / M_ * 0 + G_]) - [0, 0, G_]
+        np.testing.assert_allclose(acc - want_drag, thrust, atol=2e-5)
+
+
+# ---------------------------------------------------------------------------------- P14 integrator order
+def _smooth_run(cfo, integ, f_phys, T=0.2):
+    """Open-loop (rotor interface) tumbling flight: smooth right-hand side, no controller ticks, no clipping."""
+    sim = rotor_sim(cfo, integ, dict(f_phys=float(f_phys), f_att=float(f_phys), f_pos=float(f_phys)))
+    sim.set_full(state=fp_state(q=Rotation.from_rotvec([0.2, -0.1, 0.3]).as_quat(), v=(0.3, 0.1, 0), w=(1.0, -2.0, 0.5),
+                                rpm=(14000, 14500, 15000, 14200)), step_counter=0)
+    n = int(round(T * f_phys))
+    sim.step(cmd1([15200, 14300, 14100, 15400]), n, cmd_hold=n)
+    return sim.get_state()[:13, 0]
+
+
+def test_p14_integrator_order(cfo):
+    ref = _smooth_run(cfo, 1, 16000)
+    e_eu = [np.linalg.norm(_smooth_run(cfo, 0, f) - ref) for f in (1000, 2000)]
+    e_rk = [np.linalg.norm(_smooth_run(cfo, 1, f) - ref) for f in (250, 500)]
+    assert 1.8 < e_eu[0] / e_eu[1] < 2.2, e_eu
+    assert 12.0 < e_rk[0] / e_rk[1] < 20.0, e_rk
+    assert e_rk[1] < 1e-3 * e_eu[0]
+
+
+# ---------------------------------------------------------------------------------- P15 / P16 Philox and distributions
+def test_p15_philox_known_answers(cfo):
+    rows = [l.split() for l in open(os.path.join(GOLD, "philox_kat.txt")) if not l.startswith("#") and l.strip()]
+    assert len(rows) == 5
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        out = cfo.philox(v[4] | (v[5] << 32), v[:4])
+        assert [int(o) for o in out] == v[6:], r
+
+
+def test_p15_philox_matches_numpy_philox4x64_structure_independent_reimplementation(cfo):
+    """Independent pure-Python restatement of the round function from Salmon et al. on random counters."""
+    def ref(seed, c):
+        k0, k1 = seed & 0xFFFFFFFF, seed >> 32
+        c = list(c)
+        for r in range(10):
+            if r:
+                k0 = (k0 + 0x9E3779B9) & 0xFFFFFFFF
+                k1 = (k1 + 0xBB67AE85) & 0xFFFFFFFF
+            p0, p1 = 0xD2511F53 * c[0], 0xCD9E8D57 * c[2]
+            c = [(p1 >> 32) ^ c[1] ^ k0, p1 & 0xFFFFFFFF, (p0 >> 32) ^ c[3] ^ k1, p0 & 0xFFFFFFFF]
+        return c
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        seed = int(rng.integers(0, 2 ** 63)) * 2 + int(rng.integers(0, 2))
+        c = [int(v) for v in rng.integers(0, 2 ** 32, 4)]
+        assert [int(o) for o in cfo.philox(seed, c)] == ref(seed, c)
+
+
+def test_p16_uniform_exact_and_moments(cfo):
+    assert cfo.uniform(0) == 0.5 / 2 ** 23 and cfo.uniform(0xFFFFFFFF) == 1 - 0.5 / 2 ** 23
+    assert cfo.uniform(0x80000000) == (2 ** 22 + 0.5) / 2 ** 23
+    assert cfo.uniform(0x000001FF) == cfo.uniform(0)                    # low 9 bits dropped
+    assert float(np.float32(cfo.uniform(0x12345678))) == cfo.uniform(0x12345678)   # exact in float32
+    n = 50000
+    us, zs = [], []
+    for i in range(n // 4):
+        w = cfo.philox(99, [i, 0, 7, 2])
+        us += [cfo.uniform(int(v)) for v in w]
+        zs += [*cfo.normal_pair(int(w[0]), int(w[1])), *cfo.normal_pair(int(w[2]), int(w[3]))]
+    us, zs = np.array(us), np.array(zs)
+    assert abs(us.mean() - 0.5) < 4 * math.sqrt(1 / 12 / n) and abs(us.var() - 1 / 12) < 4 * math.sqrt(1 / 180 / n)
+    assert abs(zs.mean()) < 4 / math.sqrt(n) and abs(zs.var() - 1) < 4 * math.sqrt(2 / n)
+    assert abs((zs ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
+    assert np.abs(zs).max() <= math.sqrt(48 * math.log(2)) + 1e-12
+    z0, z1 = cfo.normal_pair(0, 0)       # smallest u: r = sqrt(-2 ln(2^-24)), angle 2 pi 2^-24
+    assert abs(math.hypot(z0, z1) - math.sqrt(48 * math.log(2))) < 1e-12 and z1 > 0 and z0 > 0
+
+
+# ---------------------------------------------------------------------------------- P17 obstacle distance
+def test_p17_obstacle_distance_brute_force(cfo):
+    from paper_2606_01478_b200 import workloads as W
+    wl = W.cfg3(seed=3, M=8, n_steps=40)
+    sim = cfo.OracleSim(wl.M, wl.N, wl.model, wl.params)
+    sim.reset(wl.seed)
+    sim.set_state(wl.broadcast_state, broadcast=True)
+    rec = sim.step(wl.cmds, wl.n_steps, cmd_hold=1, record_every=1)
+    obs = np.asarray(wl.params["obstacles"])
+    want = np.full(8, np.inf)
+    for k in range(40):
+        for w in range(8):
+            for j in range(8):
+                want[w] = min(want[w], np.linalg.norm(rec[k, 0:3, w] - obs[j, :3]) - obs[j, 3])
+    np.testing.assert_allclose(sim.min_dist(), want, rtol=1e-13)
+    assert len(np.unique(want)) == 8                      # the noise stream really differs per world
+
+
+def test_p17_min_over_drones_of_a_world(cfo):
+    from paper_2606_01478_b200 import workloads as W
+    wl = W.cfg4(seed=2, M=2, N=5, n_steps=30)
+    ov = dict(wl.params, n_obstacles=2, obstacles=[[0, 0, 1, 0.2], [-2, -2, 0.5, 0.1]])
+    sim = cfo.OracleSim(2, 5, wl.model, ov)
+    sim.reset(1)
+    rec = sim.step(wl.cmds, 30, cmd_hold=30, record_every=1)
+    obs = np.array(ov["obstacles"])
+    want = [min(np.linalg.norm(rec[k, 0:3, w * 5 + n] - o[:3]) - o[3] for k in range(30) for n in range(5) for o in obs)
+            for w in range(2)]
+    np.testing.assert_allclose(sim.min_dist(), want, rtol=1e-13)
+
+
+# ---------------------------------------------------------------------------------- P18 / P19 controllers
+def test_p18_position_controller_special_cases(cfo):
+    p = cfo.make_params(1)
+    att, ip = cfo.position_tick(p, [1, 2, 3], [0, 0, 0], [0, 0, 1], [1, 2, 3, 0.7], [0, 0, 0])
+    np.testing.assert_allclose(att, [0, 0, 0.7, M_ * G_], atol=1e-15)
+    e = 0.2
+    att, ip = cfo.position_tick(p, [0, 0, 1], [0, 0, 0], [0, 0, 1], [e, 0, 1, 0.0], [0, 0, 0])
+    hpos = 0.01
+    ax = 8 * e + 1 * e * hpos                       # k_p e + k_i (e h_pos): integral updated before use
+    assert abs(att[1] - math.atan(ax / G_)) < 1e-14 and att[1] > 0 and abs(att[0]) < 1e-15 and abs(att[2]) < 1e-15
+    assert abs(att[3] - M_ * G_) < 1e-15            # thrust = t . z_B with z_B = e_z
+    assert abs(ip[0] - e * hpos) < 1e-18
+    # pure +y error must roll negative (right-hand rule about x), tilt limit and thrust limit clip
+    att, _ = cfo.position_tick(p, [0, 0, 1], [0, 0, 0], [0, 0, 1], [0, 0.2, 1, 0.0], [0, 0, 0])
+    assert att[0] < 0 and abs(att[1]) < 1e-15
+    att, _ = cfo.position_tick(p, [0, 0, 1], [0, 0, 0], [0, 0, 1], [50, 0, 60, 0.0], [0, 0, 0])
+    assert att[1] == 0.5 and att[3] == 0.55
+    # the commanded attitude, fed to the abstracted model's thrust direction, points along the desired force
+    tgt = [0.3, -0.2, 1.4, 0.6]
+    att, _ = cfo.position_tick(p, [0, 0, 1], [0.1, 0, 0], [0, 0, 1], tgt, [0, 0, 0])
+    zB = Rotation.from_euler("xyz", att[:3]).apply([0, 0, 1])
+    t = M_ * (np.array([8, 8, 12]) * [0.3, -0.2, 0.4] - np.array([5, 5, 7]) * [0.1, 0, 0]
+              + np.array([1, 1, 6]) * np.array([0.3, -0.2, 0.4]) * hpos + [0, 0, G_])
+    np.testing.assert_allclose(zB, t / np.linalg.norm(t), atol=1e-12)
+
+
+def test_p19_attitude_error_closed_form_and_scipy(cfo):
+    p = cfo.make_params(0)
+    for phi, th in [(0.2, -0.1), (-0.3, 0.25), (0.05, 0.4)]:
+        eR, *_ = cfo.attitude_tick(p, [0, 0, 0, 1], [0, 0, 0], [phi, th, 0, 0.3], [0, 0, 0])
+        want = [-0.5 * math.sin(phi) * (1 + math.cos(th)), -0.5 * math.sin(th) * (1 + math.cos(phi)),
+                0.5 * math.sin(th) * math.sin(phi)]
+        np.testing.assert_allclose(eR, want, atol=1e-15)
+    rng = np.random.default_rng(1)
+    for _ in range(20):   # general case against scipy: e_R = 1/2 vee(Rd^T R - R^T Rd)
+        rot = Rotation.from_rotvec(rng.uniform(-0.6, 0.6, 3))
+        cmd = rng.uniform(-0.5, 0.5, 3)
+        Mx = Rotation.from_euler("xyz", cmd).as_matrix().T @ rot.as_matrix()
+        A = 0.5 * (Mx - Mx.T)
+        eR, *_ = cfo.attitude_tick(p, rot.as_quat(), [0, 0, 0], [*cmd, 0.3], [0, 0, 0])
+        np.testing.assert_allclose(eR, [A[2, 1], A[0, 2], A[1, 0]], atol=1e-15)
+    # small-angle closed loop = identified response (a,b,c) = (-130,-16,130): tau/J = -130 e - 16 w, e ~ -(cmd - angle)
+    eR, iR, tau, _ = cfo.attitude_tick(p, [0, 0, 0, 1], [0.01, 0, 0], [1e-4, 0, 0, 0.3], [0, 0, 0])
+    assert abs(tau[0] / J_[0] - (130 * 1e-4 - 16 * 0.01 - 20 * iR[0])) < 1e-9
+    g = gold("worked_step.txt")
+    eR, iR, tau, rpm = cfo.attitude_tick(p, [0, 0, 0, 1], [0, 0, 0], [0.2, -0.1, 0, 0.265], [0, 0, 0])
+    np.testing.assert_allclose(eR, g["e_R"], atol=1e-12)
+    np.testing.assert_allclose(iR, g["e_R"] * 0.002, atol=1e-14)
+    np.testing.assert_allclose(tau, g["tau_des"], rtol=1e-11)
+    np.testing.assert_allclose(rpm, g["rpm_cmd"], rtol=1e-12)
+
+
+def test_controller_uses_nominal_parameters_under_randomisation(cfo):
+    """Reading R11: the plant uses the per-world m, J, k_f; the onboard controller the nominal ones."""
+    lo, hi = [1.0] * 12, [1.0] * 12
+    lo[0], hi[0] = 1.5, 1.5            # every world 50 % heavier
+    sim = cfo.OracleSim(1, 1, 0, dict(rnd_lo=lo, rnd_hi=hi))
+    sim.reset(3)
+    assert abs(sim.world_params()[0, 0] - 1.5 * M_) < 1e-17
+    sim.step(cmd1([0, 0, 0, M_ * G_]), 1)
+    x = sim.get_state()[:, 0]
+    np.testing.assert_allclose(x[13:], W_HOVER, rtol=1e-7)       # controller still commands nominal hover speed
+    assert abs(x[9] - 1e-3 * (G_ / 1.5 - G_)) < 1e-9             # and the heavier plant sinks
+
+
+# ---------------------------------------------------------------------------------- worked example + P20
+def test_worked_example_first_steps_and_1000_step_state(cfo):
+    g = gold("worked_step.txt")
+    sim = cfo.OracleSim(1, 1, 0, dict(integrator=0))
+    sim.reset(0)
+    cmd = cmd1([0.2, -0.1, 0, 0.265])
+    rec = sim.step(cmd, 1000, cmd_hold=1000, record_every=1)
+    # commands reach the oracle as float32 (relative 3e-8), so the survey's float64 digits hold to ~1e-6 relative
+    np.testing.assert_allclose(rec[0, 13:, 0], g["rpm_step1"], rtol=2e-9)
+    np.testing.assert_allclose(rec[0, :13, 0], fp_state()[:13, 0], atol=1e-15)      # only Omega changed in step 1
+    np.testing.assert_allclose(rec[1, 10:13, 0], g["w_step2"], rtol=1e-6)
+    np.testing.assert_allclose(rec[1, 13:, 0], g["rpm_step2"], rtol=2e-9)
+    assert abs(rec[1, 9, 0] - g["vz_step2"][0]) < 1e-10
+    np.testing.assert_allclose(rec[1, :7, 0], [0, 0, 1, 0, 0, 0, 1], atol=1e-11)
+    np.testing.assert_allclose(rec[-1, 0:3, 0], g["p_euler_1000"], atol=2e-7)
+    np.testing.assert_allclose(rec[-1, 3:7, 0], g["q_euler_1000"], atol=2e-7)
+    np.testing.assert_allclose(rec[-1, 7:10, 0], g["v_euler_1000"], atol=5e-7)
+    sim = cfo.OracleSim(1, 1, 0, dict(integrator=1))
+    sim.reset(0)
+    sim.step(cmd, 1000, cmd_hold=1000)
+    np.testing.assert_allclose(sim.get_state()[0:3, 0], g["p_rk4_1000"], atol=2e-7)
+    assert list(sim.counters()) == [1000, 500, 0, 0]
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+def test_p20_fused_equals_split_bit_identical(cfo, name):
+    from paper_2606_01478_b200 import workloads as W
+    small = dict(cfg2=dict(M=6, n_steps=120), cfg3=dict(M=6, n_steps=30), cfg4=dict(M=2, N=7, n_steps=60),
+                 cfg5=dict(M=5, n_steps=40))[name]
+    wl = W.make(name, seed=2, **small)
+
+    from util import fresh_oracle, split_calls
+    rec_every = max(wl.record_every, 1)
+    a = fresh_oracle(cfo, wl)
+    ra = a.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every)
+    b = fresh_oracle(cfo, wl)
+    recs = []
+    for cm, n, hold in split_calls(wl, [1, 2, 7, 13]):
+        r = b.step(cm, n, cmd_hold=hold, record_every=rec_every)
+        if r is not None:
+            recs.append(r)
+    assert np.array_equal(np.concatenate(recs), ra)
+    assert np.array_equal(a.get_state(), b.get_state())
+    assert np.array_equal(a.ctrl(), b.ctrl())
+    assert np.array_equal(a.counters(), b.counters())
+    assert np.array_equal(a.rec_table(), b.rec_table())
+    if wl.params.get("n_obstacles"):
+        assert np.array_equal(a.min_dist(), b.min_dist())
+
+
+def test_record_slots_counters_and_errors(cfo):
+    sim = cfo.OracleSim(3, 2, 0, dict(integrator=0))
+    cm = np.zeros((1, 6, 4), dtype=np.float32)
+    rc, _ = sim.step(cm, 1, check=False)
+    assert rc == -3                                            # step before reset
+    sim.reset(1)
+    r1 = sim.step(cm, 7, cmd_hold=7, record_every=3)          # s: 0 -> 7, records at 3, 6
+    r2 = sim.step(cm, 5, cmd_hold=5, record_every=3)          # s: 7 -> 12, records at 9, 12
+    assert r1.shape == (2, 17, 6) and r2.shape == (2, 17, 6)
+    assert list(sim.rec_table()[:5]) == [3, 6, 9, 12, 0]
+    assert list(sim.counters()) == [12, 6, 0, 4]
+    rc, _ = sim.step(cm, 8, cmd_hold=7, check=False)
+    assert rc == -2                                            # not enough commands
+    with pytest.raises(ValueError):
+        cfo.OracleSim(1, 1, 0, dict(f_att=300.0))              # 1000/300 not an integer
+    with pytest.raises(ValueError):
+        cfo.OracleSim(1, 1, 1, dict(iface=cfo.IF_ROTOR))       # abstracted model has no rotors
+
+
+def test_reset_distributions_and_world_offset(cfo):
+    from paper_2606_01478_b200 import workloads as W
+    wl = W.cfg2(seed=7, M=512, n_steps=50)
+    sim = cfo.OracleSim(wl.M, 1, wl.model, wl.params)
+    sim.reset(wl.seed)
+    x = sim.get_state()
+    assert x[0].min() >= -1 and x[0].max() <= 1 and x[2].min() >= 0 and x[2].max() <= 2
+    assert abs(x[0].mean()) < 0.12 and abs(x[2].mean() - 1) < 0.12
+    np.testing.assert_allclose(np.linalg.norm(x[3:7], axis=0), 1, atol=1e-15)
+    ang = 2 * np.arccos(np.clip(x[6], -1, 1))
+    assert ang.max() <= 0.5 and ang.min() >= 0 and abs(ang.mean() - 0.25) < 0.03     # R19: angle ~ U[0, 0.5]
+    ax = x[3:6] / np.linalg.norm(x[3:6], axis=0)
+    assert np.abs(ax.mean(axis=1)).max() < 0.12                                       # axis uniform on the sphere
+    np.testing.assert_allclose(x[13:], W_HOVER, rtol=1e-15)
+    # sharding: worlds [200, 328) of the same seed reproduce that slice exactly
+    sub = cfo.OracleSim(128, 1, wl.model, dict(wl.params, world_offset=200))
+    sub.reset(wl.seed)
+    assert np.array_equal(sub.get_state(), x[:, 200:328])
+    # cfg5 parameter jitter: factors uniform in their ranges, k_m untouched
+    w5 = W.cfg5(seed=7, M=2000, n_steps=10)
+    s5 = cfo.OracleSim(w5.M, 1, w5.model, w5.params)
+    s5.reset(7)
+    wp = s5.world_params()
+    fm, fk = wp[0] / M_, wp[6] / KF
+    assert 0.9 <= fm.min() and fm.max() <= 1.1 and abs(fm.mean() - 1) < 0.01 and abs(fm.std() - 0.2 / math.sqrt(12)) < 0.004
+    assert 0.95 <= fk.min() and fk.max() <= 1.05 and abs(fk.std() - 0.1 / math.sqrt(12)) < 0.002
+    assert np.all(wp[9] == KM) and np.all(wp[4] == 0) and np.all(wp[10] == 1 / 0.03)
+    assert abs(np.corrcoef(wp[1], wp[2])[0, 1]) < 0.08                                # R17: independent per axis
+    # cfg4 grid placement
+    w4 = W.cfg4(seed=7, M=2, N=600, n_steps=10)
+    s4 = cfo.OracleSim(2, 600, w4.model, w4.params)
+    s4.reset(7)
+    x4 = s4.get_state()
+    n = np.arange(600)
+    cell = np.stack([n % 16, (n // 16) % 16, n // 256])
+    centre = np.array([[-2.25], [-2.25], [0.5]]) + 0.3 * cell
+    assert np.abs(x4[0:3, :600] - centre).max() <= 0.02 and np.abs(x4[0:3, 600:] - centre).max() <= 0.02
+    assert not np.array_equal(x4[0:3, :600], x4[0:3, 600:])
+    wm = s4.world_params()[0]
+    assert 0.025 <= wm.min() and wm.max() <= 0.032 and wm[0] != wm[1]
+
+
+def test_p13_first_principles_roll_step_resembles_identified_response(cfo):
+    """Soft sanity (not a tolerance test): with the C5 gains a 0.2 rad roll step on the FP model behaves like
+    Eq. (10) with (-130,-16,130): settles near 0.2 rad within 0.5 s with modest overshoot."""
+    sim = cfo.OracleSim(1, 1, 0, dict(integrator=1))
+    sim.reset(0)
+    rec = sim.step(cmd1([0.2, 0, 0, M_ * G_ / math.cos(0.2)]), 700, cmd_hold=700, record_every=1)
+    roll = Rotation.from_quat(rec[:, 3:7, 0]).as_euler("xyz")[:, 0]
+    assert 0.2 < roll.max() < 0.2 * 1.35
+    assert np.abs(roll[500:] - 0.2).max() < 0.02
