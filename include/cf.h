@@ -1,0 +1,183 @@
+/* cf.h -- C ABI of libcf.so: the batched quadrotor simulation step of Crazyflow
+ * (arxiv/paper_2606_01478) as hand-written sm_100a CUDA kernels.
+ *
+ * The calls follow the paper's problem statement: a simulator object holding M_worlds x N_drones drones
+ * (PAPER.md:L23, L264), a control-interface level, stepping n steps at once (the XLA scan of
+ * PAPER.md:L264 becomes one kernel launch with the state held in registers), and resets.
+ * BASELINE.json:north_star names the four mandatory calls: cf_create, cf_reset, cf_step, cf_get_state.
+ *
+ * GENERAL RULES
+ *  - Every function returns CF_OK (0) or a negative cf_status; none throws, aborts or prints.  cf_last_error()
+ *    returns a thread-local description of the last failure.
+ *  - Ownership: the CALLER owns every device byte (workspace, commands, records, outputs).  The library owns only
+ *    the host handle and never allocates device memory.  Pointers named *_dev are device pointers, *_host are host
+ *    pointers (pinned memory makes the copies asynchronous to the host but the *_host calls still synchronise the
+ *    stream before returning).
+ *  - Asynchrony: all *_dev calls enqueue on the bound CUDA stream (cf_set_stream, default stream 0) and return; there
+ *    is no implicit synchronisation.  Launch errors are caught with cudaGetLastError -> CF_E_CUDA.
+ *  - There is no CPU path: an unsupported combination returns CF_E_UNSUPPORTED.
+ *
+ * LAYOUTS (float32, component-major "planes"; i = w*N + n is the flat drone index, MN = M*N)
+ *   state  [D][MN]     D = 17 first-principles: p(0-2) q(3-6; x y z w, scalar-last)
+ *                                                               v(7-9) omega_body(10-12) Omega(13-16, rpm)
+ *                      D = 13 abstracted:       p(0-2) Psi(3-5 roll pitch yaw) v(6-8) dPsi(9-11) f_Sigma(12)
+ *   record [n_rec][D][MN]
+ *   cmds   [K][MN] of float4 (CF_CMD_BUFFER) or [K] of float4 (CF_CMD_NOMINAL_PLUS_NOISE), 16-byte aligned:
+ *            attitude (roll, pitch, yaw [rad], collective thrust [N]);  position (x, y, z [m], yaw [rad]);
+ *            rotor (4 x rpm);  torque (tau_x, tau_y, tau_z [N m], collective thrust [N])
+ *   ctrl   [14][MN]    i_R(0-2) i_p(3-5) held attitude cmd(6-9) held rotor cmd(10-13)
+ *   wparam [P][M]      P = 14 FP: m Jx Jy Jz kf0 kf1 kf2 km0 km1 km2 cv_up cv_dn cd_up cd_dn;  P = 11 AB: m a[3] b[3] c[3] c_tau
+ *
+ * STEP SEMANTICS.  The simulator keeps a global step counter s
+ * (uint32, 0 after reset).  For each of the n_steps physics steps of length 1/f_phys:
+ *   (1) if (s - s0) % cmd_hold == 0 the command with index (s - s0)/cmd_hold is fetched (or formed from
+ *       nominal + Philox noise);  (2) position-controller tick if s % (f_phys/f_pos) == 0;  (3) attitude-controller
+ *       tick + motor mixer if s % (f_phys/f_att) == 0 (first-principles model);  (4) disturbance draw for this s;
+ *   (5) explicit Euler or classical RK4 step with the inputs held, then quaternion renormalisation;  (6) s += 1;
+ *   (7) obstacle minima updated with the new position;  (8) if record_every > 0 and s % record_every == 0 the state
+ *       is written to record slot  s/record_every - s0/record_every - 1.
+ * Controller ticks, record slots and Philox counters depend only on the global s, so one fused call and any split
+ * into shorter calls (down to n_steps = 1, the interactive mode) give the same trajectory.
+ */
+#ifndef CF_H
+#define CF_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cf_sim cf_sim;   /* opaque host handle */
+
+typedef enum {
+  CF_OK = 0,
+  CF_E_ARG = -1,          /* NULL / out-of-range argument */
+  CF_E_SHAPE = -2,        /* sizes inconsistent (M*N >= 2^31, too few commands, non-integer rate ratio) */
+  CF_E_STATE = -3,        /* cf_step / cf_set_state before the first cf_reset */
+  CF_E_BUFFER = -4,       /* caller buffer too small or misaligned */
+  CF_E_CUDA = -5,         /* CUDA runtime error (text in cf_last_error) */
+  CF_E_UNSUPPORTED = -6   /* combination not built (e.g. rotor interface with the abstracted model) */
+} cf_status;
+
+enum { CF_MODEL_FIRST_PRINCIPLES = 0, CF_MODEL_ABSTRACTED = 1 };          /* PAPER.md:L296 / L334 */
+enum { CF_EULER = 0, CF_RK4 = 1 };                                        /* BASELINE.json:configs */
+enum { CF_IF_ROTOR = 0, CF_IF_TORQUE = 1, CF_IF_ATTITUDE = 2, CF_IF_POSITION = 3 };
+enum { CF_CMD_BUFFER = 0, CF_CMD_NOMINAL_PLUS_NOISE = 1 };
+enum { CF_AUX_COUNTERS = 0,      /* uint32[4]: s, attitude ticks, position ticks, records written */
+       CF_AUX_MIN_DIST = 1,      /* float[M]: min over steps, drones of the world and obstacles of |p - c_j| - r_j */
+       CF_AUX_CTRL = 2,          /* float[14][MN] */
+       CF_AUX_WORLD_PARAMS = 3,  /* float[P][M] */
+       CF_AUX_REC_TABLE = 4,     /* uint32[CF_REC_TABLE_CAP]: record slot (since reset) -> step counter */
+       CF_AUX_MIN_D2 = 5 };      /* float[8][MN]: running minimum squared centre distance per obstacle */
+#define CF_REC_TABLE_CAP 4096
+#define CF_MAX_OBSTACLES 8
+
+/* POD parameter block.  cf_default_params() fills the values of BASELINE.json:configs[0] / configs[2] and the
+ * readings of DESIGN.md (limits, controller gains).  struct_size must equal sizeof(cf_params). */
+typedef struct cf_params {
+  uint32_t struct_size;
+  int32_t  integrator, iface, cmd_source;
+  int32_t  ab_thrust_dyn;            /* 1: Eq. (9) thrust lag; 0: f_Sigma == f_cmd (simplified model) */
+  int32_t  init_mode;                /* 0 fixed (p = p0_lo, level), 1 uniform box + random axis-angle tilt, 2 grid */
+  int32_t  grid_dims[3];
+  int32_t  n_obstacles;              /* 0..8; > 0 switches the running minimum distance on */
+  int64_t  world_offset;             /* global index of local world 0: Philox is keyed by the global world index,
+                                        so a shard of worlds reproduces the same slice of the full run */
+  float f_phys, f_att, f_pos;        /* Hz; f_phys/f_att and f_phys/f_pos must be integers >= 1 */
+  /* plant, nominal (Eqs. (1)-(6)); rotor speeds in rpm */
+  float mass, J[3], arm, kf[3], km[3] /* c0 + c1 W + c2 W^2 */, g;
+  float cv_up, cv_dn, cd_up, cd_dn;  /* Eq. (6): accelerate / decelerate coefficients */
+  float Jp, Ca[3];                   /* Eq. (5) rotor inertia, body drag; 0 = off */
+  /* abstracted model, Eqs. (7)-(10) */
+  float ab_a[3], ab_b[3], ab_c[3], ab_ctau, ab_cf;
+  /* limits */
+  float rpm_min, rpm_max, thrust_min, thrust_max, tilt_max;
+  /* attitude controller (C5) and position controller (C7) */
+  float kR[3], kW[3], kI[3], iR_max;
+  float kp[3], kd[3], ki[3], ip_max[3];
+  /* per-world multiplicative randomisation U[lo,hi] per slot (lo = hi = 1: off).
+   * FP slots: 0 m, 1-3 J, 4 k_f, 5 k_m, 6 motor time constant.  AB slots: 0 m, 1-3 a, 4-6 b, 8-10 c, 11 c_tau. */
+  float rnd_lo[12], rnd_hi[12];
+  float dist_sigma;                  /* per-step Gaussian force disturbance [N], world frame; 0 = off */
+  /* reset */
+  float p0_lo[3], p0_hi[3], tilt0_max;
+  float grid_spacing, grid_jitter, grid_origin[3];
+  /* planning rollouts (config 3) */
+  float obstacles[CF_MAX_OBSTACLES][4];   /* cx cy cz r */
+  float noise_sigma[4], cmd_lo[4], cmd_hi[4];
+} cf_params;
+
+/* Fill *p with the defaults for `model`.  Host only. */
+void cf_default_params(cf_params *p, int model);
+int  cf_state_dim(int model);          /* 17 / 13 */
+int  cf_world_param_dim(int model);    /* 14 / 11 */
+
+/* Bytes of device workspace cf_create needs for (M, N, model, p).  0 on invalid arguments. */
+size_t cf_workspace_bytes(int64_t M, int64_t N, int model, const cf_params *p);
+
+/* Create a simulator of M worlds x N drones.  workspace_dev: device memory of >= cf_workspace_bytes() bytes, 256-byte
+ * aligned, owned by the caller and kept alive until cf_destroy.  Validates p (CF_E_ARG / CF_E_SHAPE /
+ * CF_E_UNSUPPORTED), never touches the device. */
+int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf_params *p,
+              void *workspace_dev, size_t workspace_bytes);
+int cf_destroy(cf_sim *sim);
+
+/* Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) all later calls enqueue on. */
+int cf_set_stream(cf_sim *sim, void *cuda_stream);
+
+/* Draw the per-world parameters (Philox PARAM stream) and the initial state (INIT stream) from `seed`, zero the
+ * controller integrals, set the held commands to hover, re-arm the minimum distance, s = 0.  (C9) */
+int cf_reset(cf_sim *sim, uint64_t seed);
+
+/* Overwrite the drone states: state_dev is [D][MN], or [D] broadcast to every drone when broadcast != 0 (the MPPI
+ * "all rollouts start from the measured state" reset).  Keeps s and the world parameters; zeroes the
+ * controller integrals, re-arms the minimum distance, held commands = hover.  Needs a prior cf_reset. */
+int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast);
+
+/* Teacher forcing / checkpoint restore: overwrite any of state [D][MN], ctrl [14][MN], wparam [P][M],
+ * min_d2 [8][MN] (NULL = keep) and, if step_counter >= 0, the global step counter. */
+int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctrl_dev, const float *wparam_dev,
+                const float *min_d2_dev, int64_t step_counter);
+
+/* Advance n_steps >= 1 physics steps in ONE kernel launch (state in registers across all of them).
+ *   cmds_dev     [n_cmds][MN] float4, or [n_cmds] float4 for CF_CMD_NOMINAL_PLUS_NOISE; n_cmds*cmd_hold >= n_steps
+ *   record_every 0: nothing recorded; else see STEP SEMANTICS; record_dev must hold
+ *                n_rec = (s0+n_steps)/record_every - s0/record_every slots of D*MN floats (else CF_E_BUFFER). */
+int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold,
+            int n_steps, int record_every, float *record_dev, size_t record_bytes);
+
+/* The same step driven from HOST buffers (the end-to-end path): copies the commands host->device into staging_dev,
+ * runs cf_step recording into staging_dev, copies the records device->host, synchronises the stream.
+ * staging_dev must hold cf_staging_bytes(...) bytes (caller-owned device scratch). */
+size_t cf_staging_bytes(const cf_sim *sim, int n_cmds, int n_steps, int record_every);
+int cf_step_host(cf_sim *sim, const void *cmds_host, int n_cmds, int cmd_hold,
+                 int n_steps, int record_every, float *record_host, size_t record_bytes,
+                 void *staging_dev, size_t staging_bytes);
+
+/* Copy the state planes [D][MN] to out_dev (device, on the stream) / out_host (host, synchronises). */
+int cf_get_state(cf_sim *sim, float *out_dev);
+int cf_get_state_host(cf_sim *sim, float *out_host);
+
+/* Auxiliary outputs, see CF_AUX_*.  The _host variant needs device scratch only for CF_AUX_MIN_DIST (M floats). */
+int cf_get_aux(cf_sim *sim, int which, void *out_dev);
+int cf_get_aux_host(cf_sim *sim, int which, void *out_host, void *scratch_dev, size_t scratch_bytes);
+
+/* Host mirror of the step counter.  It advances with every cf_step CALL; after replaying a captured CUDA graph call
+ * cf_sync_counters (synchronises the stream and re-reads the device counter). */
+int64_t cf_step_counter(const cf_sim *sim);
+int cf_sync_counters(cf_sim *sim);
+
+/* Name of the kernel instantiation the next cf_step would launch and its launch geometry (for profiling notes). */
+int cf_describe_launch(const cf_sim *sim, char *buf, size_t buf_len, int *grid, int *block);
+
+const char *cf_last_error(void);
+/* Host-side Philox4x32-10 of this library, for the bit-exact check against the oracle's (C9). */
+int cf_debug_philox(uint64_t seed, const uint32_t ctr[4], uint32_t out[4]);
+/* Device-side Philox4x32-10 + uniform + Box-Muller as the kernels use them: n counters -> n x 4 words, uniforms, normals */
+int cf_debug_philox_dev(cf_sim *sim, uint64_t seed, const uint32_t *ctr_dev, int n,
+                        uint32_t *words_dev, float *uniform_dev, float *normal_dev);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

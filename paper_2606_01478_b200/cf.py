@@ -1,0 +1,320 @@
+"""Thin Python binding of libcf.so (include/cf.h): argument marshalling only.
+
+PyTorch is used for device memory (`torch.empty`) and the current CUDA stream; every step of the path runs in the
+library's own kernels.  There is no fallback: if libcf.so is missing this module raises on first use.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcf.so")
+
+MODEL_FP, MODEL_AB = 0, 1
+EULER, RK4 = 0, 1
+IF_ROTOR, IF_TORQUE, IF_ATTITUDE, IF_POSITION = 0, 1, 2, 3
+CMD_BUFFER, CMD_NOMINAL_PLUS_NOISE = 0, 1
+AUX_COUNTERS, AUX_MIN_DIST, AUX_CTRL, AUX_WORLD_PARAMS, AUX_REC_TABLE, AUX_MIN_D2 = range(6)
+REC_TABLE_CAP = 4096
+OK, E_ARG, E_SHAPE, E_STATE, E_BUFFER, E_CUDA, E_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+
+f = C.c_float
+
+
+class Params(C.Structure):
+    """Mirror of `cf_params` (include/cf.h)."""
+    _fields_ = [
+        ("struct_size", C.c_uint32),
+        ("integrator", C.c_int32), ("iface", C.c_int32), ("cmd_source", C.c_int32),
+        ("ab_thrust_dyn", C.c_int32), ("init_mode", C.c_int32), ("grid_dims", C.c_int32 * 3),
+        ("n_obstacles", C.c_int32), ("world_offset", C.c_int64),
+        ("f_phys", f), ("f_att", f), ("f_pos", f),
+        ("mass", f), ("J", f * 3), ("arm", f), ("kf", f * 3), ("km", f * 3), ("g", f),
+        ("cv_up", f), ("cv_dn", f), ("cd_up", f), ("cd_dn", f),
+        ("Jp", f), ("Ca", f * 3),
+        ("ab_a", f * 3), ("ab_b", f * 3), ("ab_c", f * 3), ("ab_ctau", f), ("ab_cf", f),
+        ("rpm_min", f), ("rpm_max", f), ("thrust_min", f), ("thrust_max", f), ("tilt_max", f),
+        ("kR", f * 3), ("kW", f * 3), ("kI", f * 3), ("iR_max", f),
+        ("kp", f * 3), ("kd", f * 3), ("ki", f * 3), ("ip_max", f * 3),
+        ("rnd_lo", f * 12), ("rnd_hi", f * 12),
+        ("dist_sigma", f),
+        ("p0_lo", f * 3), ("p0_hi", f * 3), ("tilt0_max", f),
+        ("grid_spacing", f), ("grid_jitter", f), ("grid_origin", f * 3),
+        ("obstacles", (f * 4) * 8),
+        ("noise_sigma", f * 4), ("cmd_lo", f * 4), ("cmd_hi", f * 4),
+    ]
+
+
+class CfError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"cf status {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libcf.so (fails loudly if it was not built: there is no CPU path)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_01478_b200.build` "
+                          "(or __graft_entry__.build()); this package has no CPU fallback")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, sz = C.c_void_p, C.c_int64, C.c_size_t
+    sig = {
+        "cf_default_params": (None, [C.POINTER(Params), C.c_int]),
+        "cf_state_dim": (C.c_int, [C.c_int]),
+        "cf_world_param_dim": (C.c_int, [C.c_int]),
+        "cf_workspace_bytes": (sz, [i64, i64, C.c_int, C.POINTER(Params)]),
+        "cf_create": (C.c_int, [C.POINTER(vp), i64, i64, C.c_int, C.POINTER(Params), vp, sz]),
+        "cf_destroy": (C.c_int, [vp]),
+        "cf_set_stream": (C.c_int, [vp, vp]),
+        "cf_reset": (C.c_int, [vp, C.c_uint64]),
+        "cf_set_state": (C.c_int, [vp, vp, C.c_int]),
+        "cf_set_full": (C.c_int, [vp, vp, vp, vp, vp, i64]),
+        "cf_step": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, sz]),
+        "cf_staging_bytes": (sz, [vp, C.c_int, C.c_int, C.c_int]),
+        "cf_step_host": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, sz, vp, sz]),
+        "cf_get_state": (C.c_int, [vp, vp]),
+        "cf_get_state_host": (C.c_int, [vp, vp]),
+        "cf_get_aux": (C.c_int, [vp, C.c_int, vp]),
+        "cf_get_aux_host": (C.c_int, [vp, C.c_int, vp, vp, sz]),
+        "cf_step_counter": (i64, [vp]),
+        "cf_sync_counters": (C.c_int, [vp]),
+        "cf_describe_launch": (C.c_int, [vp, C.c_char_p, sz, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+        "cf_last_error": (C.c_char_p, []),
+        "cf_debug_philox": (C.c_int, [C.c_uint64, C.POINTER(C.c_uint32 * 4), C.POINTER(C.c_uint32 * 4)]),
+        "cf_debug_philox_dev": (C.c_int, [vp, C.c_uint64, vp, C.c_int, vp, vp, vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_workspace_bytes", "cf_create", "cf_destroy",
+           "cf_set_stream", "cf_reset", "cf_set_state", "cf_set_full", "cf_step", "cf_staging_bytes", "cf_step_host",
+           "cf_get_state", "cf_get_state_host", "cf_get_aux", "cf_get_aux_host", "cf_step_counter", "cf_sync_counters",
+           "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev"]
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise CfError(rc, lib().cf_last_error().decode())
+
+
+def _assign(struct, key, val):
+    cur = getattr(struct, key)
+    if not isinstance(cur, C.Array):
+        setattr(struct, key, val)
+        return
+    flat = np.asarray(val).reshape(-1).tolist()
+    if isinstance(cur[0], C.Array):
+        inner = len(cur[0])
+        if len(flat) % inner or len(flat) > inner * len(cur):
+            raise ValueError(f"{key}: bad size {len(flat)}")
+        for r in range(len(flat) // inner):
+            for c_ in range(inner):
+                cur[r][c_] = flat[r * inner + c_]
+    else:
+        if len(flat) != len(cur):
+            raise ValueError(f"{key}: expected {len(cur)} values, got {len(flat)}")
+        for j, v in enumerate(flat):
+            cur[j] = v
+
+
+def default_params(model: int, overrides: dict | None = None) -> Params:
+    p = Params()
+    lib().cf_default_params(C.byref(p), model)
+    for k, v in (overrides or {}).items():
+        _assign(p, k, v)
+    return p
+
+
+def debug_philox(seed: int, ctr) -> np.ndarray:
+    c = (C.c_uint32 * 4)(*[int(v) for v in ctr])
+    o = (C.c_uint32 * 4)()
+    _check(lib().cf_debug_philox(seed, C.byref(c), C.byref(o)))
+    return np.array(list(o), dtype=np.uint32)
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class Sim:
+    """cf_create / cf_reset / cf_step / cf_get_state with torch tensors as the caller-owned device buffers."""
+
+    def __init__(self, M: int, N: int, model: int, overrides: dict | None = None, device="cuda:0"):
+        torch = _torch()
+        self.M, self.N, self.model = int(M), int(N), int(model)
+        self.MN = self.M * self.N
+        self.D = lib().cf_state_dim(model)
+        self.P = lib().cf_world_param_dim(model)
+        self.params = default_params(model, overrides)
+        self.device = torch.device(device)
+        nbytes = lib().cf_workspace_bytes(self.M, self.N, model, C.byref(self.params))
+        self._h = C.c_void_p()
+        if nbytes == 0:      # let cf_create report why
+            _check(lib().cf_create(C.byref(self._h), self.M, self.N, model, C.byref(self.params), None, 0))
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-self.workspace.data_ptr()) % 256
+        self._ws_ptr = self.workspace.data_ptr() + off
+        _check(lib().cf_create(C.byref(self._h), self.M, self.N, model, C.byref(self.params),
+                               C.c_void_p(self._ws_ptr), nbytes))
+        self._staging = None
+        self.bind_stream()
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h is not None and h.value and _lib is not None:
+            _lib.cf_destroy(h)
+            self._h = C.c_void_p()
+
+    # -- plumbing ------------------------------------------------------------------------------------------------
+    def bind_stream(self, stream=None):
+        torch = _torch()
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        _check(lib().cf_set_stream(self._h, C.c_void_p(st.cuda_stream)))
+
+    def _dev(self, a, dtype=None):
+        torch = _torch()
+        if isinstance(a, torch.Tensor):
+            t = a.to(self.device)
+            return t.contiguous() if dtype is None else t.to(dtype).contiguous()
+        return torch.as_tensor(np.ascontiguousarray(a), device=self.device).to(dtype or torch.float32).contiguous()
+
+    def describe_launch(self):
+        buf = C.create_string_buffer(256)
+        g, b = C.c_int(), C.c_int()
+        _check(lib().cf_describe_launch(self._h, buf, 256, C.byref(g), C.byref(b)))
+        return buf.value.decode(), g.value, b.value
+
+    # -- the four calls ------------------------------------------------------------------------------------------
+    def reset(self, seed: int):
+        _check(lib().cf_reset(self._h, int(seed)))
+
+    def set_state(self, state, broadcast: bool = False):
+        t = self._dev(state, _torch().float32)
+        assert t.numel() == (self.D if broadcast else self.D * self.MN)
+        _check(lib().cf_set_state(self._h, _dptr(t), int(broadcast)))
+
+    def set_full(self, state=None, ctrl=None, wparam=None, min_d2=None, step_counter=-1):
+        f32 = _torch().float32
+        ts = [None if a is None else self._dev(a, f32) for a in (state, ctrl, wparam, min_d2)]
+        for t, n in zip(ts, (self.D * self.MN, 14 * self.MN, self.P * self.M, 8 * self.MN)):
+            assert t is None or t.numel() == n
+        _check(lib().cf_set_full(self._h, *[_dptr(t) for t in ts], int(step_counter)))
+
+    def n_records(self, n_steps: int, record_every: int) -> int:
+        if record_every <= 0:
+            return 0
+        s0 = self.step_counter
+        return (s0 + n_steps) // record_every - s0 // record_every
+
+    def step(self, cmds, n_steps: int, cmd_hold: int = 1, record_every: int = 0, record=None):
+        """cmds: device tensor float32 [K][MN][4] (or [K][4] for nominal+noise).  Returns the record tensor
+        [n_rec][D][MN] (allocated here unless `record` is given) or None.  Asynchronous on the bound stream."""
+        torch = _torch()
+        cm = self._dev(cmds, torch.float32)
+        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4
+        assert cm.numel() % per == 0, (tuple(cm.shape), per)
+        n_rec = self.n_records(n_steps, record_every)
+        if n_rec and record is None:
+            record = torch.empty((n_rec, self.D, self.MN), dtype=torch.float32, device=self.device)
+        _check(lib().cf_step(self._h, _dptr(cm), cm.numel() // per, int(cmd_hold), int(n_steps), int(record_every),
+                             _dptr(record) if n_rec else None, record.numel() * 4 if n_rec else 0))
+        return record[:n_rec] if n_rec else None
+
+    def get_state(self):
+        out = _torch().empty((self.D, self.MN), dtype=_torch().float32, device=self.device)
+        _check(lib().cf_get_state(self._h, _dptr(out)))
+        return out
+
+    # -- host-buffer (end-to-end) path ---------------------------------------------------------------------------
+    def step_host(self, cmds_host, n_steps: int, cmd_hold: int = 1, record_every: int = 0, record_host=None):
+        """cmds_host / record_host: CPU tensors (pinned for full speed).  Synchronous."""
+        torch = _torch()
+        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4
+        assert cmds_host.dtype == torch.float32 and cmds_host.is_contiguous() and not cmds_host.is_cuda
+        n_cmds = cmds_host.numel() // per
+        need = lib().cf_staging_bytes(self._h, n_cmds, int(n_steps), int(record_every))
+        if self._staging is None or self._staging.numel() < need + 256:
+            self._staging = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+        sp = self._staging.data_ptr() + (-self._staging.data_ptr()) % 256
+        n_rec = self.n_records(n_steps, record_every)
+        if n_rec and record_host is None:
+            record_host = torch.empty((n_rec, self.D, self.MN), dtype=torch.float32, pin_memory=True)
+        _check(lib().cf_step_host(self._h, C.c_void_p(cmds_host.data_ptr()), n_cmds, int(cmd_hold), int(n_steps),
+                                  int(record_every), C.c_void_p(record_host.data_ptr()) if n_rec else None,
+                                  record_host.numel() * 4 if n_rec else 0, C.c_void_p(sp), need))
+        return record_host[:n_rec] if n_rec else None
+
+    def get_state_host(self, out=None):
+        torch = _torch()
+        if out is None:
+            out = torch.empty((self.D, self.MN), dtype=torch.float32, pin_memory=True)
+        _check(lib().cf_get_state_host(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def min_dist_host(self, out=None):
+        torch = _torch()
+        if out is None:
+            out = torch.empty(self.M, dtype=torch.float32, pin_memory=True)
+        scratch = torch.empty(self.M, dtype=torch.float32, device=self.device)
+        _check(lib().cf_get_aux_host(self._h, AUX_MIN_DIST, C.c_void_p(out.data_ptr()), _dptr(scratch), self.M * 4))
+        return out
+
+    # -- auxiliary outputs ---------------------------------------------------------------------------------------
+    def _aux(self, which, shape, dtype):
+        out = _torch().empty(shape, dtype=dtype, device=self.device)
+        _check(lib().cf_get_aux(self._h, which, _dptr(out)))
+        return out
+
+    def counters(self):
+        return self._aux(AUX_COUNTERS, (4,), _torch().int32).cpu().numpy().view(np.uint32)
+
+    def min_dist(self):
+        return self._aux(AUX_MIN_DIST, (self.M,), _torch().float32)
+
+    def ctrl(self):
+        return self._aux(AUX_CTRL, (14, self.MN), _torch().float32)
+
+    def world_params(self):
+        return self._aux(AUX_WORLD_PARAMS, (self.P, self.M), _torch().float32)
+
+    def min_d2(self):
+        return self._aux(AUX_MIN_D2, (8, self.MN), _torch().float32)
+
+    def rec_table(self):
+        return self._aux(AUX_REC_TABLE, (REC_TABLE_CAP,), _torch().int32).cpu().numpy().view(np.uint32)
+
+    @property
+    def step_counter(self) -> int:
+        return int(lib().cf_step_counter(self._h))
+
+    def sync_counters(self):
+        _check(lib().cf_sync_counters(self._h))
+
+    def philox_dev(self, seed: int, ctr: np.ndarray):
+        """ctr: uint32 [n][4] -> (words uint32 [n][4], uniforms f32 [n][4], normals f32 [n][4]) from the device code."""
+        torch = _torch()
+        c = torch.as_tensor(np.ascontiguousarray(ctr, dtype=np.uint32).view(np.int32), device=self.device)
+        n = c.shape[0]
+        words = torch.empty((n, 4), dtype=torch.int32, device=self.device)
+        uni = torch.empty((n, 4), dtype=torch.float32, device=self.device)
+        nrm = torch.empty((n, 4), dtype=torch.float32, device=self.device)
+        _check(lib().cf_debug_philox_dev(self._h, int(seed), _dptr(c), n, _dptr(words), _dptr(uni), _dptr(nrm)))
+        return words.cpu().numpy().view(np.uint32), uni.cpu().numpy(), nrm.cpu().numpy()

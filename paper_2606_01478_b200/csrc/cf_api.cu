@@ -1,0 +1,626 @@
+// cf_api.cu -- the C ABI of include/cf.h: argument checking, workspace carving, kernel dispatch, and the small
+// non-hot kernels (reset, set_state, minimum-distance read-out, Philox debug).  No device allocation, no CPU path.
+#include "../../include/cf.h"
+#include "cf_device.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace cf;
+
+struct cf_sim {
+  long long M, N, MN;
+  int model, D, P;
+  cf_params p;
+  DevParams dp;
+  int opt;                    // option bits this configuration needs
+  // workspace carving (device pointers into the caller's buffer)
+  float *state, *ctrl, *wparam, *min_d2;
+  Counters *counters;
+  uint32_t *rec_table;
+  cudaStream_t stream;
+  uint64_t seed;
+  long long s_host;           // host mirror of the step counter
+  long long n_rec_host;
+  bool have_state;
+  float hover_rpm;
+};
+
+static thread_local char g_err[512] = "";
+static int fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+#define CF_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) \
+  return fail(CF_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+
+extern "C" const char *cf_last_error(void) { return g_err; }
+extern "C" int cf_state_dim(int model) { return model == CF_MODEL_FIRST_PRINCIPLES ? 17 : model == CF_MODEL_ABSTRACTED ? 13 : 0; }
+extern "C" int cf_world_param_dim(int model) { return model == CF_MODEL_FIRST_PRINCIPLES ? 14 : model == CF_MODEL_ABSTRACTED ? 11 : 0; }
+
+// BASELINE.json:configs[0], configs[2]; limits / gains: DESIGN.md readings R7, R12, R16
+extern "C" void cf_default_params(cf_params *p, int model) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->struct_size = (uint32_t)sizeof(cf_params);
+  p->integrator = CF_EULER; p->iface = CF_IF_ATTITUDE; p->cmd_source = CF_CMD_BUFFER;
+  p->ab_thrust_dyn = 1;
+  p->grid_dims[0] = p->grid_dims[1] = p->grid_dims[2] = 1;
+  p->f_phys = model == CF_MODEL_FIRST_PRINCIPLES ? 1000.f : 500.f; p->f_att = 500.f; p->f_pos = 100.f;
+  p->mass = 0.027f; p->J[0] = 1.395e-5f; p->J[1] = 1.395e-5f; p->J[2] = 2.173e-5f; p->arm = 0.046f;
+  p->kf[2] = 3.16e-10f; p->km[2] = 7.94e-12f; p->g = 9.81f;
+  p->cv_up = p->cv_dn = (float)(1.0 / 0.03);
+  for (int j = 0; j < 3; ++j) { p->ab_a[j] = -130.f; p->ab_b[j] = -16.f; p->ab_c[j] = 130.f; }
+  p->ab_ctau = (float)(1.0 / 0.03); p->ab_cf = 1.f;
+  p->rpm_min = 0.f; p->rpm_max = 21700.f; p->thrust_min = 0.f; p->thrust_max = 0.55f; p->tilt_max = 0.5f;
+  for (int j = 0; j < 3; ++j) { p->kR[j] = 130.f; p->kW[j] = 16.f; }
+  p->kI[0] = 20.f; p->kI[1] = 20.f; p->kI[2] = 0.f; p->iR_max = 0.2f;
+  p->kp[0] = 8.f; p->kp[1] = 8.f; p->kp[2] = 12.f;
+  p->kd[0] = 5.f; p->kd[1] = 5.f; p->kd[2] = 7.f;
+  p->ki[0] = 1.f; p->ki[1] = 1.f; p->ki[2] = 6.f;
+  p->ip_max[0] = 0.25f; p->ip_max[1] = 0.25f; p->ip_max[2] = 0.4f;
+  for (int j = 0; j < 12; ++j) { p->rnd_lo[j] = 1.f; p->rnd_hi[j] = 1.f; }
+  p->p0_lo[2] = 1.f; p->p0_hi[2] = 1.f;
+  const float pi = 3.14159265358979323846f;
+  p->cmd_lo[0] = -0.5f; p->cmd_lo[1] = -0.5f; p->cmd_lo[2] = -pi; p->cmd_lo[3] = 0.05f;
+  p->cmd_hi[0] = 0.5f;  p->cmd_hi[1] = 0.5f;  p->cmd_hi[2] = pi;  p->cmd_hi[3] = 0.55f;
+}
+
+static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+
+struct Carve { size_t state, ctrl, wparam, min_d2, counters, rec_table, total; };
+static Carve carve(long long M, long long N, int model, const cf_params *p) {
+  Carve c;
+  size_t MN = (size_t)(M * N), off = 0;
+  c.state = off;     off += align256(sizeof(float) * cf_state_dim(model) * MN);
+  c.ctrl = off;      off += align256(sizeof(float) * kCtrlPlanes * MN);
+  c.wparam = off;    off += align256(sizeof(float) * cf_world_param_dim(model) * (size_t)M);
+  c.min_d2 = off;    off += p->n_obstacles > 0 ? align256(sizeof(float) * kMaxObst * MN) : 0;
+  c.counters = off;  off += align256(sizeof(Counters));
+  c.rec_table = off; off += align256(sizeof(uint32_t) * kRecTableCap);
+  c.total = off;
+  return c;
+}
+
+static int validate(long long M, long long N, int model, const cf_params *p) {
+  if (!p) return fail(CF_E_ARG, "params is NULL");
+  if (p->struct_size != sizeof(cf_params))
+    return fail(CF_E_ARG, "cf_params.struct_size %u != %zu", p->struct_size, sizeof(cf_params));
+  if (model != CF_MODEL_FIRST_PRINCIPLES && model != CF_MODEL_ABSTRACTED) return fail(CF_E_ARG, "bad model %d", model);
+  if (M < 1 || N < 1) return fail(CF_E_ARG, "M and N must be >= 1");
+  if (M > ((long long)1 << 31) || N > ((long long)1 << 31) || M * N >= ((long long)1 << 31))
+    return fail(CF_E_SHAPE, "M*N must be < 2^31");
+  if (p->integrator != CF_EULER && p->integrator != CF_RK4) return fail(CF_E_ARG, "bad integrator");
+  if (p->iface < CF_IF_ROTOR || p->iface > CF_IF_POSITION) return fail(CF_E_ARG, "bad iface");
+  if (p->cmd_source != CF_CMD_BUFFER && p->cmd_source != CF_CMD_NOMINAL_PLUS_NOISE) return fail(CF_E_ARG, "bad cmd_source");
+  if (!(p->f_phys > 0) || !(p->f_att > 0) || !(p->f_pos > 0)) return fail(CF_E_ARG, "rates must be > 0");
+  double ad = (double)p->f_phys / p->f_att, pd = (double)p->f_phys / p->f_pos;
+  if (ad < 1 || pd < 1 || ad != std::floor(ad) || pd != std::floor(pd))
+    return fail(CF_E_SHAPE, "f_phys/f_att and f_phys/f_pos must be integers >= 1");
+  if (model == CF_MODEL_ABSTRACTED && p->iface != CF_IF_ATTITUDE && p->iface != CF_IF_POSITION)
+    return fail(CF_E_UNSUPPORTED, "the abstracted model interfaces at the attitude or position level only");
+  if (p->n_obstacles < 0 || p->n_obstacles > CF_MAX_OBSTACLES) return fail(CF_E_ARG, "n_obstacles out of range");
+  if (p->init_mode < 0 || p->init_mode > 2) return fail(CF_E_ARG, "bad init_mode");
+  if (p->init_mode == 2 && (p->grid_dims[0] < 1 || p->grid_dims[1] < 1)) return fail(CF_E_ARG, "bad grid_dims");
+  if (!(p->mass > 0) || !(p->J[0] > 0) || !(p->J[1] > 0) || !(p->J[2] > 0)) return fail(CF_E_ARG, "mass/J must be > 0");
+  if (model == CF_MODEL_FIRST_PRINCIPLES && p->iface != CF_IF_ROTOR && !(p->kf[2] > 0))
+    return fail(CF_E_ARG, "controller needs kf[2] > 0");
+  if (p->world_offset < 0 || p->world_offset + M > ((long long)1 << 32)) return fail(CF_E_SHAPE, "world_offset out of range");
+  return CF_OK;
+}
+
+extern "C" size_t cf_workspace_bytes(int64_t M, int64_t N, int model, const cf_params *p) {
+  if (validate(M, N, model, p) != CF_OK) return 0;
+  return carve(M, N, model, p).total;
+}
+
+static double hover_rpm_nominal(const cf_params *p) {
+  double f = (double)p->mass * p->g / 4.0, k0 = p->kf[0], k1 = p->kf[1], k2 = p->kf[2];
+  if (!(k2 > 0)) return 0.0;
+  if (k0 == 0 && k1 == 0) return std::sqrt(f / k2);
+  double disc = k1 * k1 - 4 * k2 * (k0 - f);
+  return (-k1 + std::sqrt(disc > 0 ? disc : 0)) / (2 * k2);
+}
+
+static void fill_dev_params(cf_sim *s) {
+  const cf_params &p = s->p;
+  DevParams &d = s->dp;
+  memset(&d, 0, sizeof(d));
+  double h = 1.0 / p.f_phys;
+  d.att_div = (int)std::llround((double)p.f_phys / p.f_att);
+  d.pos_div = (int)std::llround((double)p.f_phys / p.f_pos);
+  d.h = (float)h; d.half_h = (float)(0.5 * h); d.h_sixth = (float)(h / 6.0);
+  d.h_att = (float)(d.att_div * h); d.h_pos = (float)(d.pos_div * h); d.g = p.g;
+  d.mass = p.mass; d.inv_mass = (float)(1.0 / p.mass);
+  double lever = (double)p.arm / std::sqrt(2.0);      // reading R6: arm is centre-to-rotor, X configuration
+  d.lever = (float)lever;
+  for (int j = 0; j < 3; ++j) {
+    d.J[j] = p.J[j]; d.inv_J[j] = (float)(1.0 / p.J[j]); d.kf[j] = p.kf[j]; d.km[j] = p.km[j]; d.Ca[j] = p.Ca[j];
+    d.ab_a[j] = p.ab_a[j]; d.ab_b[j] = p.ab_b[j]; d.ab_c[j] = p.ab_c[j];
+    d.kR[j] = p.kR[j]; d.kW[j] = p.kW[j]; d.kI[j] = p.kI[j]; d.Jnom[j] = p.J[j];
+    d.kp[j] = p.kp[j]; d.kd[j] = p.kd[j]; d.ki[j] = p.ki[j]; d.ip_max[j] = p.ip_max[j];
+  }
+  d.cv_up = p.cv_up; d.cv_dn = p.cv_dn; d.cd_up = p.cd_up; d.cd_dn = p.cd_dn;
+  d.Jp_rad = (float)((double)p.Jp * 2.0 * 3.14159265358979323846 / 60.0);
+  d.ab_ctau = p.ab_ctau; d.ab_cf = p.ab_cf; d.ab_thrust_dyn = p.ab_thrust_dyn;
+  d.thrust_poly = (p.kf[0] != 0.f || p.kf[1] != 0.f);
+  d.has_drag = (p.Ca[0] != 0.f || p.Ca[1] != 0.f || p.Ca[2] != 0.f);
+  d.has_gyro = p.Jp != 0.f;
+  d.inv_4lever = (float)(1.0 / (4.0 * lever));
+  if (p.kf[2] > 0) {
+    double kappa = (double)p.km[2] / p.kf[2];
+    d.inv_4kappa = kappa != 0 ? (float)(1.0 / (4.0 * kappa)) : 0.f;
+    d.inv_kf2 = (float)(1.0 / p.kf[2]);
+  }
+  d.f_rotor_max = (float)((double)p.kf[0] + (double)p.kf[1] * p.rpm_max + (double)p.kf[2] * p.rpm_max * p.rpm_max);
+  d.rpm_min = p.rpm_min; d.rpm_max = p.rpm_max; d.thrust_min = p.thrust_min; d.thrust_max = p.thrust_max;
+  d.tilt_max = p.tilt_max; d.iR_max = p.iR_max; d.dist_sigma = p.dist_sigma; d.n_obst = p.n_obstacles;
+  d.use_noise = p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE;
+  for (int j = 0; j < kMaxObst; ++j) for (int k = 0; k < 4; ++k) d.obst[j][k] = p.obstacles[j][k];
+  for (int k = 0; k < 4; ++k) { d.noise_sigma[k] = p.noise_sigma[k]; d.cmd_lo[k] = p.cmd_lo[k]; d.cmd_hi[k] = p.cmd_hi[k]; }
+}
+
+static int needed_opt(const cf_sim *s) {
+  const cf_params &p = s->p;
+  int opt = 0;
+  for (int j = 0; j < 12; ++j) if (p.rnd_lo[j] != 1.f || p.rnd_hi[j] != 1.f) opt |= OPT_RANDP;
+  if (p.dist_sigma > 0.f) opt |= OPT_DIST;
+  if (p.n_obstacles > 0) opt |= OPT_OBST;
+  if (p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE) opt |= OPT_NOISE;
+  bool extras = p.Jp != 0.f || p.Ca[0] != 0.f || p.Ca[1] != 0.f || p.Ca[2] != 0.f;
+  if (s->model == CF_MODEL_FIRST_PRINCIPLES)
+    extras = extras || p.cv_up != p.cv_dn || p.cd_up != 0.f || p.cd_dn != 0.f || p.kf[0] != 0.f || p.kf[1] != 0.f ||
+             p.km[0] != 0.f || p.km[1] != 0.f;
+  else
+    extras = extras || !p.ab_thrust_dyn;
+  if (extras) opt |= OPT_EXTRAS;
+  return opt;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Reset kernels (C9): PARAM stream -> per-world plant parameters, INIT stream -> initial state.
+struct ResetArgs {
+  float rnd_lo[12], rnd_hi[12];
+  float nominal[14];                 // nominal world-parameter row (FP: 14, AB: 11 used)
+  float p0_lo[3], p0_hi[3], tilt0_max, grid_spacing, grid_jitter, grid_origin[3];
+  int grid_dims[3], init_mode, model;
+  float hover_rpm, hover_thrust;
+  long long M, N, MN, world_offset;
+  uint32_t seed_lo, seed_hi;
+};
+
+__global__ void reset_params_kernel(float *wparam, const __grid_constant__ ResetArgs R) {
+  long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= R.M) return;
+  uint32_t wg = (uint32_t)(w + R.world_offset);
+  float fac[12];
+#pragma unroll
+  for (int b = 0; b < 3; ++b) {
+    uint32_t r[4];
+    philox4x32_10(R.seed_lo, R.seed_hi, wg, 0u, (uint32_t)b, STREAM_PARAM, r);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) fac[4 * b + k] = R.rnd_lo[4 * b + k] + (R.rnd_hi[4 * b + k] - R.rnd_lo[4 * b + k]) * u01(r[k]);
+  }
+  const long long M = R.M;
+  if (R.model == MODEL_FP) {   // reading R17: slots (m, Jx, Jy, Jz | k_f, k_m, tau_m, -)
+    wparam[w] = R.nominal[0] * fac[0];
+    for (int j = 0; j < 3; ++j) wparam[(1 + j) * M + w] = R.nominal[1 + j] * fac[1 + j];
+    for (int j = 0; j < 3; ++j) wparam[(4 + j) * M + w] = R.nominal[4 + j] * fac[4];
+    for (int j = 0; j < 3; ++j) wparam[(7 + j) * M + w] = R.nominal[7 + j] * fac[5];
+    for (int j = 0; j < 4; ++j) wparam[(10 + j) * M + w] = R.nominal[10 + j] / fac[6];
+  } else {                     // slots (m, a[3] | b[3], - | c[3], c_tau)
+    wparam[w] = R.nominal[0] * fac[0];
+    for (int j = 0; j < 3; ++j) wparam[(1 + j) * M + w] = R.nominal[1 + j] * fac[1 + j];
+    for (int j = 0; j < 3; ++j) wparam[(4 + j) * M + w] = R.nominal[4 + j] * fac[4 + j];
+    for (int j = 0; j < 3; ++j) wparam[(7 + j) * M + w] = R.nominal[7 + j] * fac[8 + j];
+    wparam[10 * M + w] = R.nominal[10] * fac[11];
+  }
+}
+
+// controller integrals 0, held commands = hover of the nominal model, min distance +inf (reading R20)
+__device__ __forceinline__ void rearm(float *ctrl, float *min_d2, long long MN, long long i, float hover_rpm,
+                                      float hover_thrust) {
+#pragma unroll
+  for (int c = 0; c < 9; ++c) ctrl[c * MN + i] = 0.f;
+  ctrl[9 * MN + i] = hover_thrust;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) ctrl[(10 + k) * MN + i] = hover_rpm;
+  if (min_d2) {
+#pragma unroll
+    for (int j = 0; j < kMaxObst; ++j) min_d2[j * MN + i] = __int_as_float(0x7f800000);
+  }
+}
+
+__global__ void reset_state_kernel(float *state, float *ctrl, float *min_d2, const __grid_constant__ ResetArgs R) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= R.MN) return;
+  long long w = i / R.N, n = i - w * R.N;
+  uint32_t wg = (uint32_t)(w + R.world_offset), nn = (uint32_t)n;
+  float pos[3], q[4] = { 0.f, 0.f, 0.f, 1.f };
+  uint32_t r[4];
+  if (R.init_mode == 0) {
+    for (int j = 0; j < 3; ++j) pos[j] = R.p0_lo[j];
+  } else if (R.init_mode == 1) {
+    philox4x32_10(R.seed_lo, R.seed_hi, wg, nn, 0u, STREAM_INIT, r);
+    for (int j = 0; j < 3; ++j) pos[j] = R.p0_lo[j] + (R.p0_hi[j] - R.p0_lo[j]) * u01(r[j]);
+    philox4x32_10(R.seed_lo, R.seed_hi, wg, nn, 1u, STREAM_INIT, r);      // reading R19
+    float zeta = 2.f * u01(r[0]) - 1.f, theta = R.tilt0_max * u01(r[2]);
+    float sa, ca, sh, ch;
+    sincospif(2.f * u01(r[1]), &sa, &ca);
+    float sxy = sqrtf(fmaxf(1.f - zeta * zeta, 0.f));
+    sincosf(0.5f * theta, &sh, &ch);
+    q[0] = sxy * ca * sh; q[1] = sxy * sa * sh; q[2] = zeta * sh; q[3] = ch;
+  } else {
+    philox4x32_10(R.seed_lo, R.seed_hi, wg, nn, 0u, STREAM_INIT, r);
+    long long gx = R.grid_dims[0], gy = R.grid_dims[1];
+    long long cell[3] = { n % gx, (n / gx) % gy, n / (gx * gy) };
+    for (int j = 0; j < 3; ++j)
+      pos[j] = R.grid_origin[j] + R.grid_spacing * (float)cell[j] + R.grid_jitter * (2.f * u01(r[j]) - 1.f);
+  }
+  const long long MN = R.MN;
+  const int D = R.model == MODEL_FP ? 17 : 13;
+  for (int j = 0; j < D; ++j) state[j * MN + i] = 0.f;
+  for (int j = 0; j < 3; ++j) state[j * MN + i] = pos[j];
+  if (R.model == MODEL_FP) {
+    for (int j = 0; j < 4; ++j) state[(3 + j) * MN + i] = q[j];
+    for (int k = 0; k < 4; ++k) state[(13 + k) * MN + i] = R.hover_rpm;
+  } else {
+    float Rm[3][3];
+    quat_to_R(q, Rm);
+    state[3 * MN + i] = atan2f(Rm[2][1], Rm[2][2]);
+    state[4 * MN + i] = -asinf(clipf(Rm[2][0], -1.f, 1.f));
+    state[5 * MN + i] = atan2f(Rm[1][0], Rm[0][0]);
+    state[12 * MN + i] = R.hover_thrust;
+  }
+  rearm(ctrl, min_d2, MN, i, R.model == MODEL_FP ? R.hover_rpm : 0.f, R.hover_thrust);
+}
+
+__global__ void set_state_kernel(float *state, float *ctrl, float *min_d2, const float *src, int broadcast, int D,
+                                 long long MN, float hover_rpm, float hover_thrust) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= MN) return;
+  for (int j = 0; j < D; ++j) state[j * MN + i] = broadcast ? src[j] : src[j * MN + i];
+  rearm(ctrl, min_d2, MN, i, hover_rpm, hover_thrust);
+}
+
+__global__ void set_counters_kernel(Counters *c, uint32_t s, int zero_rest) {
+  c->s = s;
+  if (zero_rest) { c->att_ticks = 0; c->pos_ticks = 0; c->n_rec_total = 0; }
+  c->blocks_done = 0;
+}
+
+// C10: per world, min over drones, obstacles (and, through min_d2, steps) of |p - c_j| - r_j.  One warp per world.
+__global__ void min_dist_kernel(const float *min_d2, float *out, long long M, long long N, long long MN,
+                                const __grid_constant__ DevParams P) {
+  long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  int lane = threadIdx.x & 31;
+  if (w >= M) return;
+  float best = __int_as_float(0x7f800000);
+  for (long long n = lane; n < N; n += 32) {
+    for (int j = 0; j < P.n_obst; ++j) best = fminf(best, sqrtf(min_d2[j * MN + w * N + n]) - P.obst[j][3]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) best = fminf(best, __shfl_xor_sync(0xffffffffu, best, o));
+  if (lane == 0) out[w] = best;
+}
+
+__global__ void philox_debug_kernel(uint32_t seed_lo, uint32_t seed_hi, const uint32_t *ctr, int n, uint32_t *words,
+                                    float *uni, float *nrm) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint32_t r[4];
+  philox4x32_10(seed_lo, seed_hi, ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], r);
+  float z[4];
+  normal_pair(r[0], r[1], z[0], z[1]);
+  normal_pair(r[2], r[3], z[2], z[3]);
+  for (int k = 0; k < 4; ++k) {
+    if (words) words[4 * i + k] = r[k];
+    if (uni) uni[4 * i + k] = u01(r[k]);
+    if (nrm) nrm[4 * i + k] = z[k];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf_params *p, void *workspace_dev,
+                         size_t workspace_bytes) {
+  if (!out) return fail(CF_E_ARG, "out is NULL");
+  *out = nullptr;
+  int rc = validate(M, N, model, p);
+  if (rc != CF_OK) return rc;
+  Carve c = carve(M, N, model, p);
+  if (!workspace_dev) return fail(CF_E_ARG, "workspace_dev is NULL");
+  if (((uintptr_t)workspace_dev & 255) != 0) return fail(CF_E_BUFFER, "workspace must be 256-byte aligned");
+  if (workspace_bytes < c.total) return fail(CF_E_BUFFER, "workspace too small: %zu < %zu", workspace_bytes, c.total);
+  cf_sim *s = new (std::nothrow) cf_sim();
+  if (!s) return fail(CF_E_ARG, "out of host memory");
+  s->M = M; s->N = N; s->MN = M * N; s->model = model; s->D = cf_state_dim(model); s->P = cf_world_param_dim(model);
+  s->p = *p;
+  char *base = (char *)workspace_dev;
+  s->state = (float *)(base + c.state); s->ctrl = (float *)(base + c.ctrl); s->wparam = (float *)(base + c.wparam);
+  s->min_d2 = p->n_obstacles > 0 ? (float *)(base + c.min_d2) : nullptr;
+  s->counters = (Counters *)(base + c.counters); s->rec_table = (uint32_t *)(base + c.rec_table);
+  s->stream = 0; s->seed = 0; s->s_host = 0; s->n_rec_host = 0; s->have_state = false;
+  s->hover_rpm = (float)hover_rpm_nominal(p);
+  fill_dev_params(s);
+  s->opt = needed_opt(s);
+  const char *name = nullptr;
+  bool ok = model == CF_MODEL_FIRST_PRINCIPLES
+      ? launch_fp(p->integrator, p->iface, s->opt, nullptr, nullptr, nullptr, &name, nullptr, true)
+      : launch_ab(p->integrator, p->iface, s->opt, nullptr, nullptr, nullptr, &name, nullptr, true);
+  if (!ok) { delete s; return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration"); }
+  *out = s;
+  return CF_OK;
+}
+
+extern "C" int cf_destroy(cf_sim *sim) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  delete sim;
+  return CF_OK;
+}
+
+extern "C" int cf_set_stream(cf_sim *sim, void *cuda_stream) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  sim->stream = (cudaStream_t)cuda_stream;
+  return CF_OK;
+}
+
+static int grid_for(long long n, int block) { return (int)((n + block - 1) / block); }
+
+extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  const cf_params &p = sim->p;
+  ResetArgs R;
+  memset(&R, 0, sizeof(R));
+  for (int j = 0; j < 12; ++j) { R.rnd_lo[j] = p.rnd_lo[j]; R.rnd_hi[j] = p.rnd_hi[j]; }
+  if (sim->model == CF_MODEL_FIRST_PRINCIPLES) {
+    R.nominal[0] = p.mass;
+    for (int j = 0; j < 3; ++j) { R.nominal[1 + j] = p.J[j]; R.nominal[4 + j] = p.kf[j]; R.nominal[7 + j] = p.km[j]; }
+    R.nominal[10] = p.cv_up; R.nominal[11] = p.cv_dn; R.nominal[12] = p.cd_up; R.nominal[13] = p.cd_dn;
+  } else {
+    R.nominal[0] = p.mass;
+    for (int j = 0; j < 3; ++j) { R.nominal[1 + j] = p.ab_a[j]; R.nominal[4 + j] = p.ab_b[j]; R.nominal[7 + j] = p.ab_c[j]; }
+    R.nominal[10] = p.ab_ctau;
+  }
+  for (int j = 0; j < 3; ++j) {
+    R.p0_lo[j] = p.p0_lo[j]; R.p0_hi[j] = p.p0_hi[j]; R.grid_origin[j] = p.grid_origin[j]; R.grid_dims[j] = p.grid_dims[j];
+  }
+  R.tilt0_max = p.tilt0_max; R.grid_spacing = p.grid_spacing; R.grid_jitter = p.grid_jitter;
+  R.init_mode = p.init_mode; R.model = sim->model;
+  R.hover_rpm = sim->hover_rpm; R.hover_thrust = (float)((double)p.mass * p.g);
+  R.M = sim->M; R.N = sim->N; R.MN = sim->MN; R.world_offset = p.world_offset;
+  R.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu); R.seed_hi = (uint32_t)(seed >> 32);
+  reset_params_kernel<<<grid_for(sim->M, 128), 128, 0, sim->stream>>>(sim->wparam, R);
+  reset_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(sim->state, sim->ctrl, sim->min_d2, R);
+  set_counters_kernel<<<1, 1, 0, sim->stream>>>(sim->counters, 0u, 1);
+  CF_CUDA(cudaMemsetAsync(sim->rec_table, 0, sizeof(uint32_t) * kRecTableCap, sim->stream));
+  CF_CUDA(cudaGetLastError());
+  sim->seed = seed; sim->s_host = 0; sim->n_rec_host = 0; sim->have_state = true;
+  return CF_OK;
+}
+
+extern "C" int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast) {
+  if (!sim || !state_dev) return fail(CF_E_ARG, "NULL argument");
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_set_state needs a prior cf_reset (world parameters)");
+  float hover_thrust = (float)((double)sim->p.mass * sim->p.g);
+  set_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(
+      sim->state, sim->ctrl, sim->min_d2, state_dev, broadcast, sim->D, sim->MN,
+      sim->model == CF_MODEL_FIRST_PRINCIPLES ? sim->hover_rpm : 0.f, hover_thrust);
+  CF_CUDA(cudaGetLastError());
+  return CF_OK;
+}
+
+extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctrl_dev, const float *wparam_dev,
+                           const float *min_d2_dev, int64_t step_counter) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  const size_t MN = (size_t)sim->MN;
+  if (state_dev) CF_CUDA(cudaMemcpyAsync(sim->state, state_dev, sizeof(float) * sim->D * MN, cudaMemcpyDeviceToDevice, sim->stream));
+  if (ctrl_dev) CF_CUDA(cudaMemcpyAsync(sim->ctrl, ctrl_dev, sizeof(float) * kCtrlPlanes * MN, cudaMemcpyDeviceToDevice, sim->stream));
+  if (wparam_dev) {
+    CF_CUDA(cudaMemcpyAsync(sim->wparam, wparam_dev, sizeof(float) * sim->P * (size_t)sim->M, cudaMemcpyDeviceToDevice, sim->stream));
+    sim->opt |= OPT_RANDP;     // the planes are now authoritative
+  }
+  if (min_d2_dev) {
+    if (!sim->min_d2) return fail(CF_E_ARG, "no obstacles configured");
+    CF_CUDA(cudaMemcpyAsync(sim->min_d2, min_d2_dev, sizeof(float) * kMaxObst * MN, cudaMemcpyDeviceToDevice, sim->stream));
+  }
+  if (step_counter >= 0) {
+    set_counters_kernel<<<1, 1, 0, sim->stream>>>(sim->counters, (uint32_t)step_counter, 0);
+    CF_CUDA(cudaGetLastError());
+    sim->s_host = step_counter;
+  }
+  sim->have_state = true;
+  return CF_OK;
+}
+
+// launch geometry: small problems are latency-bound -> small blocks spread over all SMs; large ones use 128/256.
+static int pick_block(long long MN) {
+  const long long sms = 148;
+  if (MN >= sms * 256 * 8) return 256;
+  if (MN >= sms * 128 * 2) return 128;
+  if (MN >= sms * 64) return 64;
+  return 32;
+}
+
+static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name, int *grid, int *block) {
+  LaunchCfg L;
+  L.block = pick_block(sim->MN);
+  L.grid = grid_for(sim->MN, L.block);
+  L.smem = ((sim->opt & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
+  L.stream = sim->stream;
+  if (grid) *grid = L.grid;
+  if (block) *block = L.block;
+  bool ok = sim->model == CF_MODEL_FIRST_PRINCIPLES
+      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, A, &sim->dp, &L, name, nullptr, dry)
+      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, A, &sim->dp, &L, name, nullptr, dry);
+  if (!ok) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
+  return CF_OK;
+}
+
+extern "C" int cf_describe_launch(const cf_sim *sim, char *buf, size_t buf_len, int *grid, int *block) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  const char *name = "";
+  int rc = do_launch(const_cast<cf_sim *>(sim), nullptr, true, &name, grid, block);
+  if (rc != CF_OK) return rc;
+  if (buf && buf_len) snprintf(buf, buf_len, "%s", name);
+  return CF_OK;
+}
+
+extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, int record_every,
+                       float *record_dev, size_t record_bytes) {
+  if (!sim || !cmds_dev) return fail(CF_E_ARG, "NULL argument");
+  if (n_steps < 1 || cmd_hold < 1 || n_cmds < 1 || record_every < 0) return fail(CF_E_ARG, "n_steps, cmd_hold, n_cmds >= 1; record_every >= 0");
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_step before cf_reset");
+  if ((long long)n_cmds * cmd_hold < n_steps) return fail(CF_E_SHAPE, "n_cmds * cmd_hold < n_steps");
+  if (((uintptr_t)cmds_dev & 15) != 0) return fail(CF_E_BUFFER, "cmds must be 16-byte aligned");
+  long long s0 = sim->s_host, n_rec = 0;
+  if (s0 + n_steps >= ((long long)1 << 32)) return fail(CF_E_SHAPE, "step counter would overflow 32 bits");
+  if (record_every > 0) {
+    n_rec = (s0 + n_steps) / record_every - s0 / record_every;
+    if (n_rec > 0 && (!record_dev || record_bytes < (size_t)n_rec * sim->D * (size_t)sim->MN * sizeof(float)))
+      return fail(CF_E_BUFFER, "record buffer too small for %lld records", n_rec);
+  }
+  StepArgs A;
+  A.state = sim->state; A.ctrl = sim->ctrl; A.wparam = sim->wparam; A.min_d2 = sim->min_d2;
+  A.counters = sim->counters; A.rec_table = sim->rec_table;
+  A.cmds = (const float4 *)cmds_dev; A.record = record_dev;
+  A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.world_offset = sim->p.world_offset;
+  A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.record_every = record_every; A.n_rec_cap = (int)n_rec;
+  A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);
+  int rc = do_launch(sim, &A, false, nullptr, nullptr, nullptr);
+  if (rc != CF_OK) return rc;
+  CF_CUDA(cudaGetLastError());
+  sim->s_host = s0 + n_steps;
+  sim->n_rec_host += n_rec;
+  return CF_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// host-buffer (end-to-end) path
+static size_t cmd_bytes(const cf_sim *sim, int n_cmds) {
+  size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? 1 : (size_t)sim->MN;
+  return align256(sizeof(float) * 4 * per * (size_t)n_cmds);
+}
+static long long n_records(const cf_sim *sim, int n_steps, int record_every) {
+  if (record_every <= 0) return 0;
+  return (sim->s_host + n_steps) / record_every - sim->s_host / record_every;
+}
+
+extern "C" size_t cf_staging_bytes(const cf_sim *sim, int n_cmds, int n_steps, int record_every) {
+  if (!sim || n_cmds < 1 || n_steps < 1) return 0;
+  return cmd_bytes(sim, n_cmds) + align256((size_t)n_records(sim, n_steps, record_every) * sim->D * (size_t)sim->MN * sizeof(float));
+}
+
+extern "C" int cf_step_host(cf_sim *sim, const void *cmds_host, int n_cmds, int cmd_hold, int n_steps, int record_every,
+                            float *record_host, size_t record_bytes, void *staging_dev, size_t staging_bytes) {
+  if (!sim || !cmds_host || !staging_dev) return fail(CF_E_ARG, "NULL argument");
+  if (n_cmds < 1 || n_steps < 1) return fail(CF_E_ARG, "n_cmds, n_steps >= 1");
+  if (((uintptr_t)staging_dev & 255) != 0) return fail(CF_E_BUFFER, "staging must be 256-byte aligned");
+  size_t need = cf_staging_bytes(sim, n_cmds, n_steps, record_every);
+  if (staging_bytes < need) return fail(CF_E_BUFFER, "staging too small: %zu < %zu", staging_bytes, need);
+  size_t cb = cmd_bytes(sim, n_cmds);
+  size_t rb = (size_t)n_records(sim, n_steps, record_every) * sim->D * (size_t)sim->MN * sizeof(float);
+  if (rb > 0 && (!record_host || record_bytes < rb)) return fail(CF_E_BUFFER, "host record buffer too small");
+  size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? 1 : (size_t)sim->MN;
+  CF_CUDA(cudaMemcpyAsync(staging_dev, cmds_host, sizeof(float) * 4 * per * (size_t)n_cmds, cudaMemcpyHostToDevice, sim->stream));
+  float *rec_dev = (float *)((char *)staging_dev + cb);
+  int rc = cf_step(sim, staging_dev, n_cmds, cmd_hold, n_steps, record_every, rec_dev, rb);
+  if (rc != CF_OK) return rc;
+  if (rb > 0) CF_CUDA(cudaMemcpyAsync(record_host, rec_dev, rb, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  return CF_OK;
+}
+
+extern "C" int cf_get_state(cf_sim *sim, float *out_dev) {
+  if (!sim || !out_dev) return fail(CF_E_ARG, "NULL argument");
+  CF_CUDA(cudaMemcpyAsync(out_dev, sim->state, sizeof(float) * sim->D * (size_t)sim->MN, cudaMemcpyDeviceToDevice, sim->stream));
+  return CF_OK;
+}
+extern "C" int cf_get_state_host(cf_sim *sim, float *out_host) {
+  if (!sim || !out_host) return fail(CF_E_ARG, "NULL argument");
+  CF_CUDA(cudaMemcpyAsync(out_host, sim->state, sizeof(float) * sim->D * (size_t)sim->MN, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  return CF_OK;
+}
+
+static int aux_source(cf_sim *sim, int which, const void **src, size_t *bytes) {
+  const size_t MN = (size_t)sim->MN;
+  switch (which) {
+    case CF_AUX_COUNTERS: *src = sim->counters; *bytes = 4 * sizeof(uint32_t); return CF_OK;
+    case CF_AUX_CTRL: *src = sim->ctrl; *bytes = sizeof(float) * kCtrlPlanes * MN; return CF_OK;
+    case CF_AUX_WORLD_PARAMS: *src = sim->wparam; *bytes = sizeof(float) * sim->P * (size_t)sim->M; return CF_OK;
+    case CF_AUX_REC_TABLE: *src = sim->rec_table; *bytes = sizeof(uint32_t) * kRecTableCap; return CF_OK;
+    case CF_AUX_MIN_D2:
+      if (!sim->min_d2) return fail(CF_E_ARG, "no obstacles configured");
+      *src = sim->min_d2; *bytes = sizeof(float) * kMaxObst * MN; return CF_OK;
+  }
+  return fail(CF_E_ARG, "bad aux selector %d", which);
+}
+
+static int launch_min_dist(cf_sim *sim, float *out_dev) {
+  if (!sim->min_d2) return fail(CF_E_ARG, "no obstacles configured");
+  long long threads = sim->M * 32;
+  min_dist_kernel<<<grid_for(threads, 128), 128, 0, sim->stream>>>(sim->min_d2, out_dev, sim->M, sim->N, sim->MN, sim->dp);
+  CF_CUDA(cudaGetLastError());
+  return CF_OK;
+}
+
+extern "C" int cf_get_aux(cf_sim *sim, int which, void *out_dev) {
+  if (!sim || !out_dev) return fail(CF_E_ARG, "NULL argument");
+  if (which == CF_AUX_MIN_DIST) return launch_min_dist(sim, (float *)out_dev);
+  const void *src; size_t bytes;
+  int rc = aux_source(sim, which, &src, &bytes);
+  if (rc != CF_OK) return rc;
+  CF_CUDA(cudaMemcpyAsync(out_dev, src, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  return CF_OK;
+}
+
+extern "C" int cf_get_aux_host(cf_sim *sim, int which, void *out_host, void *scratch_dev, size_t scratch_bytes) {
+  if (!sim || !out_host) return fail(CF_E_ARG, "NULL argument");
+  const void *src; size_t bytes;
+  if (which == CF_AUX_MIN_DIST) {
+    bytes = sizeof(float) * (size_t)sim->M;
+    if (!scratch_dev || scratch_bytes < bytes) return fail(CF_E_BUFFER, "scratch_dev must hold M floats");
+    int rc = launch_min_dist(sim, (float *)scratch_dev);
+    if (rc != CF_OK) return rc;
+    src = scratch_dev;
+  } else {
+    int rc = aux_source(sim, which, &src, &bytes);
+    if (rc != CF_OK) return rc;
+  }
+  CF_CUDA(cudaMemcpyAsync(out_host, src, bytes, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  return CF_OK;
+}
+
+extern "C" int64_t cf_step_counter(const cf_sim *sim) { return sim ? sim->s_host : -1; }
+
+extern "C" int cf_sync_counters(cf_sim *sim) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  uint32_t c[4];
+  CF_CUDA(cudaMemcpyAsync(c, sim->counters, sizeof(c), cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  sim->s_host = c[0];
+  sim->n_rec_host = c[3];
+  return CF_OK;
+}
+
+extern "C" int cf_debug_philox(uint64_t seed, const uint32_t ctr[4], uint32_t out[4]) {
+  if (!ctr || !out) return fail(CF_E_ARG, "NULL argument");
+  philox4x32_10((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32), ctr[0], ctr[1], ctr[2], ctr[3], out);
+  return CF_OK;
+}
+
+extern "C" int cf_debug_philox_dev(cf_sim *sim, uint64_t seed, const uint32_t *ctr_dev, int n, uint32_t *words_dev,
+                                   float *uniform_dev, float *normal_dev) {
+  if (!sim || !ctr_dev || n < 1) return fail(CF_E_ARG, "bad argument");
+  philox_debug_kernel<<<grid_for(n, 128), 128, 0, sim->stream>>>((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32),
+                                                                 ctr_dev, n, words_dev, uniform_dev, normal_dev);
+  CF_CUDA(cudaGetLastError());
+  return CF_OK;
+}

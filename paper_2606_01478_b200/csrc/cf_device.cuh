@@ -1,0 +1,618 @@
+// cf_device.cuh -- device side of libcf.so: the fused rollout kernel (thread = drone, state in registers across all
+// sub-steps) and its building blocks.  float32 arithmetic, uint32 counters / Philox.  sm_100a only.
+//
+// What each piece computes is defined by PAPER.md Eqs. (1)-(10) and the readings in DESIGN.md; citations are at
+// each function.  This file shares nothing with oracle/ (the float64 CPU oracle).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cf {
+
+constexpr int kMaxObst = 8;
+constexpr int kCtrlPlanes = 14;
+constexpr int kRecTableCap = 4096;
+
+// option bits of a kernel instantiation
+enum : int {
+  OPT_RANDP = 1,    // plant parameters come from the per-world planes (domain randomisation)
+  OPT_DIST = 2,     // per-step Philox force disturbance
+  OPT_OBST = 4,     // running minimum squared distance to the obstacle spheres
+  OPT_NOISE = 8,    // command = clip(nominal[k] + sigma * z), z from Philox (CF_CMD_NOMINAL_PLUS_NOISE)
+  OPT_EXTRAS = 16,  // full Eq. (6) (asymmetric + quadratic), thrust/torque polynomials, Eq. (5) gyro, body drag,
+                    // simplified AB variant
+  OPT_ALL = 31
+};
+enum : int { MODEL_FP = 0, MODEL_AB = 1 };
+enum : int { INTEG_EULER = 0, INTEG_RK4 = 1 };
+enum : int { IF_ROTOR = 0, IF_TORQUE = 1, IF_ATTITUDE = 2, IF_POSITION = 3 };
+enum : int { STREAM_INIT = 0, STREAM_PARAM = 1, STREAM_DIST = 2, STREAM_NOISE = 3 };
+
+struct Counters {          // device-resident, 64 B
+  uint32_t s, att_ticks, pos_ticks, n_rec_total;
+  uint32_t blocks_done, pad[11];
+};
+
+// Uniform (per-launch) constants; lives in the kernel parameter constant bank.
+struct DevParams {
+  float h, half_h, h_sixth, h_att, h_pos, g;
+  // nominal plant
+  float mass, inv_mass, J[3], inv_J[3], lever, kf[3], km[3];
+  float cv_up, cv_dn, cd_up, cd_dn, Jp_rad /* Jp * 2pi/60 */, Ca[3];
+  float ab_a[3], ab_b[3], ab_c[3], ab_ctau, ab_cf;
+  int   ab_thrust_dyn, thrust_poly /* kf0 or kf1 != 0 */, has_drag, has_gyro;
+  // controller (nominal parameters, reading R11)
+  float inv_4lever, inv_4kappa, f_rotor_max, inv_kf2, rpm_min, rpm_max, thrust_min, thrust_max, tilt_max;
+  float kR[3], kW[3], kI[3], iR_max, Jnom[3];
+  float kp[3], kd[3], ki[3], ip_max[3];
+  float dist_sigma;
+  int   use_noise;   // cmd_source == CF_CMD_NOMINAL_PLUS_NOISE
+  int   n_obst;
+  float obst[kMaxObst][4];
+  float noise_sigma[4], cmd_lo[4], cmd_hi[4];
+  int   att_div, pos_div;
+};
+
+struct StepArgs {
+  float *state;            // [D][MN]
+  float *ctrl;             // [14][MN]
+  const float *wparam;     // [P][M]
+  float *min_d2;           // [8][MN] or nullptr
+  Counters *counters;
+  uint32_t *rec_table;     // [kRecTableCap]
+  const float4 *cmds;      // [K][MN] or [K]
+  float *record;           // [n_rec][D][MN]
+  long long MN, M, N, world_offset;
+  int n_steps, cmd_hold, record_every, n_rec_cap;
+  uint32_t seed_lo, seed_hi;
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al. 2011), reading C9: key = (seed lo, seed hi), counter = (world, drone, index, stream)
+__host__ __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
+                                                       uint32_t c2, uint32_t c3, uint32_t out[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+#ifdef __CUDA_ARCH__
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+#else
+    uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+#endif
+    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// reading R18: 23-bit midpoint uniform in (0,1), exact in float32
+__device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * (1.0f / 8388608.0f); }
+
+// Box-Muller (C9): r = sqrt(-2 ln ua), (z0, z1) = r (cos 2 pi ub, sin 2 pi ub).  sincospi keeps the angle exact.
+__device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, float &z0, float &z1) {
+  float ua = u01(xa), ub = u01(xb);
+  float r = sqrtf(-2.0f * logf(ua));
+  float s, c;
+  sincospif(2.0f * ub, &s, &c);
+  z0 = r * c; z1 = r * s;
+}
+
+__device__ __forceinline__ float clipf(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Plant parameters of one world, in the derived form the derivative wants.
+template <int MODEL, int OPT> struct Plant;
+
+template <int OPT> struct Plant<MODEL_FP, OPT> {
+  float inv_m, inv_J[3], cJ[3];      // cJ = ((Jy-Jz)/Jx, (Jz-Jx)/Jy, (Jx-Jy)/Jz): Euler's equation cross term
+  float kf2, km2, cv;                // lean rotor / thrust model
+  float J[3], kf0, kf1, km0, km1, cv_dn, cd_up, cd_dn;   // only read when OPT_EXTRAS
+
+  __device__ __forceinline__ void set(float m, float Jx, float Jy, float Jz, const float kf[3], const float km[3],
+                                      float cvu, float cvd, float cdu, float cdd) {
+    inv_m = 1.0f / m;
+    inv_J[0] = 1.0f / Jx; inv_J[1] = 1.0f / Jy; inv_J[2] = 1.0f / Jz;
+    cJ[0] = (Jy - Jz) * inv_J[0]; cJ[1] = (Jz - Jx) * inv_J[1]; cJ[2] = (Jx - Jy) * inv_J[2];
+    kf2 = kf[2]; km2 = km[2]; cv = cvu;
+    J[0] = Jx; J[1] = Jy; J[2] = Jz;
+    kf0 = kf[0]; kf1 = kf[1]; km0 = km[0]; km1 = km[1]; cv_dn = cvd; cd_up = cdu; cd_dn = cdd;
+  }
+  __device__ __forceinline__ void load(const DevParams &P, const float *wp, long long M, long long w, bool randp) {
+    if (randp) {
+      float kf[3] = { wp[4 * M + w], wp[5 * M + w], wp[6 * M + w] };
+      float km[3] = { wp[7 * M + w], wp[8 * M + w], wp[9 * M + w] };
+      set(wp[w], wp[M + w], wp[2 * M + w], wp[3 * M + w], kf, km, wp[10 * M + w], wp[11 * M + w], wp[12 * M + w],
+          wp[13 * M + w]);
+    } else {
+      set(P.mass, P.J[0], P.J[1], P.J[2], P.kf, P.km, P.cv_up, P.cv_dn, P.cd_up, P.cd_dn);
+    }
+  }
+};
+
+template <int OPT> struct Plant<MODEL_AB, OPT> {
+  float inv_m, a[3], b[3], c[3], ctau;
+  __device__ __forceinline__ void load(const DevParams &P, const float *wp, long long M, long long w, bool randp) {
+    if (randp) {
+      inv_m = 1.0f / wp[w];
+#pragma unroll
+      for (int j = 0; j < 3; ++j) { a[j] = wp[(1 + j) * M + w]; b[j] = wp[(4 + j) * M + w]; c[j] = wp[(7 + j) * M + w]; }
+      ctau = wp[10 * M + w];
+    } else {
+      inv_m = P.inv_mass;
+#pragma unroll
+      for (int j = 0; j < 3; ++j) { a[j] = P.ab_a[j]; b[j] = P.ab_b[j]; c[j] = P.ab_c[j]; }
+      ctau = P.ab_ctau;
+    }
+  }
+};
+
+// rotation matrix of a scalar-last unit quaternion
+__device__ __forceinline__ void quat_to_R(const float *q, float R[3][3]) {
+  float x = q[0], y = q[1], z = q[2], w = q[3];
+  float xx = x * x, yy = y * y, zz = z * z, xy = x * y, xz = x * z, yz = y * z, wx = w * x, wy = w * y, wz = w * z;
+  R[0][0] = 1.0f - 2.0f * (yy + zz); R[0][1] = 2.0f * (xy - wz);        R[0][2] = 2.0f * (xz + wy);
+  R[1][0] = 2.0f * (xy + wz);        R[1][1] = 1.0f - 2.0f * (xx + zz); R[1][2] = 2.0f * (yz - wx);
+  R[2][0] = 2.0f * (xz - wy);        R[2][1] = 2.0f * (yz + wx);        R[2][2] = 1.0f - 2.0f * (xx + yy);
+}
+// reading R13: R = Rz(yaw) Ry(pitch) Rx(roll)
+__device__ __forceinline__ void euler_to_R(float roll, float pitch, float yaw, float R[3][3]) {
+  float sr, cr, sp, cp, sy, cy;
+  sincosf(roll, &sr, &cr); sincosf(pitch, &sp, &cp); sincosf(yaw, &sy, &cy);
+  R[0][0] = cy * cp; R[0][1] = cy * sp * sr - sy * cr; R[0][2] = cy * sp * cr + sy * sr;
+  R[1][0] = sy * cp; R[1][1] = sy * sp * sr + cy * cr; R[1][2] = sy * sp * cr - cy * sr;
+  R[2][0] = -sp;     R[2][1] = cp * sr;                R[2][2] = cp * cr;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// First-principles derivative, Eqs. (1)-(6) (C2).  x = p(0-2) q(3-6) v(7-9) w(10-12) Omega(13-16).
+// Mixing matrix C1: sx = (-,-,+,+), sy = (-,+,+,-), sz = (-,+,-,+) (X configuration, spin +,-,+,-).
+template <int OPT>
+__device__ __forceinline__ void deriv_fp(const DevParams &P, const Plant<MODEL_FP, OPT> &pl, const float *x,
+                                         const float *rpm_cmd, const float *fdist, float *dx) {
+  const float *q = x + 3, *v = x + 7, *w = x + 10, *Om = x + 13;
+  constexpr bool EX = (OPT & OPT_EXTRAS) != 0;
+  float dOm[4];
+  float F, tau[3];   // F [N] ; tau already divided by nothing (N m)
+  if (!EX) {
+    // Eq. (6) with c_v^ = c_v_, c_d = 0: first-order lag;  f = kf2 W^2, m = km2 W^2
+    float w2[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { dOm[k] = pl.cv * (rpm_cmd[k] - Om[k]); w2[k] = Om[k] * Om[k]; }
+    float A = w2[0] + w2[1], B = w2[2] + w2[3], C = w2[1] + w2[2], D = w2[0] + w2[3];
+    float E = w2[1] + w2[3], G = w2[0] + w2[2];
+    F = pl.kf2 * (A + B);
+    tau[0] = (P.lever * pl.kf2) * (B - A);
+    tau[1] = (P.lever * pl.kf2) * (C - D);
+    tau[2] = pl.km2 * (E - G);
+  } else {
+    float f[4], mk[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      float e = rpm_cmd[k] - Om[k];
+      bool up = e >= 0.0f;
+      float cv = up ? pl.cv : pl.cv_dn, cd = up ? pl.cd_up : pl.cd_dn;
+      dOm[k] = cv * e + cd * (rpm_cmd[k] * rpm_cmd[k] - Om[k] * Om[k]);
+      f[k] = pl.kf0 + Om[k] * (pl.kf1 + pl.kf2 * Om[k]);
+      mk[k] = pl.km0 + Om[k] * (pl.km1 + pl.km2 * Om[k]);
+    }
+    F = (f[0] + f[1]) + (f[2] + f[3]);
+    tau[0] = P.lever * ((f[2] + f[3]) - (f[0] + f[1]));
+    tau[1] = P.lever * ((f[1] + f[2]) - (f[0] + f[3]));
+    tau[2] = (mk[1] + mk[3]) - (mk[0] + mk[2]);
+    if (P.has_gyro) {   // Eq. (5), reading R2: Jp (-wy S, +wx S, -dS), S = W1 - W2 + W3 - W4 in rad/s
+      float S = (Om[0] - Om[1]) + (Om[2] - Om[3]), dS = (dOm[0] - dOm[1]) + (dOm[2] - dOm[3]);
+      tau[0] -= P.Jp_rad * w[1] * S;
+      tau[1] += P.Jp_rad * w[0] * S;
+      tau[2] -= P.Jp_rad * dS;
+    }
+  }
+  // Eq. (3): dv = z_B F/m + f_dist/m - g e_z (+ body drag)
+  float zx = 2.0f * (q[0] * q[2] + q[3] * q[1]);
+  float zy = 2.0f * (q[1] * q[2] - q[3] * q[0]);
+  float zz = 1.0f - 2.0f * (q[0] * q[0] + q[1] * q[1]);
+  float acc = F * pl.inv_m;
+  float ax = zx * acc, ay = zy * acc, az = zz * acc - P.g;
+  if (OPT & OPT_DIST) { ax += fdist[0] * pl.inv_m; ay += fdist[1] * pl.inv_m; az += fdist[2] * pl.inv_m; }
+  if (EX && P.has_drag) {
+    float R[3][3];
+    quat_to_R(q, R);
+    float fb[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) fb[j] = P.Ca[j] * (R[0][j] * v[0] + R[1][j] * v[1] + R[2][j] * v[2]);
+    ax += (R[0][0] * fb[0] + R[0][1] * fb[1] + R[0][2] * fb[2]) * pl.inv_m;
+    ay += (R[1][0] * fb[0] + R[1][1] * fb[1] + R[1][2] * fb[2]) * pl.inv_m;
+    az += (R[2][0] * fb[0] + R[2][1] * fb[1] + R[2][2] * fb[2]) * pl.inv_m;
+  }
+  dx[7] = ax; dx[8] = ay; dx[9] = az;
+  // Eq. (4), diagonal J: dw = tau/J + cJ * (w_j w_k)
+  dx[10] = tau[0] * pl.inv_J[0] + pl.cJ[0] * (w[1] * w[2]);
+  dx[11] = tau[1] * pl.inv_J[1] + pl.cJ[1] * (w[2] * w[0]);
+  dx[12] = tau[2] * pl.inv_J[2] + pl.cJ[2] * (w[0] * w[1]);
+  // Eq. (2), reading R1: dq = 1/2 q (x) (w, 0)
+  dx[3] = 0.5f * (q[3] * w[0] + q[1] * w[2] - q[2] * w[1]);
+  dx[4] = 0.5f * (q[3] * w[1] + q[2] * w[0] - q[0] * w[2]);
+  dx[5] = 0.5f * (q[3] * w[2] + q[0] * w[1] - q[1] * w[0]);
+  dx[6] = -0.5f * (q[0] * w[0] + q[1] * w[1] + q[2] * w[2]);
+  // Eq. (1)
+  dx[0] = v[0]; dx[1] = v[1]; dx[2] = v[2];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) dx[13 + k] = dOm[k];
+}
+
+// Abstracted derivative, Eqs. (7)-(10) (C3).  x = p(0-2) Psi(3-5) v(6-8) dPsi(9-11) f_Sigma(12); u = attitude cmd.
+template <int OPT>
+__device__ __forceinline__ void deriv_ab(const DevParams &P, const Plant<MODEL_AB, OPT> &pl, const float *x,
+                                         const float *u, const float *fdist, float *dx) {
+  constexpr bool EX = (OPT & OPT_EXTRAS) != 0;
+  float sr, cr, sp, cp, sy, cy;
+  sincosf(x[3], &sr, &cr); sincosf(x[4], &sp, &cp); sincosf(x[5], &sy, &cy);
+  float zx = cy * sp * cr + sy * sr, zy = sy * sp * cr - cy * sr, zz = cp * cr;
+  float fS = (EX && !P.ab_thrust_dyn) ? u[3] : x[12];
+  float acc = (P.ab_cf * fS) * pl.inv_m;
+  float ax = zx * acc, ay = zy * acc, az = zz * acc - P.g;
+  if (OPT & OPT_DIST) { ax += fdist[0] * pl.inv_m; ay += fdist[1] * pl.inv_m; az += fdist[2] * pl.inv_m; }
+  if (EX && P.has_drag) {
+    float R[3][3];
+    R[0][0] = cy * cp; R[0][1] = cy * sp * sr - sy * cr; R[0][2] = zx;
+    R[1][0] = sy * cp; R[1][1] = sy * sp * sr + cy * cr; R[1][2] = zy;
+    R[2][0] = -sp;     R[2][1] = cp * sr;                R[2][2] = zz;
+    const float *v = x + 6;
+    float fb[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) fb[j] = P.Ca[j] * (R[0][j] * v[0] + R[1][j] * v[1] + R[2][j] * v[2]);
+    ax += (R[0][0] * fb[0] + R[0][1] * fb[1] + R[0][2] * fb[2]) * pl.inv_m;
+    ay += (R[1][0] * fb[0] + R[1][1] * fb[1] + R[1][2] * fb[2]) * pl.inv_m;
+    az += (R[2][0] * fb[0] + R[2][1] * fb[1] + R[2][2] * fb[2]) * pl.inv_m;
+  }
+  dx[0] = x[6]; dx[1] = x[7]; dx[2] = x[8];
+  dx[6] = ax; dx[7] = ay; dx[8] = az;
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    dx[3 + j] = x[9 + j];
+    dx[9 + j] = pl.a[j] * x[3 + j] + pl.b[j] * x[9 + j] + pl.c[j] * u[j];
+  }
+  dx[12] = (EX && !P.ab_thrust_dyn) ? 0.0f : pl.ctau * (u[3] - x[12]);
+}
+
+template <int MODEL, int OPT>
+__device__ __forceinline__ void deriv(const DevParams &P, const Plant<MODEL, OPT> &pl, const float *x,
+                                      const float *u, const float *fdist, float *dx) {
+  if constexpr (MODEL == MODEL_FP) deriv_fp<OPT>(P, pl, x, u, fdist, dx);
+  else deriv_ab<OPT>(P, pl, x, u, fdist, dx);
+}
+
+// C4: explicit Euler / classical RK4, inputs held; q renormalised once per step, not inside the stages (R8-R10).
+template <int MODEL, int INTEG, int OPT>
+__device__ __forceinline__ void integrate(const DevParams &P, const Plant<MODEL, OPT> &pl, float *x, const float *u,
+                                          const float *fdist) {
+  constexpr int D = MODEL == MODEL_FP ? 17 : 13;
+  float k[D];
+  if constexpr (INTEG == INTEG_EULER) {
+    deriv<MODEL, OPT>(P, pl, x, u, fdist, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) x[j] = fmaf(P.h, k[j], x[j]);
+  } else {
+    float xs[D], acc[D];
+    deriv<MODEL, OPT>(P, pl, x, u, fdist, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { acc[j] = k[j]; xs[j] = fmaf(P.half_h, k[j], x[j]); }
+    deriv<MODEL, OPT>(P, pl, xs, u, fdist, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { acc[j] = fmaf(2.0f, k[j], acc[j]); xs[j] = fmaf(P.half_h, k[j], x[j]); }
+    deriv<MODEL, OPT>(P, pl, xs, u, fdist, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { acc[j] = fmaf(2.0f, k[j], acc[j]); xs[j] = fmaf(P.h, k[j], x[j]); }
+    deriv<MODEL, OPT>(P, pl, xs, u, fdist, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) x[j] = fmaf(P.h_sixth, acc[j] + k[j], x[j]);
+  }
+  if constexpr (MODEL == MODEL_FP) {
+    float *q = x + 3;
+    float inv = rsqrtf(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) q[j] *= inv;
+  } else if ((OPT & OPT_EXTRAS) && !P.ab_thrust_dyn) {
+    x[12] = u[3];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// C6 motor mixer (nominal parameters): (F_c, tau_des) -> rotor thrusts -> clip -> rpm -> clip
+template <int OPT>
+__device__ __forceinline__ void mixer(const DevParams &P, float Fc, const float *tau, float *rpm_cmd) {
+  float a = 0.25f * Fc, bx = tau[0] * P.inv_4lever, by = tau[1] * P.inv_4lever, bz = tau[2] * P.inv_4kappa;
+  float f[4] = { a - bx - by - bz, a - bx + by + bz, a + bx + by - bz, a + bx - by + bz };
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    float fk = clipf(f[k], 0.0f, P.f_rotor_max);
+    float r;
+    if ((OPT & OPT_EXTRAS) && P.thrust_poly) {
+      float disc = fmaxf(P.kf[1] * P.kf[1] - 4.0f * P.kf[2] * (P.kf[0] - fk), 0.0f);
+      r = (sqrtf(disc) - P.kf[1]) * (0.5f * P.inv_kf2);
+    } else {
+      r = sqrtf(fk * P.inv_kf2);
+    }
+    rpm_cmd[k] = clipf(r, P.rpm_min, P.rpm_max);
+  }
+}
+
+// C5 attitude controller tick (reading R7).  Rd = columns of the desired rotation, hoisted to the command fetch.
+template <int OPT>
+__device__ __forceinline__ void attitude_tick(const DevParams &P, const float *q, const float *w, const float Rd[3][3],
+                                              float Fc, float *iR, float *rpm_cmd) {
+  float R[3][3];
+  quat_to_R(q, R);
+  // M = Rd^T R ; e_R = 1/2 (M32 - M23, M13 - M31, M21 - M12)
+  auto Mij = [&](int i, int j) { return Rd[0][i] * R[0][j] + Rd[1][i] * R[1][j] + Rd[2][i] * R[2][j]; };
+  float eR[3] = { 0.5f * (Mij(2, 1) - Mij(1, 2)), 0.5f * (Mij(0, 2) - Mij(2, 0)), 0.5f * (Mij(1, 0) - Mij(0, 1)) };
+  float tau[3];
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    iR[j] = clipf(fmaf(eR[j], P.h_att, iR[j]), -P.iR_max, P.iR_max);
+    tau[j] = P.Jnom[j] * (-P.kR[j] * eR[j] - P.kW[j] * w[j] - P.kI[j] * iR[j]);
+  }
+  mixer<OPT>(P, Fc, tau, rpm_cmd);
+}
+
+// C7 geometric position controller tick (reading R16): target (x,y,z,yaw) -> attitude command (roll,pitch,yaw,F)
+__device__ __forceinline__ void position_tick(const DevParams &P, const float *pos, const float *vel, const float *zB,
+                                              const float *target, float *ip, float *att_cmd) {
+  float t[3];
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    float ep = target[j] - pos[j];
+    ip[j] = clipf(fmaf(ep, P.h_pos, ip[j]), -P.ip_max[j], P.ip_max[j]);
+    float ad = P.kp[j] * ep - P.kd[j] * vel[j] + P.ki[j] * ip[j] + (j == 2 ? P.g : 0.0f);
+    t[j] = P.mass * ad;
+  }
+  float Fc = clipf(t[0] * zB[0] + t[1] * zB[1] + t[2] * zB[2], P.thrust_min, P.thrust_max);
+  float nt = fmaxf(sqrtf(t[0] * t[0] + t[1] * t[1] + t[2] * t[2]), 1e-6f);
+  float inv = 1.0f / nt;
+  float zd[3] = { t[0] * inv, t[1] * inv, t[2] * inv };
+  float sy, cy;
+  sincosf(target[3], &sy, &cy);
+  // y_d = z_d x x_c,  x_c = (cos yaw, sin yaw, 0)
+  float yd[3] = { -zd[2] * sy, zd[2] * cy, zd[0] * sy - zd[1] * cy };
+  float ny = fmaxf(sqrtf(yd[0] * yd[0] + yd[1] * yd[1] + yd[2] * yd[2]), 1e-6f);
+  float invy = 1.0f / ny;
+  yd[0] *= invy; yd[1] *= invy; yd[2] *= invy;
+  // x_d = y_d x z_d
+  float xd[3] = { yd[1] * zd[2] - yd[2] * zd[1], yd[2] * zd[0] - yd[0] * zd[2], yd[0] * zd[1] - yd[1] * zd[0] };
+  att_cmd[0] = clipf(atan2f(yd[2], zd[2]), -P.tilt_max, P.tilt_max);
+  att_cmd[1] = clipf(asinf(clipf(-xd[2], -1.0f, 1.0f)), -P.tilt_max, P.tilt_max);
+  att_cmd[2] = atan2f(xd[1], xd[0]);
+  att_cmd[3] = Fc;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// The rollout kernel.  One thread = one drone; the state, controller state, held commands and plant parameters stay
+// in registers for all n_steps; HBM is touched for command loads, recorded states and the final store only.
+template <int MODEL, int INTEG, int IFACE, int OPT>
+__global__ void __launch_bounds__(256)
+rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevParams P) {
+  constexpr int D = MODEL == MODEL_FP ? 17 : 13;
+  constexpr int NP = MODEL == MODEL_FP ? 14 : 11;
+  constexpr bool FP = MODEL == MODEL_FP;
+  constexpr bool HAS_ATT = FP && IFACE >= IF_ATTITUDE;       // attitude controller + mixer active
+  constexpr bool HAS_POS = IFACE == IF_POSITION;
+  extern __shared__ float wp_s[];                            // [NP][span]: per-world parameters of this block (N > 1)
+
+  const long long MN = A.MN;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool active = i < MN;
+  const uint32_t s0 = *((volatile uint32_t *)&A.counters->s);
+  const uint32_t rec0 = *((volatile uint32_t *)&A.counters->n_rec_total);
+
+  Plant<MODEL, OPT> pl;
+  long long w = 0, n = 0;
+  if (active) { w = i / A.N; n = i - w * A.N; }
+  if ((OPT & OPT_RANDP) && A.N > 1) {
+    // stage the parameter rows of the worlds this block touches in shared memory, then read them from there
+    long long first = (long long)blockIdx.x * blockDim.x;
+    long long last = first + blockDim.x - 1 < MN - 1 ? first + blockDim.x - 1 : MN - 1;
+    long long w_first = first / A.N;
+    int span = (int)(last / A.N - w_first) + 1;
+    for (int idx = threadIdx.x; idx < NP * span; idx += blockDim.x) {
+      int pidx = idx / span, j = idx - pidx * span;
+      wp_s[idx] = A.wparam[pidx * A.M + w_first + j];
+    }
+    __syncthreads();
+    if (active) pl.load(P, wp_s, span, w - w_first, true);
+  } else if (active) {
+    pl.load(P, A.wparam, A.M, w, (OPT & OPT_RANDP) != 0);
+  }
+
+  uint32_t my_att = 0, my_pos = 0;
+  if (active) {
+    float x[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) x[j] = A.state[j * MN + i];
+    float iR[3] = { 0, 0, 0 }, ip[3] = { 0, 0, 0 }, att_cmd[4] = { 0, 0, 0, 0 }, rpm_cmd[4] = { 0, 0, 0, 0 };
+    float target[4] = { 0, 0, 0, 0 };
+    if (HAS_ATT) {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) iR[j] = A.ctrl[j * MN + i];
+    }
+    if (HAS_POS) {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) ip[j] = A.ctrl[(3 + j) * MN + i];
+    }
+    if (HAS_ATT || HAS_POS || !FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) att_cmd[j] = A.ctrl[(6 + j) * MN + i];
+    }
+    if (FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) rpm_cmd[j] = A.ctrl[(10 + j) * MN + i];
+    }
+    float md2[kMaxObst];
+    const bool obst = (OPT & OPT_OBST) != 0 && A.min_d2 != nullptr;
+    if (obst) {
+#pragma unroll
+      for (int j = 0; j < kMaxObst; ++j) md2[j] = A.min_d2[j * MN + i];
+    }
+    float Rd[3][3];
+    if (HAS_ATT) euler_to_R(att_cmd[0], att_cmd[1], att_cmd[2], Rd);
+
+    const uint32_t wg = (uint32_t)(w + A.world_offset), nn = (uint32_t)n;
+    uint32_t s = s0;
+    int att_phase = (int)(s0 % (uint32_t)P.att_div), pos_phase = (int)(s0 % (uint32_t)P.pos_div);
+    int rec_phase = A.record_every > 0 ? (int)(s0 % (uint32_t)A.record_every) : 0;
+    int rec_slot = 0;
+    int cmd_cd = 0, cmd_k = 0;
+    const bool noise = (OPT & OPT_NOISE) != 0 && P.use_noise;   // compiled in AND requested
+    const float4 *cp = noise ? A.cmds : A.cmds + i;
+    const long long cstride = noise ? 1 : MN;
+    float4 next_cmd = __ldg(cp);
+
+    for (int t = 0; t < A.n_steps; ++t) {
+      // (1) command fetch (prefetched one segment ahead)
+      if (cmd_cd == 0) {
+        float4 c4 = next_cmd;
+        cmd_cd = A.cmd_hold;
+        ++cmd_k;
+        if ((long long)cmd_k * A.cmd_hold < A.n_steps) next_cmd = __ldg(cp + cmd_k * cstride);
+        float c[4] = { c4.x, c4.y, c4.z, c4.w };
+        if (noise) {
+          uint32_t r[4]; float z[4];
+          philox4x32_10(A.seed_lo, A.seed_hi, wg, nn, s, STREAM_NOISE, r);
+          normal_pair(r[0], r[1], z[0], z[1]);
+          normal_pair(r[2], r[3], z[2], z[3]);
+#pragma unroll
+          for (int j = 0; j < 4; ++j) c[j] = clipf(fmaf(P.noise_sigma[j], z[j], c[j]), P.cmd_lo[j], P.cmd_hi[j]);
+        }
+        if (IFACE == IF_ATTITUDE) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) att_cmd[j] = c[j];
+          if (HAS_ATT) euler_to_R(att_cmd[0], att_cmd[1], att_cmd[2], Rd);
+        } else if (IFACE == IF_POSITION) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) target[j] = c[j];
+        } else if (IFACE == IF_ROTOR) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) rpm_cmd[j] = clipf(c[j], P.rpm_min, P.rpm_max);
+        } else {   // torque interface: (tau_x, tau_y, tau_z, F) straight into the mixer
+          mixer<OPT>(P, c[3], c, rpm_cmd);
+        }
+      }
+      --cmd_cd;
+      // (2) position controller tick
+      if (HAS_POS) {
+        if (pos_phase == 0) {
+          float zB[3];
+          if (FP) {
+            const float *q = x + 3;
+            zB[0] = 2.0f * (q[0] * q[2] + q[3] * q[1]);
+            zB[1] = 2.0f * (q[1] * q[2] - q[3] * q[0]);
+            zB[2] = 1.0f - 2.0f * (q[0] * q[0] + q[1] * q[1]);
+          } else {
+            float sr, cr, sp, cp_, sy, cy;
+            sincosf(x[3], &sr, &cr); sincosf(x[4], &sp, &cp_); sincosf(x[5], &sy, &cy);
+            zB[0] = cy * sp * cr + sy * sr; zB[1] = sy * sp * cr - cy * sr; zB[2] = cp_ * cr;
+          }
+          position_tick(P, x, FP ? x + 7 : x + 6, zB, target, ip, att_cmd);
+          if (HAS_ATT) euler_to_R(att_cmd[0], att_cmd[1], att_cmd[2], Rd);
+          ++my_pos;
+        }
+        pos_phase = pos_phase + 1 == P.pos_div ? 0 : pos_phase + 1;
+      }
+      // (3) attitude controller tick + mixer
+      if (HAS_ATT) {
+        if (att_phase == 0) {
+          attitude_tick<OPT>(P, x + 3, x + 10, Rd, att_cmd[3], iR, rpm_cmd);
+          ++my_att;
+        }
+        att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
+      }
+      // (4) disturbance draw, held over the RK4 stages
+      float fdist[3] = { 0, 0, 0 };
+      if ((OPT & OPT_DIST) && P.dist_sigma > 0.0f) {
+        uint32_t r[4]; float z[4];
+        philox4x32_10(A.seed_lo, A.seed_hi, wg, nn, s, STREAM_DIST, r);
+        normal_pair(r[0], r[1], z[0], z[1]);
+        normal_pair(r[2], r[3], z[2], z[3]);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) fdist[j] = P.dist_sigma * z[j];
+      }
+      // (5) integrate, (6) count
+      integrate<MODEL, INTEG, OPT>(P, pl, x, FP ? rpm_cmd : att_cmd, fdist);
+      ++s;
+      // (7) obstacle minima (squared centre distance; the square roots are taken once, at read-out)
+      if (obst) {
+#pragma unroll
+        for (int j = 0; j < kMaxObst; ++j) {
+          if (j < P.n_obst) {
+            float dx_ = x[0] - P.obst[j][0], dy_ = x[1] - P.obst[j][1], dz_ = x[2] - P.obst[j][2];
+            md2[j] = fminf(md2[j], dx_ * dx_ + dy_ * dy_ + dz_ * dz_);
+          }
+        }
+      }
+      // (8) record (streaming stores; a warp writes whole 128-byte lines of each plane)
+      if (A.record_every > 0) {
+        if (++rec_phase == A.record_every) {
+          rec_phase = 0;
+          if (rec_slot < A.n_rec_cap) {
+            float *r = A.record + (size_t)rec_slot * D * MN + i;
+#pragma unroll
+            for (int j = 0; j < D; ++j) __stcs(r + j * MN, x[j]);
+            if (i == 0 && rec0 + (uint32_t)rec_slot < (uint32_t)kRecTableCap) A.rec_table[rec0 + rec_slot] = s;
+          }
+          ++rec_slot;
+        }
+      }
+    }
+    // final store
+#pragma unroll
+    for (int j = 0; j < D; ++j) A.state[j * MN + i] = x[j];
+    if (HAS_ATT) {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) A.ctrl[j * MN + i] = iR[j];
+    }
+    if (HAS_POS) {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) A.ctrl[(3 + j) * MN + i] = ip[j];
+    }
+    if (HAS_ATT || HAS_POS || !FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) A.ctrl[(6 + j) * MN + i] = att_cmd[j];
+    }
+    if (FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) A.ctrl[(10 + j) * MN + i] = rpm_cmd[j];
+    }
+    if (obst) {
+#pragma unroll
+      for (int j = 0; j < kMaxObst; ++j) A.min_d2[j * MN + i] = md2[j];
+    }
+    if (i == 0) {
+      if (my_att) atomicAdd(&A.counters->att_ticks, my_att);
+      if (my_pos) atomicAdd(&A.counters->pos_ticks, my_pos);
+    }
+  }
+  // the last block to finish advances the device-side step counter (every block has read s0 by then), so that a
+  // captured CUDA graph of single-step launches replays correctly
+  if (threadIdx.x == 0) {
+    __threadfence();
+    uint32_t done = atomicAdd(&A.counters->blocks_done, 1u);
+    if (done == gridDim.x - 1) {
+      uint32_t n_rec = A.record_every > 0
+          ? (s0 + (uint32_t)A.n_steps) / (uint32_t)A.record_every - s0 / (uint32_t)A.record_every : 0u;
+      A.counters->s = s0 + (uint32_t)A.n_steps;
+      A.counters->n_rec_total = rec0 + n_rec;
+      A.counters->blocks_done = 0;
+      __threadfence();
+    }
+  }
+}
+
+// launch table entry points, one translation unit per model (cf_rollout_fp.cu / cf_rollout_ab.cu)
+struct LaunchCfg { int grid, block; size_t smem; cudaStream_t stream; };
+// returns false if (integ, iface, opt) has no instantiation that covers it; *name = instantiation label, *opt_used
+bool launch_fp(int integ, int iface, int opt, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
+               const char **name, int *opt_used, bool dry);
+bool launch_ab(int integ, int iface, int opt, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
+               const char **name, int *opt_used, bool dry);
+
+}  // namespace cf

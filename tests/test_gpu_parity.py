@@ -1,0 +1,305 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the float64 oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json:north_star's:
+  T1 per-step, teacher-forced: |gpu - oracle| <= 1e-4 * max(|oracle|, floor) per state component
+  T2 drift: position error <= 1e-3 m after 1000 free-running steps (hover / tracking runs)
+  T3 bit-exact: Philox words, step / tick counters, record-slot table
+  T4 reset: <= 2e-6 relative
+"""
+import math
+
+import numpy as np
+import pytest
+
+from util import fresh_oracle, split_calls
+
+pytestmark = pytest.mark.gpu
+
+W_HOVER = math.sqrt(0.027 * 9.81 / (4 * 3.16e-10))
+MG = 0.027 * 9.81
+FLOOR_FP = np.array([1] * 3 + [1] * 4 + [1] * 3 + [1] * 3 + [W_HOVER] * 4, dtype=np.float64)
+FLOOR_AB = np.array([1] * 3 + [1] * 3 + [1] * 3 + [1] * 3 + [MG], dtype=np.float64)
+# builder's stricter increment check: rate floors per component
+RATE_FP = np.array([1] * 3 + [1] * 4 + [9.81] * 3 + [100] * 3 + [1e5] * 4, dtype=np.float64)
+RATE_AB = np.array([1] * 3 + [1] * 3 + [9.81] * 3 + [100] * 3 + [MG / 0.03], dtype=np.float64)
+
+
+@pytest.fixture(scope="module")
+def cf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_01478_b200 import build, cf as m
+    build.build()
+    m.lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def W():
+    from paper_2606_01478_b200 import workloads
+    return workloads
+
+
+def fresh_gpu(cf, wl, **extra):
+    sim = cf.Sim(wl.M, wl.N, wl.model, dict(wl.params, **extra))
+    sim.reset(wl.seed)
+    if wl.broadcast_state is not None:
+        sim.set_state(wl.broadcast_state.astype(np.float32), broadcast=True)
+    return sim
+
+
+def floors(model):
+    return (FLOOR_FP, RATE_FP) if model == 0 else (FLOOR_AB, RATE_AB)
+
+
+def assert_state_close(g, o, model, rtol=1e-4, what=""):
+    fl = floors(model)[0][:, None]
+    err = np.abs(g.astype(np.float64) - o) / np.maximum(np.abs(o), fl)
+    j, i = np.unravel_index(np.argmax(err), err.shape)
+    assert err.max() <= rtol, f"{what}: component {j} drone {i}: gpu {g[j, i]} oracle {o[j, i]} rel {err.max():.3e}"
+    return err.max()
+
+
+SMALL = dict(cfg1=dict(M=3, n_steps=150), cfg2=dict(M=300, n_steps=160), cfg3=dict(M=700, n_steps=60),
+             cfg3b=dict(M=500, n_steps=60), cfg4=dict(M=3, N=333, n_steps=60), cfg5=dict(M=300, n_steps=60),
+             cfg5e=dict(M=300, n_steps=60))
+
+
+# ------------------------------------------------------------------------------------------------ T3 Philox
+def test_t3_device_philox_bit_exact_uniform_exact_normals_close(cf, cfo):
+    sim = cf.Sim(1, 1, 0)
+    rng = np.random.default_rng(3)
+    ctr = rng.integers(0, 2 ** 32, (4096, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[:8] = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [1, 2, 3, 4], [7, 0, 999, 1], [5, 0, 0, 2], [5, 0, 1, 2], [5, 1, 0, 2], [6, 0, 0, 3]]
+    seed = 0x0123456789ABCDEF
+    words, uni, nrm = sim.philox_dev(seed, ctr)
+    for k in range(0, 4096, 37):
+        want = cfo.philox(seed, ctr[k])
+        assert np.array_equal(words[k], want), k
+        for c in range(4):
+            assert float(uni[k, c]) == cfo.uniform(int(want[c]))                  # exact in float32 (R18)
+        z = [*cfo.normal_pair(int(want[0]), int(want[1])), *cfo.normal_pair(int(want[2]), int(want[3]))]
+        np.testing.assert_allclose(nrm[k], z, rtol=2e-6, atol=2e-6)
+    w0, _, _ = sim.philox_dev(0, np.zeros((1, 4), dtype=np.uint32))
+    assert [hex(v) for v in w0[0]] == ["0x6627e8d5", "0xe169c58d", "0xbc57ac4c", "0x9b00dbd8"]
+
+
+# ------------------------------------------------------------------------------------------------ T4 reset
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+def test_t4_reset_parity(cf, cfo, W, name):
+    wl = W.make(name, seed=5, **SMALL[name])
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    xs, xo = g.get_state().cpu().numpy(), o.get_state()
+    fl = floors(wl.model)[0][:, None]
+    assert (np.abs(xs - xo) / np.maximum(np.abs(xo), fl)).max() <= 2e-6
+    wg, wo = g.world_params().cpu().numpy(), o.world_params()
+    np.testing.assert_allclose(wg, wo, rtol=2e-6, atol=0)
+    np.testing.assert_allclose(g.ctrl().cpu().numpy(), o.ctrl(), rtol=2e-6, atol=0)
+    assert list(g.counters()) == [0, 0, 0, 0]
+    if wl.params.get("n_obstacles"):
+        assert np.all(np.isinf(g.min_d2().cpu().numpy()))
+
+
+# ------------------------------------------------------------------------------------------------ T1 teacher-forced
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"])
+def test_t1_teacher_forced_single_steps(cf, cfo, W, name):
+    """At >= 20 sampled steps (including controller-tick and command-change steps): widen the GPU's own float32
+    state / controller planes / world parameters / obstacle minima, advance oracle and GPU one step, compare."""
+    wl = W.make(name, seed=1, **SMALL[name])
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    fl, rate = floors(wl.model)
+    h = 1.0 / wl.params["f_phys"]
+    n_checked, worst, worst_rate = 0, 0.0, 0.0
+    t = 0
+    for cm, n, hold in split_calls(wl, [1, 1, 1, 2, 1, 3, 1, 1, 4, 1]):
+        # teacher-force the oracle from the GPU's current float32 data
+        xg = g.get_state().cpu().numpy().astype(np.float64)
+        md = g.min_d2().cpu().numpy().astype(np.float64) if wl.params.get("n_obstacles") else None
+        o.set_full(state=xg, ctrl=g.ctrl().cpu().numpy().astype(np.float64),
+                   wparam=g.world_params().cpu().numpy().astype(np.float64), mind2=md, step_counter=t)
+        g.step(cm, n, cmd_hold=hold)
+        o.step(cm, n, cmd_hold=hold)
+        t += n
+        if n == 1:
+            xn, xo = g.get_state().cpu().numpy().astype(np.float64), o.get_state()
+            worst = max(worst, assert_state_close(xn, xo, wl.model, 1e-4, f"{name} step {t}"))
+            r = np.abs((xn - xg) - (xo - xg)) / h / rate[:, None]
+            worst_rate = max(worst_rate, r.max())
+            if md is not None:
+                np.testing.assert_allclose(g.min_d2().cpu().numpy(), o.min_d2(), rtol=1e-4)
+            n_checked += 1
+    assert n_checked >= 20
+    assert worst_rate <= 2e-3, worst_rate
+    assert list(g.counters())[:3] == list(o.counters())[:3]
+    print(f"{name}: {n_checked} teacher-forced steps, worst rel err {worst:.2e}, worst rate err {worst_rate:.2e}")
+
+
+# ------------------------------------------------------------------------------------------------ free-running
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"])
+def test_free_running_records_counters_and_outputs(cf, cfo, W, name):
+    """The whole run in ONE fused launch vs the oracle: every recorded state, the final state, counters (bit-exact),
+    record table (bit-exact), controller planes, minimum distance."""
+    wl = W.make(name, seed=2, **SMALL[name])
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    rec_every = wl.record_every
+    rg = g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every)
+    ro = o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every)
+    tol = 2e-4      # a short free run: float32 rounding accumulates over <= 160 steps, still far below 1e-3
+    if ro is not None:
+        rgn = rg.cpu().numpy()
+        assert rgn.shape == ro.shape
+        for k in range(ro.shape[0]):
+            assert_state_close(rgn[k], ro[k], wl.model, tol, f"{name} record {k}")
+    assert_state_close(g.get_state().cpu().numpy(), o.get_state(), wl.model, tol, f"{name} final")
+    assert np.array_equal(g.counters(), o.counters())                             # T3
+    assert np.array_equal(g.rec_table(), o.rec_table())                           # T3
+    assert g.step_counter == wl.n_steps
+    co = o.ctrl()
+    cerr = np.abs(g.ctrl().cpu().numpy() - co) / (np.abs(co).max(axis=1, keepdims=True) + 1e-3)
+    assert cerr.max() <= 5e-4, cerr.max(axis=1)
+    if wl.params.get("n_obstacles"):
+        np.testing.assert_allclose(g.min_dist().cpu().numpy(), o.min_dist(), rtol=2e-4, atol=2e-4)
+
+
+def test_t2_drift_hover_config1(cf, cfo, W):
+    """configs[0]: 1000 Euler steps, record every step; position drift <= 1e-3 m, in fused AND single-step mode."""
+    wl = W.cfg1(seed=20260601)
+    o = fresh_oracle(cfo, wl)
+    ro = o.step(wl.cmds, 1000, cmd_hold=1000, record_every=1)
+    g = fresh_gpu(cf, wl)
+    rg = g.step(wl.cmds, 1000, cmd_hold=1000, record_every=1).cpu().numpy()
+    drift = np.abs(rg[:, 0:3, 0] - ro[:, 0:3, 0]).max(axis=1)
+    assert drift[-1] <= 1e-3 and drift.max() <= 1e-3, drift.max()
+    assert_state_close(rg[-1], ro[-1], 0, 1e-3, "cfg1 step 1000")
+    g1 = fresh_gpu(cf, wl)                       # interactive mode: 1000 launches of n_steps = 1
+    recs = [g1.step(wl.cmds, 1, cmd_hold=1, record_every=1) for _ in range(1000)]
+    r1 = np.stack([r.cpu().numpy()[0] for r in recs])
+    np.testing.assert_allclose(r1, rg, rtol=1e-6, atol=1e-7)                       # P20: fused == split
+    assert list(g1.counters()) == [1000, 500, 0, 1000] == list(g.counters())
+    print(f"cfg1 drift after 1000 steps: {drift[-1]:.3e} m (budget 1e-3)")
+
+
+def test_t2_drift_tracking_config4(cf, cfo, W):
+    """configs[3] shape (M=2 worlds): position controller tracking run, 1000 steps, drift <= 1e-3 m."""
+    wl = W.cfg4(seed=20260601, M=2, N=200, n_steps=1000)
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    g.step(wl.cmds, 1000, cmd_hold=1000)
+    o.step(wl.cmds, 1000, cmd_hold=1000)
+    xg, xo = g.get_state().cpu().numpy(), o.get_state()
+    drift = np.abs(xg[0:3] - xo[0:3]).max()
+    assert drift <= 1e-3, drift
+    tgt = wl.cmds[0, :, :3].T
+    assert np.abs(xo[0:3] - tgt).max() < 0.15                                     # it really tracked its targets
+    assert list(g.counters()) == list(o.counters()) == [1000, 0, 200, 0]
+    print(f"cfg4 tracking drift after 1000 steps: {drift:.3e} m")
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+def test_p20_fused_equals_split_on_gpu(cf, W, name):
+    wl = W.make(name, seed=4, **SMALL[name])
+    rec_every = max(wl.record_every, 1)
+    a = fresh_gpu(cf, wl)
+    ra = a.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every).cpu().numpy()
+    b = fresh_gpu(cf, wl)
+    recs = []
+    for cm, n, hold in split_calls(wl, [1, 2, 7, 13]):
+        r = b.step(cm, n, cmd_hold=hold, record_every=rec_every)
+        if r is not None:
+            recs.append(r.cpu().numpy())
+    rb = np.concatenate(recs)
+    fl = floors(wl.model)[0][None, :, None]
+    assert (np.abs(ra - rb) / np.maximum(np.abs(ra), fl)).max() <= 1e-6
+    assert np.array_equal(a.counters(), b.counters()) and np.array_equal(a.rec_table(), b.rec_table())
+
+
+def test_world_offset_shards_reproduce_the_full_run(cf, W):
+    """worlds [lo, lo+m) with world_offset = lo give exactly that slice of the full run."""
+    wl = W.cfg5(seed=9, M=256, n_steps=30)
+    full = fresh_gpu(cf, wl)
+    full.step(wl.cmds, 30, cmd_hold=30)
+    xf = full.get_state().cpu().numpy()
+    for rank in range(2):
+        lo, m = W.shard_worlds(256, 2, rank)
+        sub = cf.Sim(m, 1, wl.model, dict(wl.params, world_offset=lo))
+        sub.reset(wl.seed)
+        sub.step(wl.cmds[:, lo:lo + m], 30, cmd_hold=30)
+        assert np.array_equal(sub.get_state().cpu().numpy(), xf[:, lo:lo + m])
+
+
+def test_host_buffer_path_equals_device_path(cf, W):
+    import torch
+    wl = W.cfg2(seed=6, M=200, n_steps=100)
+    a, b = fresh_gpu(cf, wl), fresh_gpu(cf, wl)
+    ra = a.step(wl.cmds, 100, cmd_hold=wl.cmd_hold, record_every=10).cpu().numpy()
+    ch = torch.from_numpy(wl.cmds).pin_memory()
+    rb = b.step_host(ch, 100, cmd_hold=wl.cmd_hold, record_every=10).numpy()
+    assert np.array_equal(ra, rb)
+    assert np.array_equal(a.get_state().cpu().numpy(), b.get_state_host().numpy())
+    w3 = W.cfg3(seed=6, M=300, n_steps=20)
+    c, d = fresh_gpu(cf, w3), fresh_gpu(cf, w3)
+    c.step(w3.cmds, 20)
+    d.step_host(torch.from_numpy(w3.cmds).pin_memory(), 20)
+    assert np.array_equal(c.min_dist().cpu().numpy(), d.min_dist_host().numpy())
+
+
+def test_edge_cases_and_status_codes(cf, W):
+    import torch
+    sim = cf.Sim(5, 1, 0)
+    cm = torch.zeros((1, 5, 4), device="cuda")
+    with pytest.raises(cf.CfError) as e:
+        sim.step(cm, 1)
+    assert e.value.code == cf.E_STATE
+    sim.reset(1)
+    with pytest.raises(cf.CfError) as e:
+        sim.step(cm, 3, cmd_hold=2)
+    assert e.value.code == cf.E_SHAPE
+    small = torch.empty((1, 17, 5), device="cuda")
+    with pytest.raises(cf.CfError) as e:
+        sim.step(cm, 4, cmd_hold=4, record_every=2, record=small)
+    assert e.value.code == cf.E_BUFFER
+    assert sim.step(cm, 3, cmd_hold=3, record_every=5) is None and sim.step_counter == 3      # no record due yet
+    r = sim.step(cm, 2, cmd_hold=2, record_every=5)                                            # s = 5 -> one record
+    assert r.shape == (1, 17, 5) and list(sim.rec_table()[:2]) == [5, 0]
+    # ragged sizes around warp / block boundaries and a single drone
+    for M in (1, 31, 33, 257):
+        wl = W.cfg2(seed=3, M=M, n_steps=20)
+        g = fresh_gpu(cf, wl)
+        g.step(wl.cmds, 20, cmd_hold=wl.cmd_hold)
+        x = g.get_state().cpu().numpy()
+        assert np.isfinite(x).all() and np.allclose(np.linalg.norm(x[3:7], axis=0), 1, atol=1e-6)
+
+
+def test_general_kernel_fidelity_switches(cf, cfo, W):
+    """The OPT_ALL instantiations: full Eq. (6), thrust/torque polynomials, Eq. (5) gyro, body drag, all four
+    interfaces, RK4 on the abstracted model, simplified AB variant -- teacher-free short runs vs the oracle."""
+    base = W.cfg2(seed=8, M=64, n_steps=40)
+    extras = dict(cv_up=40.0, cv_dn=25.0, cd_up=2e-4, cd_dn=5e-4, Jp=2.0e-8, Ca=[-0.004, -0.004, -0.002],
+                  kf=[1e-3, 2e-7, 3.0e-10], km=[1e-5, 1e-9, 7.9e-12])
+    rng = np.random.default_rng(0)
+    cases = []
+    for integ in (0, 1):
+        cases.append((0, dict(base.params, integrator=integ, **extras), base.cmds))
+        rot = np.zeros((1, 64, 4), dtype=np.float32) + rng.uniform(12000, 17000, (1, 64, 4)).astype(np.float32)
+        cases.append((0, dict(base.params, integrator=integ, iface=0, **extras), rot))
+        tq = np.zeros((1, 64, 4), dtype=np.float32)
+        tq[..., :3] = rng.uniform(-2e-4, 2e-4, (1, 64, 3))
+        tq[..., 3] = 0.3
+        cases.append((0, dict(base.params, integrator=integ, iface=1, **extras), tq))
+        pos = np.zeros((1, 64, 4), dtype=np.float32)
+        pos[..., :3] = rng.uniform(-1, 1, (1, 64, 3)) + [0, 0, 1]
+        pos[..., 3] = rng.uniform(-0.5, 0.5, (1, 64))
+        cases.append((0, dict(base.params, integrator=integ, iface=3, **extras), pos))
+        ab = dict(integrator=integ, f_phys=500.0, init_mode=1, p0_lo=[-1, -1, 0], p0_hi=[1, 1, 2], tilt0_max=0.4,
+                  Ca=[-0.004, -0.004, -0.002], dist_sigma=0.003)
+        cases.append((1, dict(ab, iface=2), base.cmds))
+        cases.append((1, dict(ab, iface=3, ab_thrust_dyn=0), pos))
+    for model, prm, cmds in cases:
+        hold = 50 if cmds.shape[0] > 1 else 40
+        g = cf.Sim(64, 1, model, prm)
+        o = cfo.OracleSim(64, 1, model, prm)
+        g.reset(8), o.reset(8)
+        rg = g.step(cmds, 40, cmd_hold=hold, record_every=8).cpu().numpy()
+        ro = o.step(cmds, 40, cmd_hold=hold, record_every=8)
+        for k in range(5):
+            assert_state_close(rg[k], ro[k], model, 3e-4, f"model {model} iface {prm.get('iface')} integ {prm['integrator']} rec {k}")
+        assert np.array_equal(g.counters(), o.counters())
