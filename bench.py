@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched simulation step (drone-steps/s) on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference] [--no-others]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: for the planning workload (cfg3) that is
+cf_set_state(broadcast) + ONE fused cf_step of 100 sub-steps over 2^20 worlds + the per-world minimum-distance
+read-out; for the recording workloads it is one cf_step call (1000 / 2000 / 500 sub-steps) writing its record buffer.
+One JSON line is printed by rank 0.  Multi-GPU: one process per GPU (torchrun), worlds
+sharded by world_offset with no data-path collective (weak scaling: every rank runs the full per-GPU workload).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC, UNIT = "drone_steps_per_sec", "drone-steps/s"
+DEFAULT_WORKLOAD = "cfg3"
+
+# Algorithmic FP32 operations per drone-step: every add / sub / mul / div / sqrt /
+# trig / log / min / max / clip of the float64 oracle's formulas counts 1 (an FMA is 2); Philox integer work is not
+# counted.  Controller ticks are amortised over their period.
+ALGO_FLOPS = {"cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
+BOUND = {"cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
+SM_COUNT, FP32_LANES = 148, 128
+
+
+def peaks():
+    """Roofline denominators: measured HBM copy bandwidth from MEASURED_PEAKS.json (else the guide's fallback);
+    FP32 ALU peak derived from unit counts and the max SM clock: 148 SMs x 128 lanes x 2 flop x f_max."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    src, hbm, mhz = "fallback", 6650.0, 1965.0
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            hbm, mhz, src = float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+        except Exception:
+            pass
+    return dict(hbm_gbs=hbm, fp32_tflops=SM_COUNT * FP32_LANES * 2 * mhz * 1e6 / 1e12, sm_max_mhz=mhz, source=src)
+
+
+def algo_bytes_per_launch(wl) -> int:
+    """HBM bytes one cf_step launch must move: command loads + recorded states + state / controller / parameter
+    planes in and out once."""
+    MN = wl.MN
+    cmd = (wl.n_cmds * 16 * MN) if wl.params.get("cmd_source", 0) == 0 else wl.n_cmds * 16
+    rec = wl.n_records() * wl.D * 4 * MN
+    ctrl_planes = {0: 3 + 4 + 4, 1: 4 + (3 if wl.params.get("iface") == 3 else 0)}[wl.model]
+    resident = 2 * (wl.D + ctrl_planes) * 4 * MN + (2 * 8 * 4 * MN if wl.params.get("n_obstacles") else 0)
+    wparam = (14 if wl.model == 0 else 11) * 4 * wl.M
+    return cmd + rec + resident + wparam
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx, self.rows, self._stop, self._t = gpu_index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.idx)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx = max(mx, float(r[2]))
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                continue
+        sm.sort()
+        return dict(sm_mhz=sm[len(sm) // 2] if sm else None, sm_max_mhz=mx or None, reasons=sorted(reasons), samples=len(sm))
+
+
+class Runner:
+    """One workload resident on one GPU: device-side step() and host-buffer step_e2e()."""
+
+    def __init__(self, name, device, rank=0, e2e=True):
+        import numpy as np
+        import torch
+        from paper_2606_01478_b200 import cf, workloads as W
+        self.torch, self.name = torch, name
+        host_cmds = name != "cfg3b"
+        wl = W.make(name, **({} if host_cmds else dict(host_cmds=False)))
+        self.wl = wl
+        prm = dict(wl.params, world_offset=rank * wl.M)          # disjoint global worlds per rank (weak scaling)
+        self.sim = cf.Sim(wl.M, wl.N, wl.model, prm, device=device)
+        self.sim.reset(wl.seed)
+        if wl.cmds is not None:
+            self.cmds_host = torch.from_numpy(np.ascontiguousarray(wl.cmds))
+            self.cmds = self.cmds_host.to(device)
+        else:   # cfg3b: 1.7 GB of clipped Gaussian command sequences, drawn on the device (input generation only)
+            g = torch.Generator(device=device).manual_seed(wl.seed)
+            n = wl.notes
+            self.cmds = torch.empty((wl.n_steps, wl.MN, 4), dtype=torch.float32, device=device)
+            for j in range(4):
+                z = torch.randn((wl.n_steps, wl.MN), generator=g, device=device)
+                self.cmds[..., j] = (n["nominal"][j] + n["sigma"][j] * z).clamp_(n["lo"][j], n["hi"][j])
+            self.cmds_host = None
+        self.bstate = None if wl.broadcast_state is None else torch.from_numpy(wl.broadcast_state.astype(np.float32)).to(device)
+        n_rec = wl.n_records()
+        self.record = torch.empty((n_rec, wl.D, wl.MN), dtype=torch.float32, device=device) if n_rec else None
+        self.obst = bool(wl.params.get("n_obstacles"))
+        self.min_dist = torch.empty(wl.M, dtype=torch.float32, device=device) if self.obst else None
+        self.launches_per_step = 1 + (self.bstate is not None) + self.obst
+        self.kernel, self.grid, self.block = self.sim.describe_launch()
+        # host side buffers for the end-to-end path (pinned)
+        self.e2e_ok = e2e and self.cmds_host is not None
+        if self.e2e_ok:
+            self.cmds_pin = self.cmds_host.pin_memory()
+            self.rec_pin = torch.empty((n_rec, wl.D, wl.MN), dtype=torch.float32, pin_memory=True) if n_rec else None
+            self.state_pin = torch.empty((wl.D, wl.MN), dtype=torch.float32, pin_memory=True)
+            self.md_pin = torch.empty(wl.M, dtype=torch.float32, pin_memory=True) if self.obst else None
+            self.bstate_pin = None if self.bstate is None else self.bstate.cpu().pin_memory()
+            self.h2d = self.cmds_pin.numel() * 4 + (0 if self.bstate is None else self.bstate.numel() * 4)
+            self.d2h = (self.rec_pin.numel() * 4 if n_rec else self.state_pin.numel() * 4) + (wl.M * 4 if self.obst else 0)
+
+    def step(self):
+        wl, sim = self.wl, self.sim
+        if self.bstate is not None:
+            sim.set_state(self.bstate, broadcast=True)
+        sim.step(self.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every, record=self.record)
+        if self.obst:
+            sim.min_dist(out=self.min_dist)
+
+    def rollout_only(self):
+        wl = self.wl
+        self.sim.step(self.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every, record=self.record)
+
+    def step_e2e(self):
+        """The same step through the C ABI with HOST buffers: H2D of this step's inputs and D2H of its results
+        (records, or final state + min distance when nothing is recorded) inside the call."""
+        wl, sim = self.wl, self.sim
+        if self.bstate_pin is not None:
+            self.bstate.copy_(self.bstate_pin, non_blocking=True)
+            sim.set_state(self.bstate, broadcast=True)
+        sim.step_host(self.cmds_pin, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every, record_host=self.rec_pin)
+        if self.rec_pin is None:
+            sim.get_state_host(self.state_pin)
+        if self.obst:
+            sim.min_dist_host(self.md_pin)
+
+
+def time_steps(fn, torch, steps, warmup, flush, barrier=None):
+    """W untimed warm-ups, then exactly K steps, each bracketed by CUDA events on the launching (current) stream,
+    with an L2 flush (a write larger than L2) between timed iterations.  Returns per-step ms list."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        if flush is not None:
+            flush.fill_(1)
+        a.record()
+        fn()
+        b.record()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def time_host_steps(fn, torch, steps, warmup):
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        fn()                       # synchronous: returns after the D2H copy completed
+        ts.append((time.perf_counter() - t0) * 1e3)
+    return ts
+
+
+def oracle_sample(name, target_seconds=12.0, threads=None):
+    """Time the float64 oracle, as it stands, on the host cores, on a bounded sample of the same workload: the same
+    recipe at a reduced number of worlds / steps (per-drone work is independent of M)."""
+    import numpy as np
+    from oracle import cfo
+    from paper_2606_01478_b200 import workloads as W
+    if threads:
+        cfo.set_num_threads(threads)
+    small = dict(cfg1=dict(M=1, n_steps=1000), cfg2=dict(M=64, n_steps=200), cfg3=dict(M=512, n_steps=100),
+                 cfg3b=dict(M=512, n_steps=100), cfg4=dict(M=1, N=512, n_steps=100), cfg5=dict(M=64, n_steps=200),
+                 cfg5e=dict(M=64, n_steps=200))[name]
+
+    def run(kw):
+        wl = W.make(name, **kw)
+        sim = cfo.OracleSim(wl.M, wl.N, wl.model, wl.params)
+        sim.reset(wl.seed)
+        if wl.broadcast_state is not None:
+            sim.set_state(wl.broadcast_state, broadcast=True)
+        t0 = time.perf_counter()
+        sim.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every)
+        if wl.params.get("n_obstacles"):
+            sim.min_dist()
+        return wl.drone_steps / (time.perf_counter() - t0), wl
+
+    rate, _ = run(small)                                     # calibration
+    kw = dict(small)
+    if name != "cfg1":
+        scale = max(1.0, rate * target_seconds / (small.get("M", 1) * small.get("N", 1) * small["n_steps"]))
+        kw["M"] = int(min(small["M"] * scale, {"cfg4": 256}.get(name, 1 << 22)))
+    rate, wl = run(kw)
+    sample = f"{wl.M} worlds x {wl.N} drones x {wl.n_steps} steps of {name} (same recipe, reduced M)"
+    return rate, cfo.num_threads(), sample, wl
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-others", action="store_true", help="skip the secondary workloads and the CPU baseline")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    name = args.workload
+
+    if args.impl == "reference":
+        # the reference arm of this tier IS the oracle, timed on the host cores; rank 0 only
+        if rank != 0:
+            return 0
+        from paper_2606_01478_b200 import workloads as W
+        full = W.make(name) if name != "cfg3b" else W.make(name, host_cmds=False)
+        rates = []
+        for i in range(args.warmup + args.steps):
+            r, cores, sample, wl = oracle_sample(name, target_seconds=max(2.0, 60.0 / max(1, args.steps)))
+            if i >= args.warmup:
+                rates.append((r, wl.drone_steps))
+        tot = sum(d for _, d in rates)
+        secs = sum(d / r for r, d in rates)
+        value = tot / secs
+        line = dict(metric=METRIC, value=value, unit=UNIT, impl="reference", n_gpus=args.gpus, steps=args.steps,
+                    warmup=args.warmup, ms_per_step=1e3 * secs / len(rates), higher_is_better=True, scaling="weak",
+                    vs_baseline=None, dtype="f64", data="synthetic",
+                    config=dict(workload=name, M=full.M, N=full.N, sub_steps=full.n_steps, note="bounded sample per step"),
+                    cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                    e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+        print(json.dumps(line))
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    from paper_2606_01478_b200 import build
+    build.build()
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+    barrier = None
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+        barrier = dist.barrier
+    pk = peaks()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)     # 256 MiB > 126 MB L2
+
+    def measure(nm, steps, warmup, want_e2e):
+        R = Runner(nm, device, rank=rank, e2e=want_e2e)
+        wl = R.wl
+        with ClockSampler(local) as cs:
+            ms = time_steps(R.step, torch, steps, warmup, flush, barrier)
+        kms = time_steps(R.rollout_only, torch, max(3, min(steps, 10)), 1, flush)     # dominant kernel alone
+        t = torch.tensor([sum(ms)], dtype=torch.float64, device=device)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        value = world * wl.drone_steps * steps / (total_ms * 1e-3)
+        k_ms = sum(kms) / len(kms)
+        if BOUND[nm] == "hbm":
+            ach = algo_bytes_per_launch(wl) / (k_ms * 1e-3) / 1e9
+            roof = dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"], traffic=None,
+                        peak_source=pk["source"])
+        else:
+            ach = ALGO_FLOPS[nm] * wl.drone_steps / (k_ms * 1e-3) / 1e12
+            roof = dict(bound="alu", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
+                        traffic=None, peak_source=f"148 SM x 128 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz")
+        roof.update(kernel=R.kernel, kernel_ms=k_ms, grid=R.grid, block=R.block,
+                    hbm_gbs_algorithmic=algo_bytes_per_launch(wl) / (k_ms * 1e-3) / 1e9,
+                    algo_flops_per_drone_step=ALGO_FLOPS[nm], algo_bytes_per_launch=algo_bytes_per_launch(wl))
+        out = dict(value=value, ms_per_step=total_ms / steps, roofline=roof, clocks=cs.summary(),
+                   gpu_launches=R.launches_per_step * steps, M=wl.M, N=wl.N, sub_steps=wl.n_steps,
+                   record_every=wl.record_every, drone_steps_per_step=wl.drone_steps)
+        if want_e2e and R.e2e_ok:
+            ems = time_host_steps(R.step_e2e, torch, max(2, min(steps, 5)), 1)
+            et = torch.tensor([sum(ems) / len(ems)], dtype=torch.float64, device=device)
+            if world > 1:
+                dist.all_reduce(et, op=dist.ReduceOp.MAX)
+            out["e2e"] = dict(value=world * wl.drone_steps / (float(et.item()) * 1e-3), unit=UNIT,
+                              h2d_bytes_per_step=R.h2d, d2h_bytes_per_step=R.d2h, ms_per_step=float(et.item()))
+        del R
+        torch.cuda.empty_cache()
+        return out
+
+    main_res = measure(name, args.steps, args.warmup, not args.no_e2e)
+    others = {}
+    if not args.no_others and world == 1:
+        for nm in ("cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"):
+            if nm == name:
+                continue
+            r = measure(nm, 5, 3, False)
+            others[nm] = dict(value=r["value"], ms_per_step=r["ms_per_step"], roofline=r["roofline"], M=r["M"], N=r["N"],
+                              sub_steps=r["sub_steps"], record_every=r["record_every"])
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_others:
+        rate, cores, sample, _ = oracle_sample(name)
+        cpu = dict(value=rate, unit=UNIT, cores=cores, kind="oracle", sample=sample)
+    if rank == 0:
+        line = dict(metric=METRIC, value=main_res["value"], unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                    ms_per_step=main_res["ms_per_step"], higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype="f32", data="synthetic",
+                    config=dict(workload=name, M_per_gpu=main_res["M"], N=main_res["N"], sub_steps_per_step=main_res["sub_steps"],
+                                record_every=main_res["record_every"], drone_steps_per_step_per_gpu=main_res["drone_steps_per_step"],
+                                l2="flushed between timed steps (256 MiB write)", parallelism=f"worlds sharded x{world}, no collective"),
+                    roofline=main_res["roofline"], cpu_baseline=cpu, e2e=main_res.get("e2e"), clocks=main_res["clocks"],
+                    gpu_launches=main_res["gpu_launches"], workloads=others)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

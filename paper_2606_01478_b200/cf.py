@@ -273,7 +273,9 @@ class Sim:
         torch = _torch()
         if out is None:
             out = torch.empty(self.M, dtype=torch.float32, pin_memory=True)
-        scratch = torch.empty(self.M, dtype=torch.float32, device=self.device)
+        if getattr(self, "_md_scratch", None) is None:
+            self._md_scratch = torch.empty(self.M, dtype=torch.float32, device=self.device)
+        scratch = self._md_scratch
         _check(lib().cf_get_aux_host(self._h, AUX_MIN_DIST, C.c_void_p(out.data_ptr()), _dptr(scratch), self.M * 4))
         return out
 
@@ -286,8 +288,11 @@ class Sim:
     def counters(self):
         return self._aux(AUX_COUNTERS, (4,), _torch().int32).cpu().numpy().view(np.uint32)
 
-    def min_dist(self):
-        return self._aux(AUX_MIN_DIST, (self.M,), _torch().float32)
+    def min_dist(self, out=None):
+        if out is None:
+            return self._aux(AUX_MIN_DIST, (self.M,), _torch().float32)
+        _check(lib().cf_get_aux(self._h, AUX_MIN_DIST, _dptr(out)))
+        return out
 
     def ctrl(self):
         return self._aux(AUX_CTRL, (14, self.MN), _torch().float32)

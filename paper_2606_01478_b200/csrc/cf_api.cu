@@ -310,6 +310,20 @@ __global__ void min_dist_kernel(const float *min_d2, float *out, long long M, lo
   if (lane == 0) out[w] = best;
 }
 
+// N small (single drone per world): one thread per world, coalesced over worlds
+__global__ void min_dist_small_n_kernel(const float *min_d2, float *out, long long M, long long N, long long MN,
+                                        const __grid_constant__ DevParams P) {
+  long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= M) return;
+  float best = __int_as_float(0x7f800000);
+  for (long long n = 0; n < N; ++n) {
+#pragma unroll
+    for (int j = 0; j < kMaxObst; ++j)
+      if (j < P.n_obst) best = fminf(best, sqrtf(min_d2[j * MN + w * N + n]) - P.obst[j][3]);
+  }
+  out[w] = best;
+}
+
 __global__ void philox_debug_kernel(uint32_t seed_lo, uint32_t seed_hi, const uint32_t *ctr, int n, uint32_t *words,
                                     float *uni, float *nrm) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -564,8 +578,12 @@ static int aux_source(cf_sim *sim, int which, const void **src, size_t *bytes) {
 
 static int launch_min_dist(cf_sim *sim, float *out_dev) {
   if (!sim->min_d2) return fail(CF_E_ARG, "no obstacles configured");
-  long long threads = sim->M * 32;
-  min_dist_kernel<<<grid_for(threads, 128), 128, 0, sim->stream>>>(sim->min_d2, out_dev, sim->M, sim->N, sim->MN, sim->dp);
+  if (sim->N < 8) {
+    min_dist_small_n_kernel<<<grid_for(sim->M, 256), 256, 0, sim->stream>>>(sim->min_d2, out_dev, sim->M, sim->N, sim->MN, sim->dp);
+  } else {
+    long long threads = sim->M * 32;
+    min_dist_kernel<<<grid_for(threads, 128), 128, 0, sim->stream>>>(sim->min_d2, out_dev, sim->M, sim->N, sim->MN, sim->dp);
+  }
   CF_CUDA(cudaGetLastError());
   return CF_OK;
 }
