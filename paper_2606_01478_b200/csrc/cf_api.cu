@@ -452,13 +452,14 @@ extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctr
   return CF_OK;
 }
 
-// launch geometry: small problems are latency-bound -> small blocks spread over all SMs; large ones use 128/256.
+// launch geometry.  One wave always suffices for the paper's sizes up to ~600k drones (64 warps/SM x 148 SMs), so the
+// block size only decides how evenly the warps spread over the 148 SMs: the fewer warps per SM, the smaller the block.
 static int pick_block(long long MN) {
-  const long long sms = 148;
-  if (MN >= sms * 256 * 8) return 256;
-  if (MN >= sms * 128 * 2) return 128;
-  if (MN >= sms * 64) return 64;
-  return 32;
+  const long long sms = 148, warps = (MN + 31) / 32;
+  if (warps <= sms * 16) return 32;
+  if (warps <= sms * 32) return 64;
+  if (warps <= sms * 64) return 128;
+  return 256;
 }
 
 static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name, int *grid, int *block) {

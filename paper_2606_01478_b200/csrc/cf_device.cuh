@@ -87,16 +87,42 @@ __host__ __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1,
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// reading R18: 23-bit midpoint uniform in (0,1), exact in float32
-__device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * (1.0f / 8388608.0f); }
+// ---------------------------------------------------------------------------------------------------------------
+// Special-function unit (MUFU) approximations.  The rollout loop is instruction-issue bound (profiles/), so the
+// transcendental work goes to the otherwise idle XU pipe instead of ~30-instruction FMA-pipe software routines.
+// Error budget: sin/cos.approx abs err <= 2^-20.9 on [-2pi, 2pi],
+// lg2.approx abs err <= 2^-22 on the logarithm, sqrt.approx <= 2 ulp -- all >= 2 orders below the 1e-4 per-step bar.
+__device__ __forceinline__ float mufu_sin(float x) { float y; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_cos(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
-// Box-Muller (C9): r = sqrt(-2 ln ua), (z0, z1) = r (cos 2 pi ub, sin 2 pi ub).  sincospi keeps the angle exact.
+// sin / cos of a physical angle inside the step loop.  |x| <= 2 pi: MUFU; beyond (never in the paper's workloads,
+// attitude commands are clipped to +-pi) the accurate library routine, so the result is defined for any input.
+__device__ __forceinline__ void sincos_step(float x, float *s, float *c) {
+  if (fabsf(x) <= 6.2831853f) { *s = mufu_sin(x); *c = mufu_cos(x); }
+  else sincosf(x, s, c);
+}
+
+// reading R18: 23-bit midpoint uniform in (0,1), exact in float32:  u = ((x >> 9) + 0.5) 2^-23.
+// Built as the float 1.m (m = x >> 9) minus (1 - 2^-24): both are multiples of 2^-24, the difference is exact.
+__device__ __forceinline__ float u01(uint32_t x) {
+  return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994f;
+}
+// 2 pi (u - 1/2): 1.m - 1.5 is exact (a multiple of 2^-23 in [-1/2, 1/2)); the half-ulp offset 2^-24 enters through
+// the FMA's addend.  The Box-Muller angle is thus taken on (-pi, pi), where MUFU sin/cos are accurate.
+__device__ __forceinline__ float angle_centered(uint32_t x) {
+  float t = __uint_as_float(0x3F800000u | (x >> 9)) - 1.5f;
+  return fmaf(t, 6.28318530718f, 6.28318530718f * 5.9604644775390625e-8f);
+}
+
+// Box-Muller (C9): r = sqrt(-2 ln ua), (z0, z1) = r (cos 2 pi ub, sin 2 pi ub).
+// cos(2 pi ub) = -cos(2 pi (ub - 1/2)) and likewise for sin, so the sign goes into r.
 __device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, float &z0, float &z1) {
-  float ua = u01(xa), ub = u01(xb);
-  float r = sqrtf(-2.0f * logf(ua));
-  float s, c;
-  sincospif(2.0f * ub, &s, &c);
-  z0 = r * c; z1 = r * s;
+  float ua = u01(xa);
+  float ang = angle_centered(xb);
+  float r = -mufu_sqrt(-1.38629436112f * mufu_lg2(ua));     // -2 ln u = -2 ln2 * lg2 u
+  z0 = r * mufu_cos(ang); z1 = r * mufu_sin(ang);
 }
 
 __device__ __forceinline__ float clipf(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
@@ -247,7 +273,7 @@ __device__ __forceinline__ void deriv_ab(const DevParams &P, const Plant<MODEL_A
                                          const float *u, const float *fdist, float *dx) {
   constexpr bool EX = (OPT & OPT_EXTRAS) != 0;
   float sr, cr, sp, cp, sy, cy;
-  sincosf(x[3], &sr, &cr); sincosf(x[4], &sp, &cp); sincosf(x[5], &sy, &cy);
+  sincos_step(x[3], &sr, &cr); sincos_step(x[4], &sp, &cp); sincos_step(x[5], &sy, &cy);
   float zx = cy * sp * cr + sy * sr, zy = sy * sp * cr - cy * sr, zz = cp * cr;
   float fS = (EX && !P.ab_thrust_dyn) ? u[3] : x[12];
   float acc = (P.ab_cf * fS) * pl.inv_m;
@@ -332,7 +358,7 @@ __device__ __forceinline__ void mixer(const DevParams &P, float Fc, const float 
       float disc = fmaxf(P.kf[1] * P.kf[1] - 4.0f * P.kf[2] * (P.kf[0] - fk), 0.0f);
       r = (sqrtf(disc) - P.kf[1]) * (0.5f * P.inv_kf2);
     } else {
-      r = sqrtf(fk * P.inv_kf2);
+      r = mufu_sqrt(fk * P.inv_kf2);
     }
     rpm_cmd[k] = clipf(r, P.rpm_min, P.rpm_max);
   }

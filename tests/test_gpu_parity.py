@@ -79,7 +79,7 @@ def test_t3_device_philox_bit_exact_uniform_exact_normals_close(cf, cfo):
         for c in range(4):
             assert float(uni[k, c]) == cfo.uniform(int(want[c]))                  # exact in float32 (R18)
         z = [*cfo.normal_pair(int(want[0]), int(want[1])), *cfo.normal_pair(int(want[2]), int(want[3]))]
-        np.testing.assert_allclose(nrm[k], z, rtol=2e-6, atol=2e-6)
+        np.testing.assert_allclose(nrm[k], z, rtol=4e-6, atol=4e-6)
     w0, _, _ = sim.philox_dev(0, np.zeros((1, 4), dtype=np.uint32))
     assert [hex(v) for v in w0[0]] == ["0x6627e8d5", "0xe169c58d", "0xbc57ac4c", "0x9b00dbd8"]
 
