@@ -162,7 +162,15 @@ static void fill_dev_params(cf_sim *s) {
   d.rpm_min = p.rpm_min; d.rpm_max = p.rpm_max; d.thrust_min = p.thrust_min; d.thrust_max = p.thrust_max;
   d.tilt_max = p.tilt_max; d.iR_max = p.iR_max; d.dist_sigma = p.dist_sigma; d.n_obst = p.n_obstacles;
   d.use_noise = p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE;
-  for (int j = 0; j < kMaxObst; ++j) for (int k = 0; k < 4; ++k) d.obst[j][k] = p.obstacles[j][k];
+  for (int j = 0; j < kMaxObst; ++j) {
+    for (int k = 0; k < 4; ++k) d.obst[j][k] = p.obstacles[j][k];
+    if (j < p.n_obstacles) {
+      double cx = p.obstacles[j][0], cy = p.obstacles[j][1], cz = p.obstacles[j][2];
+      d.obst_q[j] = make_float4((float)(-2 * cx), (float)(-2 * cy), (float)(-2 * cz), (float)(cx * cx + cy * cy + cz * cz));
+    } else {
+      d.obst_q[j] = make_float4(0.f, 0.f, 0.f, INFINITY);
+    }
+  }
   for (int k = 0; k < 4; ++k) { d.noise_sigma[k] = p.noise_sigma[k]; d.cmd_lo[k] = p.cmd_lo[k]; d.cmd_hi[k] = p.cmd_hi[k]; }
 }
 
@@ -507,6 +515,10 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.world_offset = sim->p.world_offset;
   A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.record_every = record_every; A.n_rec_cap = (int)n_rec;
   A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);
+  for (int r = 0; r < 10; ++r) {      // Philox key schedule: k += (0x9E3779B9, 0xBB67AE85) per round
+    A.rk[2 * r] = A.seed_lo + (uint32_t)r * 0x9E3779B9u;
+    A.rk[2 * r + 1] = A.seed_hi + (uint32_t)r * 0xBB67AE85u;
+  }
   int rc = do_launch(sim, &A, false, nullptr, nullptr, nullptr);
   if (rc != CF_OK) return rc;
   CF_CUDA(cudaGetLastError());

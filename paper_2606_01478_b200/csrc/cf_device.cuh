@@ -48,7 +48,8 @@ struct DevParams {
   float dist_sigma;
   int   use_noise;   // cmd_source == CF_CMD_NOMINAL_PLUS_NOISE
   int   n_obst;
-  float obst[kMaxObst][4];
+  float obst[kMaxObst][4];        // cx cy cz r (read-out)
+  float4 obst_q[kMaxObst];        // (-2cx, -2cy, -2cz, c.c): d^2 = |p|^2 + q.(p,1); unused slots (0,0,0,+inf)
   float noise_sigma[4], cmd_lo[4], cmd_hi[4];
   int   att_div, pos_div;
 };
@@ -65,6 +66,7 @@ struct StepArgs {
   long long MN, M, N, world_offset;
   int n_steps, cmd_hold, record_every, n_rec_cap;
   uint32_t seed_lo, seed_hi;
+  uint32_t rk[20];         // Philox round keys (k0_r, k1_r), r = 0..9, precomputed on the host from the seed
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -102,6 +104,30 @@ __device__ __forceinline__ float mufu_sqrt(float x) { float y; asm("sqrt.approx.
 __device__ __forceinline__ void sincos_step(float x, float *s, float *c) {
   if (fabsf(x) <= 6.2831853f) { *s = mufu_sin(x); *c = mufu_cos(x); }
   else sincosf(x, s, c);
+}
+
+// the same 10 rounds with the key schedule precomputed (uniform per launch): 2 IMAD.WIDE + 2 LOP3 per round
+__device__ __forceinline__ void philox4x32_10_rk(const uint32_t (&rk)[20], uint32_t c0, uint32_t c1, uint32_t c2,
+                                                 uint32_t c3, uint32_t out[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ rk[2 * r], n2 = hi0 ^ c3 ^ rk[2 * r + 1];
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// the three Euler angles at once: one range check for all
+__device__ __forceinline__ void sincos3_step(const float *a, float *s, float *c) {
+  if (fmaxf(fmaxf(fabsf(a[0]), fabsf(a[1])), fabsf(a[2])) <= 6.2831853f) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { s[j] = mufu_sin(a[j]); c[j] = mufu_cos(a[j]); }
+  } else {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) sincosf(a[j], &s[j], &c[j]);
+  }
 }
 
 // reading R18: 23-bit midpoint uniform in (0,1), exact in float32:  u = ((x >> 9) + 0.5) 2^-23.
@@ -272,8 +298,9 @@ template <int OPT>
 __device__ __forceinline__ void deriv_ab(const DevParams &P, const Plant<MODEL_AB, OPT> &pl, const float *x,
                                          const float *u, const float *fdist, float *dx) {
   constexpr bool EX = (OPT & OPT_EXTRAS) != 0;
-  float sr, cr, sp, cp, sy, cy;
-  sincos_step(x[3], &sr, &cr); sincos_step(x[4], &sp, &cp); sincos_step(x[5], &sy, &cy);
+  float sn[3], cs[3];
+  sincos3_step(x + 3, sn, cs);
+  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
   float zx = cy * sp * cr + sy * sr, zy = sy * sp * cr - cy * sr, zz = cp * cr;
   float fS = (EX && !P.ab_thrust_dyn) ? u[3] : x[12];
   float acc = (P.ab_cf * fS) * pl.inv_m;
@@ -487,10 +514,11 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     int att_phase = (int)(s0 % (uint32_t)P.att_div), pos_phase = (int)(s0 % (uint32_t)P.pos_div);
     int rec_phase = A.record_every > 0 ? (int)(s0 % (uint32_t)A.record_every) : 0;
     int rec_slot = 0;
-    int cmd_cd = 0, cmd_k = 0;
+    int cmd_cd = 0;
     const bool noise = (OPT & OPT_NOISE) != 0 && P.use_noise;   // compiled in AND requested
-    const float4 *cp = noise ? A.cmds : A.cmds + i;
+    const float4 *cp = noise ? A.cmds : A.cmds + i;             // next command to prefetch
     const long long cstride = noise ? 1 : MN;
+    int cmds_left = (A.n_steps + A.cmd_hold - 1) / A.cmd_hold;  // commands this call consumes
     float4 next_cmd = __ldg(cp);
 
     for (int t = 0; t < A.n_steps; ++t) {
@@ -498,12 +526,11 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       if (cmd_cd == 0) {
         float4 c4 = next_cmd;
         cmd_cd = A.cmd_hold;
-        ++cmd_k;
-        if ((long long)cmd_k * A.cmd_hold < A.n_steps) next_cmd = __ldg(cp + cmd_k * cstride);
+        if (--cmds_left > 0) { cp += cstride; next_cmd = __ldg(cp); }
         float c[4] = { c4.x, c4.y, c4.z, c4.w };
         if (noise) {
           uint32_t r[4]; float z[4];
-          philox4x32_10(A.seed_lo, A.seed_hi, wg, nn, s, STREAM_NOISE, r);
+          philox4x32_10_rk(A.rk, wg, nn, s, STREAM_NOISE, r);
           normal_pair(r[0], r[1], z[0], z[1]);
           normal_pair(r[2], r[3], z[2], z[3]);
 #pragma unroll
@@ -556,7 +583,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       float fdist[3] = { 0, 0, 0 };
       if ((OPT & OPT_DIST) && P.dist_sigma > 0.0f) {
         uint32_t r[4]; float z[4];
-        philox4x32_10(A.seed_lo, A.seed_hi, wg, nn, s, STREAM_DIST, r);
+        philox4x32_10_rk(A.rk, wg, nn, s, STREAM_DIST, r);
         normal_pair(r[0], r[1], z[0], z[1]);
         normal_pair(r[2], r[3], z[2], z[3]);
 #pragma unroll
@@ -567,12 +594,13 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       ++s;
       // (7) obstacle minima (squared centre distance; the square roots are taken once, at read-out)
       if (obst) {
+        // |p - c_j|^2 = |p|^2 + (c_j.c_j - 2 c_j.p): 3 FFMA + FADD + FMNMX per sphere, constants straight from the
+        // uniform bank; unused slots hold (0,0,0,+inf) and never win the minimum
+        float pp = fmaf(x[2], x[2], fmaf(x[1], x[1], x[0] * x[0]));
 #pragma unroll
         for (int j = 0; j < kMaxObst; ++j) {
-          if (j < P.n_obst) {
-            float dx_ = x[0] - P.obst[j][0], dy_ = x[1] - P.obst[j][1], dz_ = x[2] - P.obst[j][2];
-            md2[j] = fminf(md2[j], dx_ * dx_ + dy_ * dy_ + dz_ * dz_);
-          }
+          float tq = fmaf(P.obst_q[j].z, x[2], fmaf(P.obst_q[j].y, x[1], fmaf(P.obst_q[j].x, x[0], P.obst_q[j].w)));
+          md2[j] = fminf(md2[j], tq + pp);
         }
       }
       // (8) record (streaming stores; a warp writes whole 128-byte lines of each plane)
