@@ -474,7 +474,9 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
   LaunchCfg L;
   L.block = pick_block(sim->MN);
   L.grid = grid_for(sim->MN, L.block);
-  L.smem = ((sim->opt & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
+  size_t smem_wp = ((sim->opt & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
+  size_t smem_rec = (A && A->rec_tiled) ? sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
+  L.smem = smem_wp > smem_rec ? smem_wp : smem_rec;
   L.stream = sim->stream;
   if (grid) *grid = L.grid;
   if (block) *block = L.block;
@@ -514,6 +516,7 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   A.cmds = (const float4 *)cmds_dev; A.record = record_dev;
   A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.world_offset = sim->p.world_offset;
   A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.record_every = record_every; A.n_rec_cap = (int)n_rec;
+  A.rec_tiled = (n_rec > 0 && sim->MN % 32 == 0 && ((uintptr_t)record_dev & 15) == 0) ? 1 : 0;
   A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);
   for (int r = 0; r < 10; ++r) {      // Philox key schedule: k += (0x9E3779B9, 0xBB67AE85) per round
     A.rk[2 * r] = A.seed_lo + (uint32_t)r * 0x9E3779B9u;

@@ -65,6 +65,8 @@ struct StepArgs {
   float *record;           // [n_rec][D][MN]
   long long MN, M, N, world_offset;
   int n_steps, cmd_hold, record_every, n_rec_cap;
+  int rec_tiled;           // 1: records leave as 16-byte stores after a shared-memory transpose (needs MN % 32 == 0,
+                           //    16-byte aligned record buffer); 0: one 4-byte store per component
   uint32_t seed_lo, seed_hi;
   uint32_t rk[20];         // Philox round keys (k0_r, k1_r), r = 0..9, precomputed on the host from the seed
 };
@@ -450,7 +452,8 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   constexpr bool FP = MODEL == MODEL_FP;
   constexpr bool HAS_ATT = FP && IFACE >= IF_ATTITUDE;       // attitude controller + mixer active
   constexpr bool HAS_POS = IFACE == IF_POSITION;
-  extern __shared__ float wp_s[];                            // [NP][span]: per-world parameters of this block (N > 1)
+  extern __shared__ __align__(128) float wp_s[];             // [NP][span] per-world parameters of this block (N > 1);
+                                                             // afterwards [warps][D][32] record staging tiles
 
   const long long MN = A.MN;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -473,6 +476,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     }
     __syncthreads();
     if (active) pl.load(P, wp_s, span, w - w_first, true);
+    __syncthreads();                                         // wp_s is reused for the record tiles below
   } else if (active) {
     pl.load(P, A.wparam, A.M, w, (OPT & OPT_RANDP) != 0);
   }
@@ -514,6 +518,11 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     int att_phase = (int)(s0 % (uint32_t)P.att_div), pos_phase = (int)(s0 % (uint32_t)P.pos_div);
     int rec_phase = A.record_every > 0 ? (int)(s0 % (uint32_t)A.record_every) : 0;
     int rec_slot = 0;
+    const int lane = threadIdx.x & 31;
+    // record staging: the warp's snapshot is a [D][32] tile = D*8 16-byte chunks; lane L stores chunks L, L+32, ...:
+    // chunk c is row c/8 (component), columns 4(c%8)..+3 (drones), so successive chunks of a lane are 4 rows apart
+    float *rec_tile = wp_s + (threadIdx.x >> 5) * (D * 32);
+    float *rec_ptr = A.record + (size_t)(lane >> 3) * MN + (i - lane) + 4 * (lane & 7);
     int cmd_cd = 0;
     const bool noise = (OPT & OPT_NOISE) != 0 && P.use_noise;   // compiled in AND requested
     const float4 *cp = noise ? A.cmds : A.cmds + i;             // next command to prefetch
@@ -608,9 +617,27 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         if (++rec_phase == A.record_every) {
           rec_phase = 0;
           if (rec_slot < A.n_rec_cap) {
-            float *r = A.record + (size_t)rec_slot * D * MN + i;
+            if (A.rec_tiled) {
+              __syncwarp();                           // everyone has read the previous snapshot out of the tile
 #pragma unroll
-            for (int j = 0; j < D; ++j) __stcs(r + j * MN, x[j]);
+              for (int j = 0; j < D; ++j) rec_tile[j * 32 + lane] = x[j];
+              __syncwarp();
+              constexpr int ROUNDS = (D * 8 + 31) / 32;
+              float *dst = rec_ptr;
+#pragma unroll
+              for (int m = 0; m < ROUNDS; ++m) {
+                if (m * 32 + lane < D * 8) {
+                  float4 v = *reinterpret_cast<const float4 *>(rec_tile + (m * 32 + lane) * 4);
+                  __stcs(reinterpret_cast<float4 *>(dst), v);
+                }
+                dst += 4 * MN;
+              }
+              rec_ptr += (size_t)D * MN;
+            } else {
+              float *r = A.record + (size_t)rec_slot * D * MN + i;
+#pragma unroll
+              for (int j = 0; j < D; ++j) __stcs(r + j * MN, x[j]);
+            }
             if (i == 0 && rec0 + (uint32_t)rec_slot < (uint32_t)kRecTableCap) A.rec_table[rec0 + rec_slot] = s;
           }
           ++rec_slot;
