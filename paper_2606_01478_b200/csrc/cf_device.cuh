@@ -162,14 +162,24 @@ template <int MODEL, int OPT> struct Plant;
 template <int OPT> struct Plant<MODEL_FP, OPT> {
   float inv_m, inv_J[3], cJ[3];      // cJ = ((Jy-Jz)/Jx, (Jz-Jx)/Jy, (Jx-Jy)/Jz): Euler's equation cross term
   float kf2, km2, cv;                // lean rotor / thrust model
+  float kfm2, ct[3];                 // lean: 2 kf2/m ; (l kf2/Jx, l kf2/Jy, km2/Jz)
+  float rc2, rc3, rc4, rho4, rho1;   // lean: closed-form first-order rotor lag inside RK4 / Euler, z = h cv (see integrate_fp_lean)
   float J[3], kf0, kf1, km0, km1, cv_dn, cd_up, cd_dn;   // only read when OPT_EXTRAS
 
-  __device__ __forceinline__ void set(float m, float Jx, float Jy, float Jz, const float kf[3], const float km[3],
-                                      float cvu, float cvd, float cdu, float cdd) {
+  __device__ __forceinline__ void set(const DevParams &P, float m, float Jx, float Jy, float Jz, const float kf[3],
+                                      const float km[3], float cvu, float cvd, float cdu, float cdd) {
     inv_m = 1.0f / m;
     inv_J[0] = 1.0f / Jx; inv_J[1] = 1.0f / Jy; inv_J[2] = 1.0f / Jz;
     cJ[0] = (Jy - Jz) * inv_J[0]; cJ[1] = (Jz - Jx) * inv_J[1]; cJ[2] = (Jx - Jy) * inv_J[2];
     kf2 = kf[2]; km2 = km[2]; cv = cvu;
+    kfm2 = 2.0f * kf2 * inv_m;
+    ct[0] = P.lever * kf2 * inv_J[0]; ct[1] = P.lever * kf2 * inv_J[1]; ct[2] = km2 * inv_J[2];
+    const float z = P.h * cv;
+    rc2 = 1.0f - 0.5f * z;
+    rc3 = 1.0f - 0.5f * z * rc2;
+    rc4 = 1.0f - z * rc3;
+    rho4 = 1.0f - z * (1.0f - z * (0.5f - z * (1.0f / 6.0f - z * (1.0f / 24.0f))));
+    rho1 = 1.0f - z;
     J[0] = Jx; J[1] = Jy; J[2] = Jz;
     kf0 = kf[0]; kf1 = kf[1]; km0 = km[0]; km1 = km[1]; cv_dn = cvd; cd_up = cdu; cd_dn = cdd;
   }
@@ -177,10 +187,10 @@ template <int OPT> struct Plant<MODEL_FP, OPT> {
     if (randp) {
       float kf[3] = { wp[4 * M + w], wp[5 * M + w], wp[6 * M + w] };
       float km[3] = { wp[7 * M + w], wp[8 * M + w], wp[9 * M + w] };
-      set(wp[w], wp[M + w], wp[2 * M + w], wp[3 * M + w], kf, km, wp[10 * M + w], wp[11 * M + w], wp[12 * M + w],
+      set(P, wp[w], wp[M + w], wp[2 * M + w], wp[3 * M + w], kf, km, wp[10 * M + w], wp[11 * M + w], wp[12 * M + w],
           wp[13 * M + w]);
     } else {
-      set(P.mass, P.J[0], P.J[1], P.J[2], P.kf, P.km, P.cv_up, P.cv_dn, P.cd_up, P.cd_dn);
+      set(P, P.mass, P.J[0], P.J[1], P.J[2], P.kf, P.km, P.cv_up, P.cv_dn, P.cd_up, P.cd_dn);
     }
   }
 };
@@ -338,11 +348,103 @@ __device__ __forceinline__ void deriv(const DevParams &P, const Plant<MODEL, OPT
   else deriv_ab<OPT>(P, pl, x, u, fdist, dx);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Lean first-principles step (no OPT_EXTRAS): Eqs. (1)-(4) + Eq. (6) with c_v^ = c_v_, c_d = 0 + pure-quadratic thrust
+// and torque curves, the same C4 scheme as the generic integrator below, restated with fewer instructions:
+//  * the rotor lag is linear and decoupled, so its RK4 stages and update are exact closed forms in z = h c_v
+//    (SURVEY.md C12): with e = W - W_cmd, stage speeds are W_cmd + e (1, 1 - z/2, 1 - z/2 + z^2/4, 1 - z + z^2/2 - z^3/4)
+//    and W+ = W_cmd + e (1 - z + z^2/2 - z^3/6 + z^4/24)   [Euler: W+ = W_cmd + e (1 - z)];
+//  * dv does not depend on v or p, so p+ = p + h v + h^2/6 (a1 + a2 + a3) and no stage velocities are formed;
+//  * rates carry their constant factors: a uses 2 k_f/m, dw uses l k_f/J, dq is 2 q-dot (stepped with h/2).
+struct FpRates { float a[3], dw[3], dq[4]; };
+
+template <int OPT>
+__device__ __forceinline__ void fp_lean_rates(const Plant<MODEL_FP, OPT> &pl, const float *q, const float *w,
+                                              const float *Om, const float *fa, FpRates &r) {
+  float w2[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) w2[k] = Om[k] * Om[k];
+  float A = w2[0] + w2[1], B = w2[2] + w2[3], C = w2[1] + w2[2], Dd = w2[0] + w2[3];
+  float E = w2[1] + w2[3], G = w2[0] + w2[2];
+  float acc2 = pl.kfm2 * (A + B);                             // 2 F / m
+  float zx = fmaf(q[0], q[2], q[3] * q[1]);                   // z_B = (2 zx, 2 zy, 1 - 2 zh)
+  float zy = fmaf(q[1], q[2], -(q[3] * q[0]));
+  float zh = fmaf(q[0], q[0], q[1] * q[1]);
+  r.a[0] = fmaf(zx, acc2, fa[0]);
+  r.a[1] = fmaf(zy, acc2, fa[1]);
+  r.a[2] = fmaf(-zh, acc2, fmaf(0.5f, acc2, fa[2]));          // fa[2] already holds f_z/m - g
+  r.dw[0] = fmaf(pl.cJ[0], w[1] * w[2], pl.ct[0] * (B - A));
+  r.dw[1] = fmaf(pl.cJ[1], w[2] * w[0], pl.ct[1] * (C - Dd));
+  r.dw[2] = fmaf(pl.cJ[2], w[0] * w[1], pl.ct[2] * (E - G));
+  r.dq[0] = fmaf(q[3], w[0], fmaf(q[1], w[2], -(q[2] * w[1])));
+  r.dq[1] = fmaf(q[3], w[1], fmaf(q[2], w[0], -(q[0] * w[2])));
+  r.dq[2] = fmaf(q[3], w[2], fmaf(q[0], w[1], -(q[1] * w[0])));
+  r.dq[3] = -fmaf(q[0], w[0], fmaf(q[1], w[1], q[2] * w[2]));
+}
+
+template <int INTEG, int OPT>
+__device__ __forceinline__ void integrate_fp_lean(const DevParams &P, const Plant<MODEL_FP, OPT> &pl, float *x,
+                                                  const float *rpm_cmd, const float *fdist) {
+  float *p = x, *q = x + 3, *v = x + 7, *w = x + 10, *Om = x + 13;
+  float fa[3] = { 0.0f, 0.0f, -P.g };
+  if (OPT & OPT_DIST) { fa[0] = fdist[0] * pl.inv_m; fa[1] = fdist[1] * pl.inv_m; fa[2] = fmaf(fdist[2], pl.inv_m, -P.g); }
+  float e[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) e[k] = Om[k] - rpm_cmd[k];
+  const float hq = 0.5f * P.h;                                // dq is twice the quaternion rate
+  FpRates r1;
+  fp_lean_rates<OPT>(pl, q, w, Om, fa, r1);
+  if constexpr (INTEG == INTEG_EULER) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { p[j] = fmaf(P.h, v[j], p[j]); v[j] = fmaf(P.h, r1.a[j], v[j]); w[j] = fmaf(P.h, r1.dw[j], w[j]); }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { q[j] = fmaf(hq, r1.dq[j], q[j]); Om[j] = fmaf(e[j], pl.rho1, rpm_cmd[j]); }
+  } else {
+    float qs[4], ws[3], Os[4];
+    FpRates r2, r3, r4;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qs[j] = fmaf(0.5f * hq, r1.dq[j], q[j]); Os[j] = fmaf(e[j], pl.rc2, rpm_cmd[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) ws[j] = fmaf(P.half_h, r1.dw[j], w[j]);
+    fp_lean_rates<OPT>(pl, qs, ws, Os, fa, r2);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qs[j] = fmaf(0.5f * hq, r2.dq[j], q[j]); Os[j] = fmaf(e[j], pl.rc3, rpm_cmd[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) ws[j] = fmaf(P.half_h, r2.dw[j], w[j]);
+    fp_lean_rates<OPT>(pl, qs, ws, Os, fa, r3);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qs[j] = fmaf(hq, r3.dq[j], q[j]); Os[j] = fmaf(e[j], pl.rc4, rpm_cmd[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) ws[j] = fmaf(P.h, r3.dw[j], w[j]);
+    fp_lean_rates<OPT>(pl, qs, ws, Os, fa, r4);
+    const float h2_6 = P.h * P.h_sixth, hq6 = 0.5f * P.h_sixth;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      float a12 = r1.a[j] + r2.a[j];
+      p[j] = fmaf(P.h, v[j], fmaf(h2_6, a12 + r3.a[j], p[j]));
+      v[j] = fmaf(P.h_sixth, fmaf(2.0f, r3.a[j], a12 + r2.a[j]) + r4.a[j], v[j]);
+      w[j] = fmaf(P.h_sixth, fmaf(2.0f, r3.dw[j], fmaf(2.0f, r2.dw[j], r1.dw[j])) + r4.dw[j], w[j]);
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      q[j] = fmaf(hq6, fmaf(2.0f, r3.dq[j], fmaf(2.0f, r2.dq[j], r1.dq[j])) + r4.dq[j], q[j]);
+      Om[j] = fmaf(e[j], pl.rho4, rpm_cmd[j]);
+    }
+  }
+  float inv = rsqrtf(fmaf(q[0], q[0], fmaf(q[1], q[1], fmaf(q[2], q[2], q[3] * q[3]))));
+#pragma unroll
+  for (int j = 0; j < 4; ++j) q[j] *= inv;
+}
+
 // C4: explicit Euler / classical RK4, inputs held; q renormalised once per step, not inside the stages (R8-R10).
 template <int MODEL, int INTEG, int OPT>
 __device__ __forceinline__ void integrate(const DevParams &P, const Plant<MODEL, OPT> &pl, float *x, const float *u,
                                           const float *fdist) {
   constexpr int D = MODEL == MODEL_FP ? 17 : 13;
+  if constexpr (MODEL == MODEL_FP && !(OPT & OPT_EXTRAS)) {
+    integrate_fp_lean<INTEG, OPT>(P, pl, x, u, fdist);
+    return;
+  }
   float k[D];
   if constexpr (INTEG == INTEG_EULER) {
     deriv<MODEL, OPT>(P, pl, x, u, fdist, k);

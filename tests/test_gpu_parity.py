@@ -304,3 +304,79 @@ def test_general_kernel_fidelity_switches(cf, cfo, W):
         for k in range(5):
             assert_state_close(rg[k], ro[k], model, 3e-4, f"model {model} iface {prm.get('iface')} integ {prm['integrator']} rec {k}")
         assert np.array_equal(g.counters(), o.counters())
+
+
+# ------------------------------------------------------------------------------------------------ full BASELINE sizes
+def _oracle_slice(cfo, wl, w0, m):
+    """The oracle on worlds [w0, w0+m) of the full workload (Philox is keyed by the global world index)."""
+    sim = cfo.OracleSim(m, wl.N, wl.model, dict(wl.params, world_offset=w0))
+    sim.reset(wl.seed)
+    if wl.broadcast_state is not None:
+        sim.set_state(wl.broadcast_state, broadcast=True)
+    cm = wl.cmds if wl.cmds.ndim == 2 else wl.cmds[:, w0 * wl.N:(w0 + m) * wl.N]
+    rec = sim.step(cm, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every)
+    return sim, rec
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5", "cfg5e"])
+def test_full_size_sampled_worlds_match_oracle(cf, cfo, W, name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (same Sim, same fused cf_step call, same
+    record buffer); sampled worlds are recomputed one slice at a time by the oracle.  Free-running over the full
+    horizon, so the bound is the drift budget (1e-3 m on position; 2e-3 relative to the floors on the rest) -- the
+    per-step bar is tested teacher-forced above."""
+    import torch
+    wl = W.make(name)
+    g = fresh_gpu(cf, wl)
+    rg = g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every)
+    xg = g.get_state().cpu().numpy()
+    assert np.isfinite(xg).all()
+    md = g.min_dist().cpu().numpy() if wl.params.get("n_obstacles") else None
+    m = {"cfg4": 1}.get(name, 16)
+    samples = [0, wl.M // 3, wl.M - m]
+    rec_slots = None if rg is None else sorted({0, rg.shape[0] // 2, rg.shape[0] - 1})
+    for w0 in samples:
+        o, ro = _oracle_slice(cfo, wl, w0, m)
+        sl = slice(w0 * wl.N, (w0 + m) * wl.N)
+        xo = o.get_state()
+        assert np.abs(xg[0:3, sl] - xo[0:3]).max() <= 1e-3, (name, w0)
+        assert_state_close(xg[:, sl], xo, wl.model, 2e-3, f"{name} world {w0} final")
+        if ro is not None:
+            for k in rec_slots:
+                rk = rg[k, :, sl].cpu().numpy()
+                assert np.abs(rk[0:3] - ro[k, 0:3]).max() <= 1e-3
+                assert_state_close(rk, ro[k], wl.model, 2e-3, f"{name} world {w0} record {k}")
+        if md is not None:
+            np.testing.assert_allclose(md[w0:w0 + m], o.min_dist(), rtol=0, atol=1e-3)
+    want_att = wl.n_steps // 2 if wl.model == 0 else 0
+    want_pos = wl.n_steps // 5 if wl.params.get("iface") == 3 else 0
+    assert list(g.counters()) == [wl.n_steps, want_att, want_pos, wl.n_records()]
+    del rg, g
+    torch.cuda.empty_cache()
+
+
+def test_cuda_graph_single_step_replay(cf, cfo, W):
+    """Interactive mode: ONE captured single-step launch replayed 200 times advances the device-side step counter,
+    controller phases and record slots exactly like 200 cf_step(1) calls."""
+    import torch
+    wl = W.cfg1(seed=5, M=64, n_steps=200)
+    a = fresh_gpu(cf, wl)
+    a.step(wl.cmds, 200, cmd_hold=200)
+    b = fresh_gpu(cf, wl)
+    cm = torch.from_numpy(wl.cmds).cuda()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        b.bind_stream(side)
+        b.step(cm, 1, cmd_hold=1)                      # warm-up launch on the capture stream (s = 1)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            b.step(cm, 1, cmd_hold=1)                  # captured, not executed
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(199):
+        graph.replay()
+    torch.cuda.synchronize()
+    b.bind_stream()
+    b.sync_counters()
+    assert b.step_counter == 200
+    assert list(b.counters()) == list(a.counters()) == [200, 100, 0, 0]
+    np.testing.assert_allclose(b.get_state().cpu().numpy(), a.get_state().cpu().numpy(), rtol=1e-6, atol=1e-7)
