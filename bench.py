@@ -204,6 +204,49 @@ def time_host_steps(fn, torch, steps, warmup):
     return ts
 
 
+def interactive_mode(device):
+    """configs[0] in single-step-per-launch mode (north_star "interactive stepping"): 1000 launches of n_steps = 1,
+    plain and as replays of one captured CUDA graph.  Returns microseconds per step (host wall clock around a
+    synchronised batch: launch latency is the quantity of interest here)."""
+    import torch
+    from paper_2606_01478_b200 import cf, workloads as W
+    wl = W.cfg1()
+    out = {}
+    sim = cf.Sim(wl.M, wl.N, wl.model, wl.params, device=device)
+    sim.reset(wl.seed)
+    cm = torch.from_numpy(wl.cmds).to(device)
+    rec = torch.empty((1, wl.D, wl.MN), dtype=torch.float32, device=device)
+    for _ in range(50):
+        sim.step(cm, 1, record_every=1, record=rec)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(1000):
+        sim.step(cm, 1, record_every=1, record=rec)
+    torch.cuda.synchronize()
+    out["launch_us_per_step"] = (time.perf_counter() - t0) * 1e3
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        sim.bind_stream(side)
+        sim.step(cm, 1, record_every=1, record=rec)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            for _ in range(10):
+                sim.step(cm, 1, record_every=1, record=rec)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(5):
+        graph.replay()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(100):
+        graph.replay()
+    torch.cuda.synchronize()
+    out["graph_us_per_step"] = (time.perf_counter() - t0) * 1e3
+    out["note"] = "1000 single-step launches; graph = 10 captured launches per replay x 100 replays"
+    sim.bind_stream()
+    return out
+
+
 def oracle_sample(name, target_seconds=12.0, threads=None):
     """Time the float64 oracle, as it stands, on the host cores, on a bounded sample of the same workload: the same
     recipe at a reduced number of worlds / steps (per-drone work is independent of M)."""
@@ -336,6 +379,8 @@ def main():
             r = measure(nm, 5, 3, False)
             others[nm] = dict(value=r["value"], ms_per_step=r["ms_per_step"], roofline=r["roofline"], M=r["M"], N=r["N"],
                               sub_steps=r["sub_steps"], record_every=r["record_every"])
+    if "cfg1" in others:
+        others["cfg1"]["interactive"] = interactive_mode(device)
     cpu = None
     if rank == 0 and world == 1 and not args.no_others:
         rate, cores, sample, _ = oracle_sample(name)
