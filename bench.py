@@ -32,6 +32,9 @@ DEFAULT_WORKLOAD = "cfg3"
 ALGO_FLOPS = {"cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
 BOUND = {"cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
 SM_COUNT, FP32_LANES = 148, 128
+# dram__bytes_read.sum + dram__bytes_write.sum of the rollout kernel, one launch, from the `ncu --set full` captures
+# summarised in profiles/r1_<workload>_rollout.md (static: ncu never runs inside bench.py)
+TRAFFIC_NCU = {"cfg2": 5.9e6, "cfg3": 201.0e6, "cfg4": 2.725e9, "cfg5": 4.415e9, "cfg5e": 4.415e9}
 
 
 def peaks():
@@ -284,7 +287,7 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -353,6 +356,7 @@ def main():
             ach = ALGO_FLOPS[nm] * wl.drone_steps / (k_ms * 1e-3) / 1e12
             roof = dict(bound="alu", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
                         traffic=None, peak_source=f"148 SM x 128 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz")
+        roof["traffic"] = TRAFFIC_NCU.get(nm)
         roof.update(kernel=R.kernel, kernel_ms=k_ms, grid=R.grid, block=R.block,
                     hbm_gbs_algorithmic=algo_bytes_per_launch(wl) / (k_ms * 1e-3) / 1e9,
                     algo_flops_per_drone_step=ALGO_FLOPS[nm], algo_bytes_per_launch=algo_bytes_per_launch(wl))
