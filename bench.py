@@ -135,7 +135,8 @@ class Runner:
         self.record = torch.empty((n_rec, wl.D, wl.MN), dtype=torch.float32, device=device) if n_rec else None
         self.obst = bool(wl.params.get("n_obstacles"))
         self.min_dist = torch.empty(wl.M, dtype=torch.float32, device=device) if self.obst else None
-        self.launches_per_step = 1 + (self.bstate is not None) + self.obst
+        # broadcast resets are folded into the rollout launch and the N = 1 minimum distance comes from its epilogue
+        self.launches_per_step = 1 + (1 if (self.obst and wl.N > 1) else 0)
         self.kernel, self.grid, self.block = self.sim.describe_launch()
         # host side buffers for the end-to-end path (pinned)
         self.e2e_ok = e2e and self.cmds_host is not None

@@ -19,6 +19,9 @@ struct cf_sim {
   int opt;                    // option bits this configuration needs
   // workspace carving (device pointers into the caller's buffer)
   float *state, *ctrl, *wparam, *min_d2;
+  float *bcast_buf;           // [D] pending broadcast state (cf_set_state(broadcast) is folded into the next cf_step)
+  float *md_drone;            // [MN] per-drone minimum distance written by the rollout kernel's epilogue
+  bool pending_bcast, md_valid;
   Counters *counters;
   uint32_t *rec_table;
   cudaStream_t stream;
@@ -74,7 +77,7 @@ extern "C" void cf_default_params(cf_params *p, int model) {
 
 static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
-struct Carve { size_t state, ctrl, wparam, min_d2, counters, rec_table, total; };
+struct Carve { size_t state, ctrl, wparam, min_d2, md_drone, bcast, counters, rec_table, total; };
 static Carve carve(long long M, long long N, int model, const cf_params *p) {
   Carve c;
   size_t MN = (size_t)(M * N), off = 0;
@@ -82,6 +85,8 @@ static Carve carve(long long M, long long N, int model, const cf_params *p) {
   c.ctrl = off;      off += align256(sizeof(float) * kCtrlPlanes * MN);
   c.wparam = off;    off += align256(sizeof(float) * cf_world_param_dim(model) * (size_t)M);
   c.min_d2 = off;    off += p->n_obstacles > 0 ? align256(sizeof(float) * kMaxObst * MN) : 0;
+  c.md_drone = off;  off += p->n_obstacles > 0 ? align256(sizeof(float) * MN) : 0;
+  c.bcast = off;     off += 256;
   c.counters = off;  off += align256(sizeof(Counters));
   c.rec_table = off; off += align256(sizeof(uint32_t) * kRecTableCap);
   c.total = off;
@@ -162,6 +167,8 @@ static void fill_dev_params(cf_sim *s) {
   d.rpm_min = p.rpm_min; d.rpm_max = p.rpm_max; d.thrust_min = p.thrust_min; d.thrust_max = p.thrust_max;
   d.tilt_max = p.tilt_max; d.iR_max = p.iR_max; d.dist_sigma = p.dist_sigma; d.n_obst = p.n_obstacles;
   d.use_noise = p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE;
+  d.hover_thrust = (float)((double)p.mass * p.g);
+  d.hover_rpm = s->model == CF_MODEL_FIRST_PRINCIPLES ? (float)hover_rpm_nominal(&p) : 0.f;
   for (int j = 0; j < kMaxObst; ++j) {
     for (int k = 0; k < 4; ++k) d.obst[j][k] = p.obstacles[j][k];
     if (j < p.n_obstacles) {
@@ -366,6 +373,9 @@ extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf
   char *base = (char *)workspace_dev;
   s->state = (float *)(base + c.state); s->ctrl = (float *)(base + c.ctrl); s->wparam = (float *)(base + c.wparam);
   s->min_d2 = p->n_obstacles > 0 ? (float *)(base + c.min_d2) : nullptr;
+  s->md_drone = p->n_obstacles > 0 ? (float *)(base + c.md_drone) : nullptr;
+  s->bcast_buf = (float *)(base + c.bcast);
+  s->pending_bcast = false; s->md_valid = false;
   s->counters = (Counters *)(base + c.counters); s->rec_table = (uint32_t *)(base + c.rec_table);
   s->stream = 0; s->seed = 0; s->s_host = 0; s->n_rec_host = 0; s->have_state = false;
   s->hover_rpm = (float)hover_rpm_nominal(p);
@@ -423,23 +433,45 @@ extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
   CF_CUDA(cudaMemsetAsync(sim->rec_table, 0, sizeof(uint32_t) * kRecTableCap, sim->stream));
   CF_CUDA(cudaGetLastError());
   sim->seed = seed; sim->s_host = 0; sim->n_rec_host = 0; sim->have_state = true;
+  sim->pending_bcast = false; sim->md_valid = false;
   return CF_OK;
 }
 
-extern "C" int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast) {
-  if (!sim || !state_dev) return fail(CF_E_ARG, "NULL argument");
-  if (!sim->have_state) return fail(CF_E_STATE, "cf_set_state needs a prior cf_reset (world parameters)");
+static int launch_set_state(cf_sim *sim, const float *src, int broadcast) {
   float hover_thrust = (float)((double)sim->p.mass * sim->p.g);
   set_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(
-      sim->state, sim->ctrl, sim->min_d2, state_dev, broadcast, sim->D, sim->MN,
+      sim->state, sim->ctrl, sim->min_d2, src, broadcast, sim->D, sim->MN,
       sim->model == CF_MODEL_FIRST_PRINCIPLES ? sim->hover_rpm : 0.f, hover_thrust);
   CF_CUDA(cudaGetLastError());
   return CF_OK;
 }
 
+// A broadcast cf_set_state is lazy: the D floats are parked in the workspace and the next cf_step starts every drone
+// from them in registers (no 35-plane write + re-read).  Anything else that touches the planes materialises it first.
+static int materialise(cf_sim *sim) {
+  if (!sim->pending_bcast) return CF_OK;
+  sim->pending_bcast = false;
+  return launch_set_state(sim, sim->bcast_buf, 1);
+}
+
+extern "C" int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast) {
+  if (!sim || !state_dev) return fail(CF_E_ARG, "NULL argument");
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_set_state needs a prior cf_reset (world parameters)");
+  sim->md_valid = false;
+  if (broadcast) {
+    CF_CUDA(cudaMemcpyAsync(sim->bcast_buf, state_dev, sizeof(float) * sim->D, cudaMemcpyDeviceToDevice, sim->stream));
+    sim->pending_bcast = true;
+    return CF_OK;
+  }
+  sim->pending_bcast = false;
+  return launch_set_state(sim, state_dev, 0);
+}
+
 extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctrl_dev, const float *wparam_dev,
                            const float *min_d2_dev, int64_t step_counter) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
+  sim->md_valid = false;
   const size_t MN = (size_t)sim->MN;
   if (state_dev) CF_CUDA(cudaMemcpyAsync(sim->state, state_dev, sizeof(float) * sim->D * MN, cudaMemcpyDeviceToDevice, sim->stream));
   if (ctrl_dev) CF_CUDA(cudaMemcpyAsync(sim->ctrl, ctrl_dev, sizeof(float) * kCtrlPlanes * MN, cudaMemcpyDeviceToDevice, sim->stream));
@@ -512,6 +544,7 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   }
   StepArgs A;
   A.state = sim->state; A.ctrl = sim->ctrl; A.wparam = sim->wparam; A.min_d2 = sim->min_d2;
+  A.bcast = sim->pending_bcast ? sim->bcast_buf : nullptr; A.md_drone = sim->md_drone;
   A.counters = sim->counters; A.rec_table = sim->rec_table;
   A.cmds = (const float4 *)cmds_dev; A.record = record_dev;
   A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.world_offset = sim->p.world_offset;
@@ -527,6 +560,8 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   CF_CUDA(cudaGetLastError());
   sim->s_host = s0 + n_steps;
   sim->n_rec_host += n_rec;
+  sim->pending_bcast = false;
+  sim->md_valid = sim->min_d2 != nullptr;
   return CF_OK;
 }
 
@@ -568,11 +603,13 @@ extern "C" int cf_step_host(cf_sim *sim, const void *cmds_host, int n_cmds, int 
 
 extern "C" int cf_get_state(cf_sim *sim, float *out_dev) {
   if (!sim || !out_dev) return fail(CF_E_ARG, "NULL argument");
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
   CF_CUDA(cudaMemcpyAsync(out_dev, sim->state, sizeof(float) * sim->D * (size_t)sim->MN, cudaMemcpyDeviceToDevice, sim->stream));
   return CF_OK;
 }
 extern "C" int cf_get_state_host(cf_sim *sim, float *out_host) {
   if (!sim || !out_host) return fail(CF_E_ARG, "NULL argument");
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
   CF_CUDA(cudaMemcpyAsync(out_host, sim->state, sizeof(float) * sim->D * (size_t)sim->MN, cudaMemcpyDeviceToHost, sim->stream));
   CF_CUDA(cudaStreamSynchronize(sim->stream));
   return CF_OK;
@@ -580,6 +617,7 @@ extern "C" int cf_get_state_host(cf_sim *sim, float *out_host) {
 
 static int aux_source(cf_sim *sim, int which, const void **src, size_t *bytes) {
   const size_t MN = (size_t)sim->MN;
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
   switch (which) {
     case CF_AUX_COUNTERS: *src = sim->counters; *bytes = 4 * sizeof(uint32_t); return CF_OK;
     case CF_AUX_CTRL: *src = sim->ctrl; *bytes = sizeof(float) * kCtrlPlanes * MN; return CF_OK;
@@ -594,6 +632,11 @@ static int aux_source(cf_sim *sim, int which, const void **src, size_t *bytes) {
 
 static int launch_min_dist(cf_sim *sim, float *out_dev) {
   if (!sim->min_d2) return fail(CF_E_ARG, "no obstacles configured");
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
+  if (sim->md_valid && sim->N == 1) {   // the rollout kernel's epilogue already reduced obstacles and steps per drone
+    CF_CUDA(cudaMemcpyAsync(out_dev, sim->md_drone, sizeof(float) * (size_t)sim->M, cudaMemcpyDeviceToDevice, sim->stream));
+    return CF_OK;
+  }
   if (sim->N < 8) {
     min_dist_small_n_kernel<<<grid_for(sim->M, 256), 256, 0, sim->stream>>>(sim->min_d2, out_dev, sim->M, sim->N, sim->MN, sim->dp);
   } else {

@@ -52,6 +52,7 @@ struct DevParams {
   float4 obst_q[kMaxObst];        // (-2cx, -2cy, -2cz, c.c): d^2 = |p|^2 + q.(p,1); unused slots (0,0,0,+inf)
   float noise_sigma[4], cmd_lo[4], cmd_hi[4];
   int   att_div, pos_div;
+  float hover_thrust, hover_rpm;   // reading R20: held commands after a reset / set_state
 };
 
 struct StepArgs {
@@ -59,6 +60,8 @@ struct StepArgs {
   float *ctrl;             // [14][MN]
   const float *wparam;     // [P][M]
   float *min_d2;           // [8][MN] or nullptr
+  const float *bcast;      // [D] or nullptr: start every drone from this state with re-armed controllers (lazy cf_set_state)
+  float *md_drone;         // [MN] or nullptr: per-drone min over obstacles and steps of |p - c_j| - r_j (epilogue)
   Counters *counters;
   uint32_t *rec_table;     // [kRecTableCap]
   const float4 *cmds;      // [K][MN] or [K]
@@ -607,31 +610,43 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   uint32_t my_att = 0, my_pos = 0;
   if (active) {
     float x[D];
-#pragma unroll
-    for (int j = 0; j < D; ++j) x[j] = A.state[j * MN + i];
     float iR[3] = { 0, 0, 0 }, ip[3] = { 0, 0, 0 }, att_cmd[4] = { 0, 0, 0, 0 }, rpm_cmd[4] = { 0, 0, 0, 0 };
     float target[4] = { 0, 0, 0, 0 };
-    if (HAS_ATT) {
-#pragma unroll
-      for (int j = 0; j < 3; ++j) iR[j] = A.ctrl[j * MN + i];
-    }
-    if (HAS_POS) {
-#pragma unroll
-      for (int j = 0; j < 3; ++j) ip[j] = A.ctrl[(3 + j) * MN + i];
-    }
-    if (HAS_ATT || HAS_POS || !FP) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) att_cmd[j] = A.ctrl[(6 + j) * MN + i];
-    }
-    if (FP) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) rpm_cmd[j] = A.ctrl[(10 + j) * MN + i];
-    }
     float md2[kMaxObst];
     const bool obst = (OPT & OPT_OBST) != 0 && A.min_d2 != nullptr;
-    if (obst) {
+    if (A.bcast != nullptr) {
+      // lazy cf_set_state(broadcast): every drone starts from the same state (uniform loads), controller integrals 0,
+      // held commands = hover, obstacle minima re-armed -- nothing is read from the planes
 #pragma unroll
-      for (int j = 0; j < kMaxObst; ++j) md2[j] = A.min_d2[j * MN + i];
+      for (int j = 0; j < D; ++j) x[j] = A.bcast[j];
+      att_cmd[3] = P.hover_thrust;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) rpm_cmd[j] = P.hover_rpm;
+#pragma unroll
+      for (int j = 0; j < kMaxObst; ++j) md2[j] = __int_as_float(0x7f800000);
+    } else {
+#pragma unroll
+      for (int j = 0; j < D; ++j) x[j] = A.state[j * MN + i];
+      if (HAS_ATT) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) iR[j] = A.ctrl[j * MN + i];
+      }
+      if (HAS_POS) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) ip[j] = A.ctrl[(3 + j) * MN + i];
+      }
+      if (HAS_ATT || HAS_POS || !FP) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) att_cmd[j] = A.ctrl[(6 + j) * MN + i];
+      }
+      if (FP) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) rpm_cmd[j] = A.ctrl[(10 + j) * MN + i];
+      }
+      if (obst) {
+#pragma unroll
+        for (int j = 0; j < kMaxObst; ++j) md2[j] = A.min_d2[j * MN + i];
+      }
     }
     float Rd[3][3];
     if (HAS_ATT) euler_to_R(att_cmd[0], att_cmd[1], att_cmd[2], Rd);
@@ -790,6 +805,13 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     if (obst) {
 #pragma unroll
       for (int j = 0; j < kMaxObst; ++j) A.min_d2[j * MN + i] = md2[j];
+      if (A.md_drone != nullptr) {       // C10 read-out fused into the epilogue: min_j sqrt(min_t d2_j) - r_j
+        float best = __int_as_float(0x7f800000);
+#pragma unroll
+        for (int j = 0; j < kMaxObst; ++j)
+          if (j < P.n_obst) best = fminf(best, sqrtf(md2[j]) - P.obst[j][3]);
+        A.md_drone[i] = best;
+      }
     }
     if (i == 0) {
       if (my_att) atomicAdd(&A.counters->att_ticks, my_att);

@@ -380,3 +380,32 @@ def test_cuda_graph_single_step_replay(cf, cfo, W):
     assert b.step_counter == 200
     assert list(b.counters()) == list(a.counters()) == [200, 100, 0, 0]
     np.testing.assert_allclose(b.get_state().cpu().numpy(), a.get_state().cpu().numpy(), rtol=1e-6, atol=1e-7)
+
+
+def test_lazy_broadcast_reset_and_fused_min_distance(cf, cfo, W):
+    """cf_set_state(broadcast) is folded into the next cf_step and the N = 1 minimum distance comes from the rollout
+    epilogue; both must be indistinguishable from the eager path and from the oracle."""
+    wl = W.cfg3(seed=11, M=777, n_steps=25)
+    a = fresh_gpu(cf, wl)                        # reset + set_state(broadcast): pending
+    xa = a.get_state().cpu().numpy()             # materialises the pending broadcast
+    assert np.array_equal(xa, np.tile(wl.broadcast_state.astype(np.float32)[:, None], (1, 777)))
+    assert np.all(np.isinf(a.min_d2().cpu().numpy())) and np.all(a.ctrl().cpu().numpy()[:9] == 0)
+    a.step(wl.cmds, 25)                          # eager: planes were written, kernel reads them
+    b = fresh_gpu(cf, wl)
+    b.step(wl.cmds, 25)                          # lazy: kernel starts from the broadcast vector
+    assert np.array_equal(a.get_state().cpu().numpy(), b.get_state().cpu().numpy())
+    assert np.array_equal(a.min_d2().cpu().numpy(), b.min_d2().cpu().numpy())
+    o = fresh_oracle(cfo, wl)
+    o.step(wl.cmds, 25)
+    fused = b.min_dist().cpu().numpy()           # epilogue plane
+    np.testing.assert_allclose(fused, o.min_dist(), rtol=0, atol=1e-4)
+    b.set_full(min_d2=b.min_d2())                # invalidates the epilogue plane -> read-out kernel path
+    np.testing.assert_allclose(b.min_dist().cpu().numpy(), fused, rtol=1e-6, atol=1e-7)
+    # a second planning iteration: broadcast again, fresh noise (global step counter moved on)
+    b.set_state(wl.broadcast_state.astype(np.float32), broadcast=True)
+    o.set_state(wl.broadcast_state, broadcast=True)
+    b.step(wl.cmds, 25)
+    o.step(wl.cmds, 25)
+    assert_state_close(b.get_state().cpu().numpy(), o.get_state(), wl.model, 2e-4, "second iteration")
+    np.testing.assert_allclose(b.min_dist().cpu().numpy(), o.min_dist(), rtol=0, atol=1e-4)
+    assert list(b.counters()) == list(o.counters())
