@@ -27,6 +27,8 @@ struct cfo_sim {
   double *ctrl;   /* [14][MN] */
   double *wp;     /* [P][M]   */
   double *mind2;  /* [8][MN]  */
+  double *eps;    /* [4][MN] AR(1) command-noise state, NaN = none drawn since the last re-arm (R25) */
+  double *cost;   /* [MN] running rollout cost (R27) */
   uint32_t s, att_ticks, pos_ticks, n_rec_total;
   uint32_t rec_table[CFO_REC_TABLE_CAP];
   uint64_t seed;
@@ -78,6 +80,7 @@ void cfo_default_params(cfo_params *p, int model) {
   p->grid_dims[0] = p->grid_dims[1] = p->grid_dims[2] = 1;
   p->cmd_lo[0] = -0.5; p->cmd_lo[1] = -0.5; p->cmd_lo[2] = -PI; p->cmd_lo[3] = 0.05;
   p->cmd_hi[0] = 0.5;  p->cmd_hi[1] = 0.5;  p->cmd_hi[2] = PI;  p->cmd_hi[3] = 0.55;
+  p->n_ctrl = 1;
 }
 
 static double clipd(double v, double lo, double hi) { return v < lo ? lo : (v > hi ? hi : v); }
@@ -354,6 +357,7 @@ int cfo_create(cfo_sim **out, int64_t M, int64_t N, int model, const cfo_params 
   if (p->f_phys <= 0 || ad < 1 || pd < 1 || ad != floor(ad) || pd != floor(pd)) return -1;
   if (model == CFO_MODEL_ABSTRACTED && p->iface != CFO_IF_ATTITUDE && p->iface != CFO_IF_POSITION) return -6;
   if (p->n_obstacles < 0 || p->n_obstacles > 8) return -1;
+  if (!(p->noise_beta >= 0.0 && p->noise_beta < 1.0) || p->n_ctrl < 1 || p->worlds_per_ctrl < 0) return -1;
   cfo_sim *S = (cfo_sim *)calloc(1, sizeof(cfo_sim));
   S->M = M; S->N = N; S->MN = M * N; S->model = model; S->p = *p;
   S->D = cfo_state_dim(model); S->P = cfo_world_param_dim(model);
@@ -361,12 +365,14 @@ int cfo_create(cfo_sim **out, int64_t M, int64_t N, int model, const cfo_params 
   S->ctrl = (double *)calloc((size_t)14 * S->MN, sizeof(double));
   S->wp = (double *)calloc((size_t)S->P * M, sizeof(double));
   S->mind2 = (double *)calloc((size_t)8 * S->MN, sizeof(double));
+  S->eps = (double *)calloc((size_t)4 * S->MN, sizeof(double));
+  S->cost = (double *)calloc((size_t)S->MN, sizeof(double));
   *out = S;
   return 0;
 }
 void cfo_destroy(cfo_sim *S) {
   if (!S) return;
-  free(S->x); free(S->ctrl); free(S->wp); free(S->mind2); free(S);
+  free(S->x); free(S->ctrl); free(S->wp); free(S->mind2); free(S->eps); free(S->cost); free(S);
 }
 
 static void rearm_controllers(cfo_sim *S) {
@@ -379,6 +385,8 @@ static void rearm_controllers(cfo_sim *S) {
     S->ctrl[9 * S->MN + i] = p->mass * p->g;
     for (int k = 0; k < 4; ++k) S->ctrl[(10 + k) * S->MN + i] = wh;
     for (int j = 0; j < 8; ++j) S->mind2[j * S->MN + i] = INFINITY;
+    for (int j = 0; j < 4; ++j) S->eps[j * S->MN + i] = NAN;   /* R25: the next command starts a fresh noise chain */
+    S->cost[i] = 0.0;                                          /* R27 */
   }
 }
 
@@ -485,6 +493,14 @@ int cfo_set_full(cfo_sim *S, const double *state, const double *ctrl, const doub
   return 0;
 }
 
+/* teacher forcing of the planning-rollout state (either pointer may be NULL = keep) */
+int cfo_set_plan_state(cfo_sim *S, const double *eps, const double *cost_run) {
+  if (!S) return -1;
+  if (eps) memcpy(S->eps, eps, sizeof(double) * 4 * S->MN);
+  if (cost_run) memcpy(S->cost, cost_run, sizeof(double) * S->MN);
+  return 0;
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* C8: one cf_step call = n_steps physics steps, per drone, in this order:
  *  (1) command fetch  (2) position tick  (3) attitude tick + mixer  (4) disturbance draw
@@ -495,6 +511,8 @@ int cfo_step(cfo_sim *S, const float *cmds, int n_cmds, int cmd_hold, int n_step
   if (!S->have_state) return -3;
   if ((int64_t)n_cmds * cmd_hold < n_steps) return -2;
   const cfo_params *p = &S->p;
+  if (p->cmd_source == CFO_CMD_NOMINAL_PLUS_NOISE && p->worlds_per_ctrl > 0 &&
+      (p->world_offset + S->M - 1) / p->worlds_per_ctrl >= p->n_ctrl) return -2;
   const int D = S->D;
   const int64_t MN = S->MN, N = S->N;
   const uint32_t s0 = S->s;
@@ -517,6 +535,8 @@ int cfo_step(cfo_sim *S, const float *cmds, int n_cmds, int cmd_hold, int n_step
     for (int j = 0; j < D; ++j) x[j] = S->x[j * MN + i];
     for (int j = 0; j < 14; ++j) c[j] = S->ctrl[j * MN + i];
     for (int j = 0; j < 8; ++j) md2[j] = S->mind2[j * MN + i];
+    double eps[4], cost = S->cost[i];
+    for (int j = 0; j < 4; ++j) eps[j] = S->eps[j * MN + i];
     double *iR = c, *ip = c + 3, *att_cmd = c + 6, *rpm_cmd = c + 10;
     uint32_t s = s0, my_att = 0, my_pos = 0;
     for (int t = 0; t < n_steps; ++t) {
@@ -530,8 +550,16 @@ int cfo_step(cfo_sim *S, const float *cmds, int n_cmds, int cmd_hold, int n_step
           philox_at(S->seed, wg, n, s, STREAM_NOISE, r);
           cfo_normal_pair(r[0], r[1], &z[0], &z[1]);
           cfo_normal_pair(r[2], r[3], &z[2], &z[3]);
+          /* R25: temporally correlated noise, AR(1): eps <- z for the first command after a
+           * re-arm, else eps <- beta eps + sqrt(1 - beta^2) z  (stationary, unit variance; beta = 0: white) */
+          const int fresh = isnan(eps[0]);
+          const double gain = sqrt(1.0 - p->noise_beta * p->noise_beta);
+          for (int j = 0; j < 4; ++j) eps[j] = fresh ? z[j] : p->noise_beta * eps[j] + gain * z[j];
+          /* R26: one nominal sequence per controller, controller = global world / worlds_per_ctrl */
+          const int64_t cidx = p->worlds_per_ctrl > 0 ? wg / p->worlds_per_ctrl : 0;
+          const float *nom = cmds + ((size_t)cidx * (size_t)n_cmds + (size_t)k) * 4;
           for (int j = 0; j < 4; ++j)
-            cmd[j] = clipd((double)cmds[(size_t)k * 4 + j] + p->noise_sigma[j] * z[j], p->cmd_lo[j], p->cmd_hi[j]);
+            cmd[j] = clipd((double)nom[j] + p->noise_sigma[j] * eps[j], p->cmd_lo[j], p->cmd_hi[j]);
         }
         if (p->iface == CFO_IF_ATTITUDE) for (int j = 0; j < 4; ++j) att_cmd[j] = cmd[j];
         if (p->iface == CFO_IF_ROTOR) for (int j = 0; j < 4; ++j) rpm_cmd[j] = clipd(cmd[j], p->rpm_min, p->rpm_max);
@@ -569,6 +597,13 @@ int cfo_step(cfo_sim *S, const float *cmds, int n_cmds, int cmd_hold, int n_step
         double d2 = dx_ * dx_ + dy_ * dy_ + dz_ * dz_;
         if (d2 < md2[j]) md2[j] = d2;
       }
+      /* (7b) running rollout cost on the post-step state (R27): h (w_pos |p - goal|^2 + w_vel |v|^2) */
+      if (p->cost_on) {
+        const double *v = fp ? x + 7 : x + 6;
+        double ex = x[0] - p->cost_goal[0], ey = x[1] - p->cost_goal[1], ez = x[2] - p->cost_goal[2];
+        cost += (1.0 / p->f_phys) * (p->cost_w_pos * (ex * ex + ey * ey + ez * ez) +
+                                     p->cost_w_vel * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
+      }
       /* (8) record */
       if (record_every > 0 && s % (uint32_t)record_every == 0) {
         size_t slot = (size_t)(s / (uint32_t)record_every - s0 / (uint32_t)record_every - 1);
@@ -582,6 +617,8 @@ int cfo_step(cfo_sim *S, const float *cmds, int n_cmds, int cmd_hold, int n_step
     for (int j = 0; j < D; ++j) S->x[j * MN + i] = x[j];
     for (int j = 0; j < 14; ++j) S->ctrl[j * MN + i] = c[j];
     for (int j = 0; j < 8; ++j) S->mind2[j * MN + i] = md2[j];
+    for (int j = 0; j < 4; ++j) S->eps[j * MN + i] = eps[j];
+    S->cost[i] = cost;
     if (i == 0) { att_ticks = my_att; pos_ticks = my_pos; }
   }
   S->s = s0 + (uint32_t)n_steps;
@@ -620,6 +657,25 @@ int cfo_get_aux(cfo_sim *S, int which, void *out) {
     case CFO_AUX_WORLD_PARAMS: memcpy(out, S->wp, sizeof(double) * S->P * S->M); return 0;
     case CFO_AUX_REC_TABLE: memcpy(out, S->rec_table, sizeof(S->rec_table)); return 0;
     case CFO_AUX_MIN_D2: memcpy(out, S->mind2, sizeof(double) * 8 * S->MN); return 0;
+    case CFO_AUX_EPS: memcpy(out, S->eps, sizeof(double) * 4 * S->MN); return 0;
+    case CFO_AUX_COST_RUN: memcpy(out, S->cost, sizeof(double) * S->MN); return 0;
+    case CFO_AUX_COST: {   /* R27: J = J_run + w_term |p - goal|^2 + w_obs max(0, d_safe - d_min)^2 + w_coll [d_min < 0] */
+      double *o = (double *)out;
+      const cfo_params *p = &S->p;
+      for (int64_t i = 0; i < S->MN; ++i) {
+        double ex = S->x[i] - p->cost_goal[0], ey = S->x[S->MN + i] - p->cost_goal[1], ez = S->x[2 * S->MN + i] - p->cost_goal[2];
+        double J = S->cost[i] + p->cost_w_term * (ex * ex + ey * ey + ez * ez);
+        double dmin = INFINITY;   /* C10 for this drone */
+        for (int j = 0; j < p->n_obstacles; ++j) {
+          double d = sqrt(S->mind2[j * S->MN + i]) - p->obstacles[j][3];
+          if (d < dmin) dmin = d;
+        }
+        if (dmin < p->cost_d_safe) J += p->cost_w_obs * (p->cost_d_safe - dmin) * (p->cost_d_safe - dmin);
+        if (dmin < 0.0) J += p->cost_w_coll;
+        o[i] = J;
+      }
+      return 0;
+    }
   }
   return -1;
 }

@@ -17,7 +17,8 @@
  *   wparam [P][M]         P = 14 FP: m Jx Jy Jz kf0 kf1 kf2 km0 km1 km2 cv_up cv_dn cd_up cd_dn
  *                         P = 11 AB: m a[3] b[3] c[3] c_tau
  *   mind2  [8][M*N]       running minimum of squared centre distance per obstacle
- *   cmds   [K][M*N][4]    float32
+ *   eps    [4][M*N]       AR(1) state of the command noise;  cost_run [M*N] running rollout cost
+ *   cmds   [K][M*N][4]    float32 (CMD_BUFFER)  or  [n_ctrl][K][4] nominal sequences (CMD_NOMINAL_PLUS_NOISE)
  *   record [n_rec][D][M*N]
  *
  * Parity pins (tests/test_oracle_pins.py): free fall, hover equilibrium, torque-free precession and
@@ -40,7 +41,10 @@ enum { CFO_EULER = 0, CFO_RK4 = 1 };
 enum { CFO_IF_ROTOR = 0, CFO_IF_TORQUE = 1, CFO_IF_ATTITUDE = 2, CFO_IF_POSITION = 3 };
 enum { CFO_CMD_BUFFER = 0, CFO_CMD_NOMINAL_PLUS_NOISE = 1 };
 enum { CFO_AUX_COUNTERS = 0, CFO_AUX_MIN_DIST = 1, CFO_AUX_CTRL = 2, CFO_AUX_WORLD_PARAMS = 3,
-       CFO_AUX_REC_TABLE = 4, CFO_AUX_MIN_D2 = 5 };
+       CFO_AUX_REC_TABLE = 4, CFO_AUX_MIN_D2 = 5,
+       CFO_AUX_COST = 6,   /* double[MN]: running cost + terminal + obstacle-clearance terms (R27) */
+       CFO_AUX_EPS = 7,    /* double[4][MN]: AR(1) noise state, NaN = no command drawn since the last re-arm (R25) */
+       CFO_AUX_COST_RUN = 8 /* double[MN]: running part only */ };
 #define CFO_REC_TABLE_CAP 4096
 
 typedef struct cfo_params {
@@ -64,6 +68,12 @@ typedef struct cfo_params {
   double grid_spacing, grid_jitter, grid_origin[3];
   double obstacles[8][4];
   double noise_sigma[4], cmd_lo[4], cmd_hi[4];
+  /* planning rollouts for the MPPI / iCEM sampler (readings R25-R27) */
+  double noise_beta;              /* AR(1) coefficient of the temporally correlated command noise, 0 = white */
+  int64_t worlds_per_ctrl;        /* controller of a world = global world index / worlds_per_ctrl (0: one controller) */
+  int32_t n_ctrl;                 /* number of nominal sequences in the command buffer [n_ctrl][n_cmds][4] */
+  int32_t cost_on;                /* accumulate the running rollout cost */
+  double cost_goal[3], cost_w_pos, cost_w_vel, cost_w_term, cost_w_obs, cost_d_safe, cost_w_coll;
 } cfo_params;
 
 typedef struct cfo_sim cfo_sim;
@@ -78,6 +88,7 @@ int  cfo_set_state(cfo_sim *s, const double *state, int broadcast);
 /* teacher forcing: overwrite everything a step depends on (any pointer may be NULL = keep) */
 int  cfo_set_full(cfo_sim *s, const double *state, const double *ctrl, const double *wparam,
                   const double *mind2, int64_t step_counter);
+int  cfo_set_plan_state(cfo_sim *s, const double *eps, const double *cost_run);
 int  cfo_step(cfo_sim *s, const float *cmds, int n_cmds, int cmd_hold, int n_steps, int record_every,
               double *record, size_t record_len /* doubles */);
 int  cfo_get_state(cfo_sim *s, double *out);

@@ -20,7 +20,7 @@ MODEL_FP, MODEL_AB = 0, 1
 EULER, RK4 = 0, 1
 IF_ROTOR, IF_TORQUE, IF_ATTITUDE, IF_POSITION = 0, 1, 2, 3
 CMD_BUFFER, CMD_NOMINAL_PLUS_NOISE = 0, 1
-AUX_COUNTERS, AUX_MIN_DIST, AUX_CTRL, AUX_WORLD_PARAMS, AUX_REC_TABLE, AUX_MIN_D2 = range(6)
+AUX_COUNTERS, AUX_MIN_DIST, AUX_CTRL, AUX_WORLD_PARAMS, AUX_REC_TABLE, AUX_MIN_D2, AUX_COST, AUX_EPS, AUX_COST_RUN = range(9)
 REC_TABLE_CAP = 4096
 
 d = C.c_double
@@ -45,6 +45,9 @@ class Params(C.Structure):
         ("grid_spacing", d), ("grid_jitter", d), ("grid_origin", d * 3),
         ("obstacles", (d * 4) * 8),
         ("noise_sigma", d * 4), ("cmd_lo", d * 4), ("cmd_hi", d * 4),
+        ("noise_beta", d), ("worlds_per_ctrl", C.c_int64), ("n_ctrl", C.c_int32), ("cost_on", C.c_int32),
+        ("cost_goal", d * 3), ("cost_w_pos", d), ("cost_w_vel", d), ("cost_w_term", d), ("cost_w_obs", d),
+        ("cost_d_safe", d), ("cost_w_coll", d),
     ]
 
 
@@ -76,6 +79,7 @@ def lib():
         L.cfo_reset.argtypes = [vp, C.c_uint64]
         L.cfo_set_state.argtypes = [vp, vp, C.c_int]
         L.cfo_set_full.argtypes = [vp, vp, vp, vp, vp, C.c_int64]
+        L.cfo_set_plan_state.argtypes = [vp, vp, vp]
         L.cfo_step.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, C.c_size_t]
         L.cfo_get_state.argtypes = [vp, vp]
         L.cfo_get_aux.argtypes = [vp, C.c_int, vp]
@@ -178,10 +182,10 @@ class OracleSim:
         return (s0 + n_steps) // record_every - s0 // record_every
 
     def step(self, cmds, n_steps: int, cmd_hold: int = 1, record_every: int = 0, check: bool = True):
-        """cmds: float32 [K][M*N][4] (buffer source) or [K][4] (nominal + noise).  Returns record
+        """cmds: float32 [K][M*N][4] (buffer source) or [n_ctrl][K][4] (nominal + noise).  Returns record
         [n_rec][D][M*N] float64 (or None)."""
         cm = np.ascontiguousarray(cmds, dtype=np.float32)
-        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4
+        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4 * self.params.n_ctrl
         assert cm.size % per == 0, (cm.shape, per)
         n_cmds = cm.size // per
         n_rec = self.n_records(n_steps, record_every)
@@ -221,6 +225,27 @@ class OracleSim:
         out = np.empty((8, self.MN), dtype=np.float64)
         assert lib().cfo_get_aux(self._h, AUX_MIN_D2, _ptr(out)) == 0
         return out
+
+    def cost(self):
+        out = np.empty(self.MN, dtype=np.float64)
+        assert lib().cfo_get_aux(self._h, AUX_COST, _ptr(out)) == 0
+        return out
+
+    def cost_run(self):
+        out = np.empty(self.MN, dtype=np.float64)
+        assert lib().cfo_get_aux(self._h, AUX_COST_RUN, _ptr(out)) == 0
+        return out
+
+    def eps(self):
+        out = np.empty((4, self.MN), dtype=np.float64)
+        assert lib().cfo_get_aux(self._h, AUX_EPS, _ptr(out)) == 0
+        return out
+
+    def set_plan_state(self, eps=None, cost_run=None):
+        e, c = _f64(eps), _f64(cost_run)
+        assert e is None or e.size == 4 * self.MN
+        assert c is None or c.size == self.MN
+        assert lib().cfo_set_plan_state(self._h, _ptr(e), _ptr(c)) == 0
 
     def rec_table(self):
         out = np.zeros(REC_TABLE_CAP, dtype=np.uint32)
