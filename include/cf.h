@@ -68,7 +68,11 @@ enum { CF_AUX_COUNTERS = 0,      /* uint32[4]: s, attitude ticks, position ticks
        CF_AUX_CTRL = 2,          /* float[14][MN] */
        CF_AUX_WORLD_PARAMS = 3,  /* float[P][M] */
        CF_AUX_REC_TABLE = 4,     /* uint32[CF_REC_TABLE_CAP]: record slot (since reset) -> step counter */
-       CF_AUX_MIN_D2 = 5 };      /* float[8][MN]: running minimum squared centre distance per obstacle */
+       CF_AUX_MIN_D2 = 5,        /* float[8][MN]: running minimum squared centre distance per obstacle */
+       CF_AUX_COST = 6,          /* float[MN]: rollout cost J (R27): running + terminal + clearance + collision */
+       CF_AUX_EPS = 7,           /* float[4][MN]: AR(1) noise state; NaN = nothing drawn since the last re-arm
+                                    (kept only when noise_beta != 0) */
+       CF_AUX_COST_RUN = 8 };    /* float[MN]: running part of the cost only */
 #define CF_REC_TABLE_CAP 4096
 #define CF_MAX_OBSTACLES 8
 
@@ -105,6 +109,19 @@ typedef struct cf_params {
   /* planning rollouts (config 3) */
   float obstacles[CF_MAX_OBSTACLES][4];   /* cx cy cz r */
   float noise_sigma[4], cmd_lo[4], cmd_hi[4];
+  /* sampling-based planning (readings R25-R27), CF_CMD_NOMINAL_PLUS_NOISE only */
+  float noise_beta;                  /* R25: AR(1) coefficient of the temporally correlated command noise in [0,1):
+                                        eps <- z for the first command after a reset / cf_set_state, afterwards
+                                        eps <- beta eps + sqrt(1 - beta^2) z;  command = clip(nominal + sigma eps) */
+  int32_t n_ctrl;                    /* R26: number of nominal sequences (independent controllers), >= 1;
+                                        the command buffer of cf_step is then [n_ctrl][n_cmds] float4 */
+  int64_t worlds_per_ctrl;           /* controller of a world = global world index / worlds_per_ctrl (0: controller 0) */
+  int32_t cost_on;                   /* R27: accumulate the rollout cost (needs N == 1) */
+  float cost_goal[3];                /* running cost per step: h (w_pos |p - goal|^2 + w_vel |v|^2), post-step state */
+  float cost_w_pos, cost_w_vel;
+  float cost_w_term;                 /* read-out adds w_term |p - goal|^2 of the current position, */
+  float cost_w_obs, cost_d_safe;     /*   w_obs max(0, d_safe - d_min)^2 with d_min = CF_AUX_MIN_DIST of the drone, */
+  float cost_w_coll;                 /*   and w_coll if d_min < 0 */
 } cf_params;
 
 /* Fill *p with the defaults for `model`.  Host only. */
@@ -139,8 +156,12 @@ int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast);
 int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctrl_dev, const float *wparam_dev,
                 const float *min_d2_dev, int64_t step_counter);
 
+/* Teacher forcing / checkpoint restore of the planning-rollout state: eps [4][MN] (needs noise_beta != 0) and the
+ * running cost [MN] (needs cost_on); NULL = keep. */
+int cf_set_plan_state(cf_sim *sim, const float *eps_dev, const float *cost_run_dev);
+
 /* Advance n_steps >= 1 physics steps in ONE kernel launch (state in registers across all of them).
- *   cmds_dev     [n_cmds][MN] float4, or [n_cmds] float4 for CF_CMD_NOMINAL_PLUS_NOISE; n_cmds*cmd_hold >= n_steps
+ *   cmds_dev     [n_cmds][MN] float4, or [n_ctrl][n_cmds] float4 for CF_CMD_NOMINAL_PLUS_NOISE; n_cmds*cmd_hold >= n_steps
  *   record_every 0: nothing recorded; else see STEP SEMANTICS; record_dev must hold
  *                n_rec = (s0+n_steps)/record_every - s0/record_every slots of D*MN floats (else CF_E_BUFFER). */
 int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold,
@@ -169,6 +190,44 @@ int cf_sync_counters(cf_sim *sim);
 
 /* Name of the kernel instantiation the next cf_step would launch and its launch geometry (for profiling notes). */
 int cf_describe_launch(const cf_sim *sim, char *buf, size_t buf_len, int *grid, int *block);
+
+/* ---- Sampling-based planner around the planning rollout: hybrid iCEM / MPPI update -------
+ * "a hybrid implementation of iCEM and MPPI ..., running five independent controllers in parallel and selecting the
+ *  best control sequence at each step.  Following iCEM, each controller truncates the top 1% of trajectories, uses
+ *  temporally correlated noise, and warmstarts its sampling from the previous mean solution.  To obtain the mean
+ *  across the best samples, we use exponential weighting over all elites, as in MPPI."
+ * No equation or parameter is printed; the readings are DESIGN.md R25-R32:
+ *   rollout k of controller c applied  u_k[t] = clip(nominal_c[t] + sigma eps_k[t])  (R25, R26) and has cost J_k (R27);
+ *   R28 elites E_c = the n_elite rollouts of c with the smallest (J_k as float32 in IEEE total order, NaN last; world index);
+ *   R29 w_k = exp(-(J_k - min_E J) / lambda);   R30 mean_c[t] = sum_E w_k u_k[t] / sum_E w_k;
+ *   R31 score S_c = sum_E w_k J_k / sum_E w_k, best controller = argmin_c S_c (float32, ties -> lowest c);
+ *   R32 plan = mean of the best controller; warm start nominal_c[t] <- mean_c[min(t + shift, H - 1)].
+ * The sampled commands are never stored: the update regenerates the elites' commands from the Philox counters.
+ * Requirements: N == 1, cmd_source == CF_CMD_NOMINAL_PLUS_NOISE, cost_on, M == n_ctrl * worlds_per_ctrl on this
+ * shard (world_offset a multiple of worlds_per_ctrl), and the last calls on sim were a reset / cf_set_state followed by
+ * ONE cf_step of horizon * cmd_hold steps with n_cmds == horizon (else CF_E_STATE). */
+typedef struct cf_mppi_params {
+  uint32_t struct_size;
+  int32_t  horizon;      /* H knots */
+  int32_t  cmd_hold;     /* physics steps per knot */
+  int32_t  n_elite;      /* per controller, 1 .. worlds_per_ctrl (and <= 4096) */
+  int32_t  shift;        /* knots executed between two plans (warm-start shift), 0 .. H */
+  float    lambda;       /* temperature of the exponential weighting, > 0 */
+} cf_mppi_params;
+/* layout of info_dev (float32 / int32 words): per controller c: [4c+0] score S_c, [4c+1] J_min, [4c+2] sum of weights,
+ * [4c+3] cost of the last elite admitted (threshold); then [4 n_ctrl] = index of the best controller (int32). */
+#define CF_MPPI_INFO_WORDS(n_ctrl) (4 * (n_ctrl) + 4)
+size_t cf_mppi_scratch_bytes(const cf_sim *sim, const cf_mppi_params *mp);
+/* nominal_dev [n_ctrl][H] float4: in = the sequences the rollout was sampled around, out = warm-started sequences;
+ * plan_dev [H] float4 (out); info_dev CF_MPPI_INFO_WORDS words (out); elite_idx_dev int32 [n_ctrl][n_elite]
+ * (out, may be NULL): world indices local to the controller, ascending; scratch_dev: cf_mppi_scratch_bytes(), 256-byte
+ * aligned, caller-owned.  Enqueues on the bound stream. */
+int cf_mppi_update(cf_sim *sim, const cf_mppi_params *mp, void *nominal_dev, void *plan_dev, void *info_dev,
+                   int32_t *elite_idx_dev, void *scratch_dev, size_t scratch_bytes);
+/* One planning iteration: cf_set_state(x0_dev [D], broadcast) + cf_step(nominal_dev, H, cmd_hold, H*cmd_hold) +
+ * cf_mppi_update(...). */
+int cf_mppi_iterate(cf_sim *sim, const cf_mppi_params *mp, const float *x0_dev, void *nominal_dev, void *plan_dev,
+                    void *info_dev, int32_t *elite_idx_dev, void *scratch_dev, size_t scratch_bytes);
 
 const char *cf_last_error(void);
 /* Host-side Philox4x32-10 of this library, for the bit-exact check against the oracle's (C9). */

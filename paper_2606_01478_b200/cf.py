@@ -17,7 +17,7 @@ MODEL_FP, MODEL_AB = 0, 1
 EULER, RK4 = 0, 1
 IF_ROTOR, IF_TORQUE, IF_ATTITUDE, IF_POSITION = 0, 1, 2, 3
 CMD_BUFFER, CMD_NOMINAL_PLUS_NOISE = 0, 1
-AUX_COUNTERS, AUX_MIN_DIST, AUX_CTRL, AUX_WORLD_PARAMS, AUX_REC_TABLE, AUX_MIN_D2 = range(6)
+AUX_COUNTERS, AUX_MIN_DIST, AUX_CTRL, AUX_WORLD_PARAMS, AUX_REC_TABLE, AUX_MIN_D2, AUX_COST, AUX_EPS, AUX_COST_RUN = range(9)
 REC_TABLE_CAP = 4096
 OK, E_ARG, E_SHAPE, E_STATE, E_BUFFER, E_CUDA, E_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
@@ -45,7 +45,16 @@ class Params(C.Structure):
         ("grid_spacing", f), ("grid_jitter", f), ("grid_origin", f * 3),
         ("obstacles", (f * 4) * 8),
         ("noise_sigma", f * 4), ("cmd_lo", f * 4), ("cmd_hi", f * 4),
+        ("noise_beta", f), ("n_ctrl", C.c_int32), ("worlds_per_ctrl", C.c_int64), ("cost_on", C.c_int32),
+        ("cost_goal", f * 3), ("cost_w_pos", f), ("cost_w_vel", f), ("cost_w_term", f), ("cost_w_obs", f),
+        ("cost_d_safe", f), ("cost_w_coll", f),
     ]
+
+
+class MppiParams(C.Structure):
+    """Mirror of `cf_mppi_params` (include/cf.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("horizon", C.c_int32), ("cmd_hold", C.c_int32), ("n_elite", C.c_int32),
+                ("shift", C.c_int32), ("lam", f)]
 
 
 class CfError(RuntimeError):
@@ -88,6 +97,10 @@ def lib():
         "cf_step_counter": (i64, [vp]),
         "cf_sync_counters": (C.c_int, [vp]),
         "cf_describe_launch": (C.c_int, [vp, C.c_char_p, sz, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+        "cf_set_plan_state": (C.c_int, [vp, vp, vp]),
+        "cf_mppi_scratch_bytes": (sz, [vp, C.POINTER(MppiParams)]),
+        "cf_mppi_update": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, sz]),
+        "cf_mppi_iterate": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, sz]),
         "cf_last_error": (C.c_char_p, []),
         "cf_debug_philox": (C.c_int, [C.c_uint64, C.POINTER(C.c_uint32 * 4), C.POINTER(C.c_uint32 * 4)]),
         "cf_debug_philox_dev": (C.c_int, [vp, C.c_uint64, vp, C.c_int, vp, vp, vp]),
@@ -102,7 +115,8 @@ def lib():
 EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_workspace_bytes", "cf_create", "cf_destroy",
            "cf_set_stream", "cf_reset", "cf_set_state", "cf_set_full", "cf_step", "cf_staging_bytes", "cf_step_host",
            "cf_get_state", "cf_get_state_host", "cf_get_aux", "cf_get_aux_host", "cf_step_counter", "cf_sync_counters",
-           "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev"]
+           "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
+           "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate"]
 
 
 def _check(rc: int):
@@ -225,11 +239,11 @@ class Sim:
         return (s0 + n_steps) // record_every - s0 // record_every
 
     def step(self, cmds, n_steps: int, cmd_hold: int = 1, record_every: int = 0, record=None):
-        """cmds: device tensor float32 [K][MN][4] (or [K][4] for nominal+noise).  Returns the record tensor
+        """cmds: device tensor float32 [K][MN][4] (or [n_ctrl][K][4] for nominal+noise).  Returns the record tensor
         [n_rec][D][MN] (allocated here unless `record` is given) or None.  Asynchronous on the bound stream."""
         torch = _torch()
         cm = self._dev(cmds, torch.float32)
-        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4
+        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4 * self.params.n_ctrl
         assert cm.numel() % per == 0, (tuple(cm.shape), per)
         n_rec = self.n_records(n_steps, record_every)
         if n_rec and record is None:
@@ -247,7 +261,7 @@ class Sim:
     def step_host(self, cmds_host, n_steps: int, cmd_hold: int = 1, record_every: int = 0, record_host=None):
         """cmds_host / record_host: CPU tensors (pinned for full speed).  Synchronous."""
         torch = _torch()
-        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4
+        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4 * self.params.n_ctrl
         assert cmds_host.dtype == torch.float32 and cmds_host.is_contiguous() and not cmds_host.is_cuda
         n_cmds = cmds_host.numel() // per
         need = lib().cf_staging_bytes(self._h, n_cmds, int(n_steps), int(record_every))
@@ -302,6 +316,67 @@ class Sim:
 
     def min_d2(self):
         return self._aux(AUX_MIN_D2, (8, self.MN), _torch().float32)
+
+    def cost(self):
+        return self._aux(AUX_COST, (self.MN,), _torch().float32)
+
+    def cost_run(self):
+        return self._aux(AUX_COST_RUN, (self.MN,), _torch().float32)
+
+    def eps(self):
+        return self._aux(AUX_EPS, (4, self.MN), _torch().float32)
+
+    def set_plan_state(self, eps=None, cost_run=None):
+        f32 = _torch().float32
+        e = None if eps is None else self._dev(eps, f32)
+        c = None if cost_run is None else self._dev(cost_run, f32)
+        assert e is None or e.numel() == 4 * self.MN
+        assert c is None or c.numel() == self.MN
+        _check(lib().cf_set_plan_state(self._h, _dptr(e), _dptr(c)))
+
+    # -- sampling-based planner (cf_mppi_*) --------------------------------------------------------------------------
+    def mppi_params(self, horizon: int, cmd_hold: int, n_elite: int, lam: float, shift: int = 1) -> MppiParams:
+        return MppiParams(C.sizeof(MppiParams), int(horizon), int(cmd_hold), int(n_elite), int(shift), float(lam))
+
+    def _mppi_buffers(self, mp: MppiParams, want_elites: bool):
+        torch = _torch()
+        key = (mp.horizon, mp.n_elite)
+        if getattr(self, "_mppi_key", None) != key:
+            need = lib().cf_mppi_scratch_bytes(self._h, C.byref(mp))
+            if need == 0:
+                raise CfError(E_ARG, lib().cf_last_error().decode())
+            self._mppi_scratch = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+            self._mppi_need = need
+            self._mppi_plan = torch.empty((mp.horizon, 4), dtype=torch.float32, device=self.device)
+            self._mppi_info = torch.empty(4 * self.params.n_ctrl + 4, dtype=torch.float32, device=self.device)
+            self._mppi_elites = torch.empty((self.params.n_ctrl, mp.n_elite), dtype=torch.int32, device=self.device)
+            self._mppi_key = key
+        sp = self._mppi_scratch.data_ptr() + (-self._mppi_scratch.data_ptr()) % 256
+        return C.c_void_p(sp), self._mppi_need, (_dptr(self._mppi_elites) if want_elites else None)
+
+    def _mppi_result(self, nominal, want_elites):
+        return dict(nominal=nominal, plan=self._mppi_plan, info=self._mppi_info,
+                    elites=self._mppi_elites if want_elites else None)
+
+    def mppi_update(self, mp: MppiParams, nominal, want_elites: bool = False):
+        """nominal: device tensor float32 [n_ctrl][H][4], updated IN PLACE to the warm-started sequences.  Returns
+        dict(nominal, plan [H][4], info [4 n_ctrl + 4] (last word viewed as int32 = best controller), elites)."""
+        sp, need, el = self._mppi_buffers(mp, want_elites)
+        assert nominal.is_cuda and nominal.dtype == _torch().float32 and nominal.is_contiguous()
+        assert nominal.numel() == self.params.n_ctrl * mp.horizon * 4
+        _check(lib().cf_mppi_update(self._h, C.byref(mp), _dptr(nominal), _dptr(self._mppi_plan),
+                                    _dptr(self._mppi_info), el, sp, need))
+        return self._mppi_result(nominal, want_elites)
+
+    def mppi_iterate(self, mp: MppiParams, x0, nominal, want_elites: bool = False):
+        """One planning iteration: broadcast reset to x0 [D] + fused rollout + update (cf_mppi_iterate)."""
+        sp, need, el = self._mppi_buffers(mp, want_elites)
+        assert x0.is_cuda and x0.dtype == _torch().float32 and x0.numel() == self.D
+        assert nominal.is_cuda and nominal.dtype == _torch().float32 and nominal.is_contiguous()
+        assert nominal.numel() == self.params.n_ctrl * mp.horizon * 4
+        _check(lib().cf_mppi_iterate(self._h, C.byref(mp), _dptr(x0), _dptr(nominal), _dptr(self._mppi_plan),
+                                     _dptr(self._mppi_info), el, sp, need))
+        return self._mppi_result(nominal, want_elites)
 
     def rec_table(self):
         return self._aux(AUX_REC_TABLE, (REC_TABLE_CAP,), _torch().int32).cpu().numpy().view(np.uint32)

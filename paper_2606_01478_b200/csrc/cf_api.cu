@@ -2,6 +2,7 @@
 // non-hot kernels (reset, set_state, minimum-distance read-out, Philox debug).  No device allocation, no CPU path.
 #include "../../include/cf.h"
 #include "cf_device.cuh"
+#include "cf_internal.h"
 
 #include <cmath>
 #include <cstdarg>
@@ -11,38 +12,8 @@
 
 using namespace cf;
 
-struct cf_sim {
-  long long M, N, MN;
-  int model, D, P;
-  cf_params p;
-  DevParams dp;
-  int opt;                    // option bits this configuration needs
-  // workspace carving (device pointers into the caller's buffer)
-  float *state, *ctrl, *wparam, *min_d2;
-  float *bcast_buf;           // [D] pending broadcast state (cf_set_state(broadcast) is folded into the next cf_step)
-  float *md_drone;            // [MN] per-drone minimum distance written by the rollout kernel's epilogue
-  bool pending_bcast, md_valid;
-  Counters *counters;
-  uint32_t *rec_table;
-  cudaStream_t stream;
-  uint64_t seed;
-  long long s_host;           // host mirror of the step counter
-  long long n_rec_host;
-  bool have_state;
-  float hover_rpm;
-};
-
 static thread_local char g_err[512] = "";
-static int fail(int code, const char *fmt, ...) {
-  va_list ap;
-  va_start(ap, fmt);
-  vsnprintf(g_err, sizeof(g_err), fmt, ap);
-  va_end(ap);
-  return code;
-}
-#define CF_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) \
-  return fail(CF_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
-
+char *cf_err_buf() { return g_err; }
 extern "C" const char *cf_last_error(void) { return g_err; }
 extern "C" int cf_state_dim(int model) { return model == CF_MODEL_FIRST_PRINCIPLES ? 17 : model == CF_MODEL_ABSTRACTED ? 13 : 0; }
 extern "C" int cf_world_param_dim(int model) { return model == CF_MODEL_FIRST_PRINCIPLES ? 14 : model == CF_MODEL_ABSTRACTED ? 11 : 0; }
@@ -73,11 +44,13 @@ extern "C" void cf_default_params(cf_params *p, int model) {
   const float pi = 3.14159265358979323846f;
   p->cmd_lo[0] = -0.5f; p->cmd_lo[1] = -0.5f; p->cmd_lo[2] = -pi; p->cmd_lo[3] = 0.05f;
   p->cmd_hi[0] = 0.5f;  p->cmd_hi[1] = 0.5f;  p->cmd_hi[2] = pi;  p->cmd_hi[3] = 0.55f;
+  p->n_ctrl = 1;
 }
 
 static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
-struct Carve { size_t state, ctrl, wparam, min_d2, md_drone, bcast, counters, rec_table, total; };
+struct Carve { size_t state, ctrl, wparam, min_d2, md_drone, eps, cost_run, cost_drone, bcast, counters, rec_table, total; };
+static bool wants_eps(const cf_params *p) { return p->cmd_source == CF_CMD_NOMINAL_PLUS_NOISE && p->noise_beta != 0.f; }
 static Carve carve(long long M, long long N, int model, const cf_params *p) {
   Carve c;
   size_t MN = (size_t)(M * N), off = 0;
@@ -86,6 +59,9 @@ static Carve carve(long long M, long long N, int model, const cf_params *p) {
   c.wparam = off;    off += align256(sizeof(float) * cf_world_param_dim(model) * (size_t)M);
   c.min_d2 = off;    off += p->n_obstacles > 0 ? align256(sizeof(float) * kMaxObst * MN) : 0;
   c.md_drone = off;  off += p->n_obstacles > 0 ? align256(sizeof(float) * MN) : 0;
+  c.eps = off;       off += wants_eps(p) ? align256(sizeof(float) * 4 * MN) : 0;
+  c.cost_run = off;  off += p->cost_on ? align256(sizeof(float) * MN) : 0;
+  c.cost_drone = off; off += p->cost_on ? align256(sizeof(float) * MN) : 0;
   c.bcast = off;     off += 256;
   c.counters = off;  off += align256(sizeof(Counters));
   c.rec_table = off; off += align256(sizeof(uint32_t) * kRecTableCap);
@@ -116,6 +92,12 @@ static int validate(long long M, long long N, int model, const cf_params *p) {
   if (!(p->mass > 0) || !(p->J[0] > 0) || !(p->J[1] > 0) || !(p->J[2] > 0)) return fail(CF_E_ARG, "mass/J must be > 0");
   if (model == CF_MODEL_FIRST_PRINCIPLES && p->iface != CF_IF_ROTOR && !(p->kf[2] > 0))
     return fail(CF_E_ARG, "controller needs kf[2] > 0");
+  if (!(p->noise_beta >= 0.f && p->noise_beta < 1.f)) return fail(CF_E_ARG, "noise_beta must be in [0, 1)");
+  if (p->n_ctrl < 1 || p->worlds_per_ctrl < 0) return fail(CF_E_ARG, "n_ctrl >= 1 and worlds_per_ctrl >= 0");
+  if (p->cmd_source == CF_CMD_NOMINAL_PLUS_NOISE && p->worlds_per_ctrl > 0 &&
+      (p->world_offset + M - 1) / p->worlds_per_ctrl >= p->n_ctrl)
+    return fail(CF_E_SHAPE, "worlds %lld.. need more than n_ctrl = %d nominal sequences", (long long)p->world_offset, p->n_ctrl);
+  if (p->cost_on && N != 1) return fail(CF_E_UNSUPPORTED, "the rollout cost needs N == 1");
   if (p->world_offset < 0 || p->world_offset + M > ((long long)1 << 32)) return fail(CF_E_SHAPE, "world_offset out of range");
   return CF_OK;
 }
@@ -179,6 +161,11 @@ static void fill_dev_params(cf_sim *s) {
     }
   }
   for (int k = 0; k < 4; ++k) { d.noise_sigma[k] = p.noise_sigma[k]; d.cmd_lo[k] = p.cmd_lo[k]; d.cmd_hi[k] = p.cmd_hi[k]; }
+  d.noise_beta = p.noise_beta; d.noise_gain = (float)std::sqrt(1.0 - (double)p.noise_beta * p.noise_beta);
+  for (int k = 0; k < 3; ++k) d.cost_goal[k] = p.cost_goal[k];
+  d.cost_hw_pos = (float)(h * p.cost_w_pos); d.cost_hw_vel = (float)(h * p.cost_w_vel);
+  d.cost_w_term = p.cost_w_term; d.cost_w_obs = p.cost_w_obs; d.cost_d_safe = p.cost_d_safe; d.cost_w_coll = p.cost_w_coll;
+  d.cost_on = p.cost_on;
 }
 
 static int needed_opt(const cf_sim *s) {
@@ -188,6 +175,7 @@ static int needed_opt(const cf_sim *s) {
   if (p.dist_sigma > 0.f) opt |= OPT_DIST;
   if (p.n_obstacles > 0) opt |= OPT_OBST;
   if (p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE) opt |= OPT_NOISE;
+  if (p.cost_on) opt |= OPT_COST;
   bool extras = p.Jp != 0.f || p.Ca[0] != 0.f || p.Ca[1] != 0.f || p.Ca[2] != 0.f;
   if (s->model == CF_MODEL_FIRST_PRINCIPLES)
     extras = extras || p.cv_up != p.cv_dn || p.cd_up != 0.f || p.cd_dn != 0.f || p.kf[0] != 0.f || p.kf[1] != 0.f ||
@@ -239,8 +227,12 @@ __global__ void reset_params_kernel(float *wparam, const __grid_constant__ Reset
 }
 
 // controller integrals 0, held commands = hover of the nominal model, min distance +inf (reading R20)
-__device__ __forceinline__ void rearm(float *ctrl, float *min_d2, long long MN, long long i, float hover_rpm,
+struct RearmPlanes { float *ctrl, *min_d2, *eps, *cost_run; };
+__device__ __forceinline__ void rearm(const RearmPlanes &rp, long long MN, long long i, float hover_rpm,
                                       float hover_thrust) {
+  float *ctrl = rp.ctrl, *min_d2 = rp.min_d2;
+  if (rp.eps) rp.eps[i] = __int_as_float(0x7fc00000);      // R25: NaN in plane 0 = the next command starts a fresh chain
+  if (rp.cost_run) rp.cost_run[i] = 0.f;                   // R27
 #pragma unroll
   for (int c = 0; c < 9; ++c) ctrl[c * MN + i] = 0.f;
   ctrl[9 * MN + i] = hover_thrust;
@@ -252,7 +244,7 @@ __device__ __forceinline__ void rearm(float *ctrl, float *min_d2, long long MN, 
   }
 }
 
-__global__ void reset_state_kernel(float *state, float *ctrl, float *min_d2, const __grid_constant__ ResetArgs R) {
+__global__ void reset_state_kernel(float *state, RearmPlanes rp, const __grid_constant__ ResetArgs R) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= R.MN) return;
   long long w = i / R.N, n = i - w * R.N;
@@ -293,15 +285,15 @@ __global__ void reset_state_kernel(float *state, float *ctrl, float *min_d2, con
     state[5 * MN + i] = atan2f(Rm[1][0], Rm[0][0]);
     state[12 * MN + i] = R.hover_thrust;
   }
-  rearm(ctrl, min_d2, MN, i, R.model == MODEL_FP ? R.hover_rpm : 0.f, R.hover_thrust);
+  rearm(rp, MN, i, R.model == MODEL_FP ? R.hover_rpm : 0.f, R.hover_thrust);
 }
 
-__global__ void set_state_kernel(float *state, float *ctrl, float *min_d2, const float *src, int broadcast, int D,
+__global__ void set_state_kernel(float *state, RearmPlanes rp, const float *src, int broadcast, int D,
                                  long long MN, float hover_rpm, float hover_thrust) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= MN) return;
   for (int j = 0; j < D; ++j) state[j * MN + i] = broadcast ? src[j] : src[j * MN + i];
-  rearm(ctrl, min_d2, MN, i, hover_rpm, hover_thrust);
+  rearm(rp, MN, i, hover_rpm, hover_thrust);
 }
 
 __global__ void set_counters_kernel(Counters *c, uint32_t s, int zero_rest) {
@@ -337,6 +329,25 @@ __global__ void min_dist_small_n_kernel(const float *min_d2, float *out, long lo
       if (j < P.n_obst) best = fminf(best, sqrtf(min_d2[j * MN + w * N + n]) - P.obst[j][3]);
   }
   out[w] = best;
+}
+
+// R27 read-out outside the rollout epilogue (after cf_set_state / cf_set_full): same terms, from the planes
+__global__ void cost_readout_kernel(const float *state, const float *min_d2, const float *cost_run, float *out,
+                                    long long MN, const __grid_constant__ DevParams P) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= MN) return;
+  float d_min = __int_as_float(0x7f800000);
+  if (min_d2) {
+#pragma unroll
+    for (int j = 0; j < kMaxObst; ++j)
+      if (j < P.n_obst) d_min = fminf(d_min, sqrtf(min_d2[j * MN + i]) - P.obst[j][3]);
+  }
+  float ex = state[i] - P.cost_goal[0], ey = state[MN + i] - P.cost_goal[1], ez = state[2 * MN + i] - P.cost_goal[2];
+  float J = fmaf(P.cost_w_term, fmaf(ez, ez, fmaf(ey, ey, ex * ex)), cost_run[i]);
+  float gap = P.cost_d_safe - d_min;
+  if (gap > 0.0f) J = fmaf(P.cost_w_obs * gap, gap, J);
+  if (d_min < 0.0f) J += P.cost_w_coll;
+  out[i] = J;
 }
 
 __global__ void philox_debug_kernel(uint32_t seed_lo, uint32_t seed_hi, const uint32_t *ctr, int n, uint32_t *words,
@@ -375,6 +386,10 @@ extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf
   s->min_d2 = p->n_obstacles > 0 ? (float *)(base + c.min_d2) : nullptr;
   s->md_drone = p->n_obstacles > 0 ? (float *)(base + c.md_drone) : nullptr;
   s->bcast_buf = (float *)(base + c.bcast);
+  s->eps = wants_eps(p) ? (float *)(base + c.eps) : nullptr;
+  s->cost_run = p->cost_on ? (float *)(base + c.cost_run) : nullptr;
+  s->cost_drone = p->cost_on ? (float *)(base + c.cost_drone) : nullptr;
+  s->cost_valid = false; s->rearmed = false; s->last_fresh = false; s->last_s0 = 0; s->last_n_steps = s->last_n_cmds = s->last_cmd_hold = 0;
   s->pending_bcast = false; s->md_valid = false;
   s->counters = (Counters *)(base + c.counters); s->rec_table = (uint32_t *)(base + c.rec_table);
   s->stream = 0; s->seed = 0; s->s_host = 0; s->n_rec_host = 0; s->have_state = false;
@@ -403,6 +418,7 @@ extern "C" int cf_set_stream(cf_sim *sim, void *cuda_stream) {
 }
 
 static int grid_for(long long n, int block) { return (int)((n + block - 1) / block); }
+static RearmPlanes rearm_planes(const cf_sim *sim) { return RearmPlanes{ sim->ctrl, sim->min_d2, sim->eps, sim->cost_run }; }
 
 extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
@@ -428,19 +444,19 @@ extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
   R.M = sim->M; R.N = sim->N; R.MN = sim->MN; R.world_offset = p.world_offset;
   R.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu); R.seed_hi = (uint32_t)(seed >> 32);
   reset_params_kernel<<<grid_for(sim->M, 128), 128, 0, sim->stream>>>(sim->wparam, R);
-  reset_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(sim->state, sim->ctrl, sim->min_d2, R);
+  reset_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(sim->state, rearm_planes(sim), R);
   set_counters_kernel<<<1, 1, 0, sim->stream>>>(sim->counters, 0u, 1);
   CF_CUDA(cudaMemsetAsync(sim->rec_table, 0, sizeof(uint32_t) * kRecTableCap, sim->stream));
   CF_CUDA(cudaGetLastError());
   sim->seed = seed; sim->s_host = 0; sim->n_rec_host = 0; sim->have_state = true;
-  sim->pending_bcast = false; sim->md_valid = false;
+  sim->pending_bcast = false; sim->md_valid = false; sim->cost_valid = false; sim->rearmed = true;
   return CF_OK;
 }
 
 static int launch_set_state(cf_sim *sim, const float *src, int broadcast) {
   float hover_thrust = (float)((double)sim->p.mass * sim->p.g);
   set_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(
-      sim->state, sim->ctrl, sim->min_d2, src, broadcast, sim->D, sim->MN,
+      sim->state, rearm_planes(sim), src, broadcast, sim->D, sim->MN,
       sim->model == CF_MODEL_FIRST_PRINCIPLES ? sim->hover_rpm : 0.f, hover_thrust);
   CF_CUDA(cudaGetLastError());
   return CF_OK;
@@ -457,7 +473,7 @@ static int materialise(cf_sim *sim) {
 extern "C" int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast) {
   if (!sim || !state_dev) return fail(CF_E_ARG, "NULL argument");
   if (!sim->have_state) return fail(CF_E_STATE, "cf_set_state needs a prior cf_reset (world parameters)");
-  sim->md_valid = false;
+  sim->md_valid = false; sim->cost_valid = false; sim->rearmed = true;
   if (broadcast) {
     CF_CUDA(cudaMemcpyAsync(sim->bcast_buf, state_dev, sizeof(float) * sim->D, cudaMemcpyDeviceToDevice, sim->stream));
     sim->pending_bcast = true;
@@ -467,11 +483,27 @@ extern "C" int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast) 
   return launch_set_state(sim, state_dev, 0);
 }
 
+extern "C" int cf_set_plan_state(cf_sim *sim, const float *eps_dev, const float *cost_run_dev) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
+  const size_t MN = (size_t)sim->MN;
+  if (eps_dev) {
+    if (!sim->eps) return fail(CF_E_ARG, "no AR(1) noise state: needs CF_CMD_NOMINAL_PLUS_NOISE with noise_beta != 0");
+    CF_CUDA(cudaMemcpyAsync(sim->eps, eps_dev, sizeof(float) * 4 * MN, cudaMemcpyDeviceToDevice, sim->stream));
+  }
+  if (cost_run_dev) {
+    if (!sim->cost_run) return fail(CF_E_ARG, "cost_on is 0");
+    CF_CUDA(cudaMemcpyAsync(sim->cost_run, cost_run_dev, sizeof(float) * MN, cudaMemcpyDeviceToDevice, sim->stream));
+  }
+  sim->cost_valid = false; sim->rearmed = false;
+  return CF_OK;
+}
+
 extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctrl_dev, const float *wparam_dev,
                            const float *min_d2_dev, int64_t step_counter) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
   { int rc = materialise(sim); if (rc != CF_OK) return rc; }
-  sim->md_valid = false;
+  sim->md_valid = false; sim->cost_valid = false; sim->rearmed = false;
   const size_t MN = (size_t)sim->MN;
   if (state_dev) CF_CUDA(cudaMemcpyAsync(sim->state, state_dev, sizeof(float) * sim->D * MN, cudaMemcpyDeviceToDevice, sim->stream));
   if (ctrl_dev) CF_CUDA(cudaMemcpyAsync(sim->ctrl, ctrl_dev, sizeof(float) * kCtrlPlanes * MN, cudaMemcpyDeviceToDevice, sim->stream));
@@ -545,6 +577,8 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   StepArgs A;
   A.state = sim->state; A.ctrl = sim->ctrl; A.wparam = sim->wparam; A.min_d2 = sim->min_d2;
   A.bcast = sim->pending_bcast ? sim->bcast_buf : nullptr; A.md_drone = sim->md_drone;
+  A.eps = sim->eps; A.cost_run = sim->cost_run; A.cost_drone = sim->cost_drone;
+  A.worlds_per_ctrl = sim->p.worlds_per_ctrl; A.n_cmds = n_cmds;
   A.counters = sim->counters; A.rec_table = sim->rec_table;
   A.cmds = (const float4 *)cmds_dev; A.record = record_dev;
   A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.world_offset = sim->p.world_offset;
@@ -562,13 +596,16 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   sim->n_rec_host += n_rec;
   sim->pending_bcast = false;
   sim->md_valid = sim->min_d2 != nullptr;
+  sim->cost_valid = sim->cost_run != nullptr;
+  sim->last_fresh = sim->rearmed; sim->last_s0 = s0; sim->last_n_steps = n_steps; sim->last_n_cmds = n_cmds;
+  sim->last_cmd_hold = cmd_hold; sim->rearmed = false;
   return CF_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // host-buffer (end-to-end) path
 static size_t cmd_bytes(const cf_sim *sim, int n_cmds) {
-  size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? 1 : (size_t)sim->MN;
+  size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? (size_t)sim->p.n_ctrl : (size_t)sim->MN;
   return align256(sizeof(float) * 4 * per * (size_t)n_cmds);
 }
 static long long n_records(const cf_sim *sim, int n_steps, int record_every) {
@@ -591,7 +628,7 @@ extern "C" int cf_step_host(cf_sim *sim, const void *cmds_host, int n_cmds, int 
   size_t cb = cmd_bytes(sim, n_cmds);
   size_t rb = (size_t)n_records(sim, n_steps, record_every) * sim->D * (size_t)sim->MN * sizeof(float);
   if (rb > 0 && (!record_host || record_bytes < rb)) return fail(CF_E_BUFFER, "host record buffer too small");
-  size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? 1 : (size_t)sim->MN;
+  size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? (size_t)sim->p.n_ctrl : (size_t)sim->MN;
   CF_CUDA(cudaMemcpyAsync(staging_dev, cmds_host, sizeof(float) * 4 * per * (size_t)n_cmds, cudaMemcpyHostToDevice, sim->stream));
   float *rec_dev = (float *)((char *)staging_dev + cb);
   int rc = cf_step(sim, staging_dev, n_cmds, cmd_hold, n_steps, record_every, rec_dev, rb);
@@ -615,6 +652,19 @@ extern "C" int cf_get_state_host(cf_sim *sim, float *out_host) {
   return CF_OK;
 }
 
+// make cost_drone hold J of the current planes (it already does straight after a cf_step: rollout epilogue)
+int cf_refresh_cost(cf_sim *sim) {
+  if (!sim->cost_run) return fail(CF_E_ARG, "cost_on is 0");
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
+  if (!sim->cost_valid) {
+    cost_readout_kernel<<<grid_for(sim->MN, 256), 256, 0, sim->stream>>>(sim->state, sim->min_d2, sim->cost_run,
+                                                                          sim->cost_drone, sim->MN, sim->dp);
+    CF_CUDA(cudaGetLastError());
+    sim->cost_valid = true;
+  }
+  return CF_OK;
+}
+
 static int aux_source(cf_sim *sim, int which, const void **src, size_t *bytes) {
   const size_t MN = (size_t)sim->MN;
   { int rc = materialise(sim); if (rc != CF_OK) return rc; }
@@ -626,6 +676,17 @@ static int aux_source(cf_sim *sim, int which, const void **src, size_t *bytes) {
     case CF_AUX_MIN_D2:
       if (!sim->min_d2) return fail(CF_E_ARG, "no obstacles configured");
       *src = sim->min_d2; *bytes = sizeof(float) * kMaxObst * MN; return CF_OK;
+    case CF_AUX_EPS:
+      if (!sim->eps) return fail(CF_E_ARG, "no AR(1) noise state: needs CF_CMD_NOMINAL_PLUS_NOISE with noise_beta != 0");
+      *src = sim->eps; *bytes = sizeof(float) * 4 * MN; return CF_OK;
+    case CF_AUX_COST_RUN:
+      if (!sim->cost_run) return fail(CF_E_ARG, "cost_on is 0");
+      *src = sim->cost_run; *bytes = sizeof(float) * MN; return CF_OK;
+    case CF_AUX_COST: {
+      int rc = cf_refresh_cost(sim);
+      if (rc != CF_OK) return rc;
+      *src = sim->cost_drone; *bytes = sizeof(float) * MN; return CF_OK;
+    }
   }
   return fail(CF_E_ARG, "bad aux selector %d", which);
 }

@@ -21,7 +21,8 @@ enum : int {
   OPT_NOISE = 8,    // command = clip(nominal[k] + sigma * z), z from Philox (CF_CMD_NOMINAL_PLUS_NOISE)
   OPT_EXTRAS = 16,  // full Eq. (6) (asymmetric + quadratic), thrust/torque polynomials, Eq. (5) gyro, body drag,
                     // simplified AB variant
-  OPT_ALL = 31
+  OPT_COST = 32,    // rollout cost for the sampling-based planner (reading R27)
+  OPT_ALL = 63
 };
 enum : int { MODEL_FP = 0, MODEL_AB = 1 };
 enum : int { INTEG_EULER = 0, INTEG_RK4 = 1 };
@@ -51,6 +52,10 @@ struct DevParams {
   float obst[kMaxObst][4];        // cx cy cz r (read-out)
   float4 obst_q[kMaxObst];        // (-2cx, -2cy, -2cz, c.c): d^2 = |p|^2 + q.(p,1); unused slots (0,0,0,+inf)
   float noise_sigma[4], cmd_lo[4], cmd_hi[4];
+  float noise_beta, noise_gain;    // R25: AR(1) coefficient and sqrt(1 - beta^2)
+  float cost_goal[3], cost_hw_pos, cost_hw_vel;   // R27: h w_pos, h w_vel (running), and the read-out terms:
+  float cost_w_term, cost_w_obs, cost_d_safe, cost_w_coll;
+  int   cost_on;
   int   att_div, pos_div;
   float hover_thrust, hover_rpm;   // reading R20: held commands after a reset / set_state
 };
@@ -62,6 +67,11 @@ struct StepArgs {
   float *min_d2;           // [8][MN] or nullptr
   const float *bcast;      // [D] or nullptr: start every drone from this state with re-armed controllers (lazy cf_set_state)
   float *md_drone;         // [MN] or nullptr: per-drone min over obstacles and steps of |p - c_j| - r_j (epilogue)
+  float *eps;              // [4][MN] or nullptr: AR(1) command-noise state (kept when noise_beta != 0)
+  float *cost_run;         // [MN] or nullptr: running rollout cost
+  float *cost_drone;       // [MN] or nullptr: total rollout cost J (epilogue, R27)
+  long long worlds_per_ctrl;   // R26: nominal sequence of a world = cmds + (global world / worlds_per_ctrl) * n_cmds
+  int n_cmds;
   Counters *counters;
   uint32_t *rec_table;     // [kRecTableCap]
   const float4 *cmds;      // [K][MN] or [K]
@@ -614,6 +624,10 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     float target[4] = { 0, 0, 0, 0 };
     float md2[kMaxObst];
     const bool obst = (OPT & OPT_OBST) != 0 && A.min_d2 != nullptr;
+    const bool ar = (OPT & OPT_NOISE) != 0 && A.eps != nullptr;              // temporally correlated noise (R25)
+    const bool costing = (OPT & OPT_COST) != 0 && A.cost_run != nullptr;     // R27
+    float eps[4] = { 0, 0, 0, 0 };
+    float cost = 0.0f;
     if (A.bcast != nullptr) {
       // lazy cf_set_state(broadcast): every drone starts from the same state (uniform loads), controller integrals 0,
       // held commands = hover, obstacle minima re-armed -- nothing is read from the planes
@@ -624,9 +638,15 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       for (int j = 0; j < 4; ++j) rpm_cmd[j] = P.hover_rpm;
 #pragma unroll
       for (int j = 0; j < kMaxObst; ++j) md2[j] = __int_as_float(0x7f800000);
+      eps[0] = __int_as_float(0x7fc00000);                     // NaN: the next command starts a fresh noise chain
     } else {
 #pragma unroll
       for (int j = 0; j < D; ++j) x[j] = A.state[j * MN + i];
+      if (ar) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) eps[j] = A.eps[j * MN + i];
+      }
+      if (costing) cost = A.cost_run[i];
       if (HAS_ATT) {
 #pragma unroll
         for (int j = 0; j < 3; ++j) iR[j] = A.ctrl[j * MN + i];
@@ -663,7 +683,9 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     float *rec_ptr = A.record + (size_t)(lane >> 3) * MN + (i - lane) + 4 * (lane & 7);
     int cmd_cd = 0;
     const bool noise = (OPT & OPT_NOISE) != 0 && P.use_noise;   // compiled in AND requested
-    const float4 *cp = noise ? A.cmds : A.cmds + i;             // next command to prefetch
+    // next command to prefetch; in noise mode the nominal sequence of this world's controller (R26)
+    const float4 *cp = noise ? A.cmds + (A.worlds_per_ctrl > 0 ? (long long)(wg / (uint32_t)A.worlds_per_ctrl) * A.n_cmds : 0)
+                             : A.cmds + i;
     const long long cstride = noise ? 1 : MN;
     int cmds_left = (A.n_steps + A.cmd_hold - 1) / A.cmd_hold;  // commands this call consumes
     float4 next_cmd = __ldg(cp);
@@ -680,6 +702,11 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           philox4x32_10_rk(A.rk, wg, nn, s, STREAM_NOISE, r);
           normal_pair(r[0], r[1], z[0], z[1]);
           normal_pair(r[2], r[3], z[2], z[3]);
+          if (ar) {                                            // eps <- z (fresh chain) or beta eps + sqrt(1-beta^2) z
+            const bool fresh = eps[0] != eps[0];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { eps[j] = fresh ? z[j] : fmaf(P.noise_beta, eps[j], P.noise_gain * z[j]); z[j] = eps[j]; }
+          }
 #pragma unroll
           for (int j = 0; j < 4; ++j) c[j] = clipf(fmaf(P.noise_sigma[j], z[j], c[j]), P.cmd_lo[j], P.cmd_hi[j]);
         }
@@ -751,6 +778,13 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           md2[j] = fminf(md2[j], tq + pp);
         }
       }
+      // (7b) running rollout cost on the post-step state (R27): h w_pos |p - goal|^2 + h w_vel |v|^2
+      if (costing) {
+        const float *v = FP ? x + 7 : x + 6;
+        float ex = x[0] - P.cost_goal[0], ey = x[1] - P.cost_goal[1], ez = x[2] - P.cost_goal[2];
+        float e2 = fmaf(ez, ez, fmaf(ey, ey, ex * ex)), v2 = fmaf(v[2], v[2], fmaf(v[1], v[1], v[0] * v[0]));
+        cost = fmaf(P.cost_hw_pos, e2, fmaf(P.cost_hw_vel, v2, cost));
+      }
       // (8) record (streaming stores; a warp writes whole 128-byte lines of each plane)
       if (A.record_every > 0) {
         if (++rec_phase == A.record_every) {
@@ -802,16 +836,29 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
 #pragma unroll
       for (int j = 0; j < 4; ++j) A.ctrl[(10 + j) * MN + i] = rpm_cmd[j];
     }
+    float d_min = __int_as_float(0x7f800000);
     if (obst) {
 #pragma unroll
       for (int j = 0; j < kMaxObst; ++j) A.min_d2[j * MN + i] = md2[j];
-      if (A.md_drone != nullptr) {       // C10 read-out fused into the epilogue: min_j sqrt(min_t d2_j) - r_j
-        float best = __int_as_float(0x7f800000);
+      if (A.md_drone != nullptr || costing) {   // C10 read-out fused into the epilogue: min_j sqrt(min_t d2_j) - r_j
 #pragma unroll
         for (int j = 0; j < kMaxObst; ++j)
-          if (j < P.n_obst) best = fminf(best, sqrtf(md2[j]) - P.obst[j][3]);
-        A.md_drone[i] = best;
+          if (j < P.n_obst) d_min = fminf(d_min, sqrtf(md2[j]) - P.obst[j][3]);
+        if (A.md_drone != nullptr) A.md_drone[i] = d_min;
       }
+    }
+    if (ar) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) A.eps[j * MN + i] = eps[j];
+    }
+    if (costing) {       // R27 read-out: J = J_run + w_term |p - goal|^2 + w_obs max(0, d_safe - d_min)^2 + w_coll [d_min < 0]
+      A.cost_run[i] = cost;
+      float ex = x[0] - P.cost_goal[0], ey = x[1] - P.cost_goal[1], ez = x[2] - P.cost_goal[2];
+      float J = fmaf(P.cost_w_term, fmaf(ez, ez, fmaf(ey, ey, ex * ex)), cost);
+      float gap = P.cost_d_safe - d_min;
+      if (gap > 0.0f) J = fmaf(P.cost_w_obs * gap, gap, J);
+      if (d_min < 0.0f) J += P.cost_w_coll;
+      A.cost_drone[i] = J;
     }
     if (i == 0) {
       if (my_att) atomicAdd(&A.counters->att_ticks, my_att);

@@ -12,6 +12,8 @@ struct EntryAB { int integ, iface, opt; const char *name; void (*fn)(const StepA
 static const EntryAB kTableAB[] = {
   // configs[2]: planning rollouts, in-kernel nominal + noise commands, obstacle distance, jittered (a,b,c)
   CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_OBST | OPT_NOISE),
+  // sampling-based planner: the same rollout + correlated noise + rollout cost
+  CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_OBST | OPT_NOISE | OPT_COST),
   // variant 3B: the same with a command buffer
   CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_OBST),
   // configs[3]: swarm, position interface, per-world mass

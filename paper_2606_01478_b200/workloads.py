@@ -194,7 +194,24 @@ def cfg5e(seed=REPORT_SEED, M=65536, n_steps=1000) -> Workload:
     return cfg5(seed, M, n_steps, integrator=EULER)
 
 
-REGISTRY = {"cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
+def mppi(seed=REPORT_SEED, n_ctrl=5, worlds_per_ctrl=100_000, horizon=25, cmd_hold=10, n_elite=None) -> Workload:
+    """The sampling-based planner of PAPER.md:L465-L471 around the configs[2] rollout: 5 controllers x 100 000 rollouts
+    (500 k), 25 knots at 50 Hz (10 physics steps of the 500 Hz abstracted model per knot), top 1 % elites, AR(1) noise.
+    The paper's own parameters are in a codebase that is not available; the values here are this build's choice."""
+    p = _cfg3_params(seed)
+    p.update(cmd_source=CMD_NOMINAL_PLUS_NOISE, noise_beta=0.7, n_ctrl=n_ctrl, worlds_per_ctrl=worlds_per_ctrl,
+             cost_on=1, cost_goal=[3.5, 0.0, 1.0], cost_w_pos=1.0, cost_w_vel=0.05, cost_w_term=10.0,
+             cost_w_obs=200.0, cost_d_safe=0.15, cost_w_coll=1000.0)
+    nominal = np.zeros((n_ctrl, horizon, 4), dtype=np.float32)
+    nominal[..., 3] = MASS * G
+    if n_elite is None:
+        n_elite = max(1, worlds_per_ctrl // 100)
+    return Workload("mppi", n_ctrl * worlds_per_ctrl, 1, MODEL_AB, p, seed, horizon * cmd_hold, cmd_hold, 0, nominal,
+                    broadcast_state=_cfg3_start(),
+                    notes=dict(horizon=horizon, n_elite=n_elite, lam=0.5, shift=1, n_ctrl=n_ctrl))
+
+
+REGISTRY = {"mppi": mppi, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
 
 
 def make(name: str, **kw) -> Workload:
