@@ -29,8 +29,8 @@ DEFAULT_WORKLOAD = "cfg3"
 # Algorithmic FP32 operations per drone-step: every add / sub / mul / div / sqrt /
 # trig / log / min / max / clip of the float64 oracle's formulas counts 1 (an FMA is 2); Philox integer work is not
 # counted.  Controller ticks are amortised over their period.
-ALGO_FLOPS = {"cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
-BOUND = {"cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
+ALGO_FLOPS = {"mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
+BOUND = {"mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
 SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of the rollout kernel, one launch, from the `ncu --set full` captures
 # summarised in profiles/r1_<workload>_rollout.md (static: ncu never runs inside bench.py)
@@ -60,7 +60,8 @@ def algo_bytes_per_launch(wl) -> int:
     ctrl_planes = {0: 3 + 4 + 4, 1: 4 + (3 if wl.params.get("iface") == 3 else 0)}[wl.model]
     resident = 2 * (wl.D + ctrl_planes) * 4 * MN + (2 * 8 * 4 * MN if wl.params.get("n_obstacles") else 0)
     wparam = (14 if wl.model == 0 else 11) * 4 * wl.M
-    return cmd + rec + resident + wparam
+    plan = (4 + 2 + 1) * 4 * MN if wl.params.get("cost_on") else 0       # eps, cost (running, total), min distance out
+    return cmd + rec + resident + wparam + plan
 
 
 class ClockSampler:
@@ -138,6 +139,11 @@ class Runner:
         # broadcast resets are folded into the rollout launch and the N = 1 minimum distance comes from its epilogue
         self.launches_per_step = 1 + (1 if (self.obst and wl.N > 1) else 0)
         self.kernel, self.grid, self.block = self.sim.describe_launch()
+        self.planner = name == "mppi"
+        if self.planner:      # planning iteration: broadcast reset + fused rollout + update (2 kernels per step)
+            n = wl.notes
+            self.mpar = self.sim.mppi_params(n["horizon"], wl.cmd_hold, n["n_elite"], n["lam"], n["shift"])
+            self.launches_per_step = 2
         # host side buffers for the end-to-end path (pinned)
         self.e2e_ok = e2e and self.cmds_host is not None
         if self.e2e_ok:
@@ -146,11 +152,20 @@ class Runner:
             self.state_pin = torch.empty((wl.D, wl.MN), dtype=torch.float32, pin_memory=True)
             self.md_pin = torch.empty(wl.M, dtype=torch.float32, pin_memory=True) if self.obst else None
             self.bstate_pin = None if self.bstate is None else self.bstate.cpu().pin_memory()
+            if self.planner:
+                self.plan_pin = torch.empty((wl.notes["horizon"], 4), dtype=torch.float32, pin_memory=True)
+                self.info_pin = torch.empty(4 * wl.notes["n_ctrl"] + 4, dtype=torch.float32, pin_memory=True)
             self.h2d = self.cmds_pin.numel() * 4 + (0 if self.bstate is None else self.bstate.numel() * 4)
             self.d2h = (self.rec_pin.numel() * 4 if n_rec else self.state_pin.numel() * 4) + (wl.M * 4 if self.obst else 0)
+            if self.planner:
+                self.h2d = self.bstate.numel() * 4
+                self.d2h = self.plan_pin.numel() * 4 + self.info_pin.numel() * 4
 
     def step(self):
         wl, sim = self.wl, self.sim
+        if self.planner:
+            sim.mppi_iterate(self.mpar, self.bstate, self.cmds)
+            return
         if self.bstate is not None:
             sim.set_state(self.bstate, broadcast=True)
         sim.step(self.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every, record=self.record)
@@ -159,12 +174,17 @@ class Runner:
 
     def rollout_only(self):
         wl = self.wl
+        if self.bstate is not None:
+            self.sim.set_state(self.bstate, broadcast=True)      # lazy: folded into the rollout launch
         self.sim.step(self.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every, record=self.record)
 
     def step_e2e(self):
         """The same step through the C ABI with HOST buffers: H2D of this step's inputs and D2H of its results
         (records, or final state + min distance when nothing is recorded) inside the call."""
         wl, sim = self.wl, self.sim
+        if self.planner:      # measured state in (52 B), plan + controller scores out; the nominal stays on the device
+            sim.mppi_iterate_host(self.mpar, self.bstate_pin, self.cmds, self.plan_pin, self.info_pin)
+            return
         if self.bstate_pin is not None:
             self.bstate.copy_(self.bstate_pin, non_blocking=True)
             sim.set_state(self.bstate, broadcast=True)
@@ -259,6 +279,8 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
     from paper_2606_01478_b200 import workloads as W
     if threads:
         cfo.set_num_threads(threads)
+    if name == "mppi":
+        return oracle_sample_mppi(target_seconds)
     small = dict(cfg1=dict(M=1, n_steps=1000), cfg2=dict(M=64, n_steps=200), cfg3=dict(M=512, n_steps=100),
                  cfg3b=dict(M=512, n_steps=100), cfg4=dict(M=1, N=512, n_steps=100), cfg5=dict(M=64, n_steps=200),
                  cfg5e=dict(M=64, n_steps=200))[name]
@@ -283,6 +305,32 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
     rate, wl = run(kw)
     sample = f"{wl.M} worlds x {wl.N} drones x {wl.n_steps} steps of {name} (same recipe, reduced M)"
     return rate, cfo.num_threads(), sample, wl
+
+
+def oracle_sample_mppi(target_seconds):
+    """One planning iteration of the oracle (C rollout + numpy update) at a reduced number of rollouts per controller."""
+    import numpy as np
+    from oracle import cfo, mppi as omppi
+    from paper_2606_01478_b200 import workloads as W
+
+    def run(wpc):
+        wl = W.mppi(worlds_per_ctrl=wpc)
+        p, n = wl.params, wl.notes
+        sim = cfo.OracleSim(wl.M, 1, wl.model, p)
+        sim.reset(wl.seed)
+        t0 = time.perf_counter()
+        sim.set_state(wl.broadcast_state, broadcast=True)
+        sim.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold)
+        omppi.update(sim.cost().astype(np.float32), wl.cmds, seed=wl.seed, world_offset=0, worlds_per_ctrl=wpc, s_start=0,
+                     cmd_hold=wl.cmd_hold, sigma=p["noise_sigma"], beta=p["noise_beta"], lo=p["cmd_lo"], hi=p["cmd_hi"],
+                     n_elite=n["n_elite"], lam=n["lam"], shift=n["shift"])
+        return wl.drone_steps / (time.perf_counter() - t0), wl
+
+    rate, wl = run(200)
+    wpc = int(min(100_000, max(200, rate * target_seconds / (5 * wl.n_steps))))
+    rate, wl = run(wpc)
+    return rate, cfo.num_threads(), (f"{wl.M} rollouts ({wpc} per controller) x {wl.n_steps} steps of mppi + the update "
+                                     f"(same recipe, fewer rollouts)"), wl
 
 
 def main():
@@ -378,7 +426,7 @@ def main():
     main_res = measure(name, args.steps, args.warmup, not args.no_e2e)
     others = {}
     if not args.no_others and world == 1:
-        for nm in ("cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"):
+        for nm in ("mppi", "cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"):
             if nm == name:
                 continue
             r = measure(nm, 5, 3, False)

@@ -229,6 +229,13 @@ int cf_mppi_update(cf_sim *sim, const cf_mppi_params *mp, void *nominal_dev, voi
 int cf_mppi_iterate(cf_sim *sim, const cf_mppi_params *mp, const float *x0_dev, void *nominal_dev, void *plan_dev,
                     void *info_dev, int32_t *elite_idx_dev, void *scratch_dev, size_t scratch_bytes);
 
+/* The same iteration driven from HOST buffers (the end-to-end path of a 50 Hz control loop): x0_host [D] is copied
+ * host->device, the iteration runs, plan_host [H] float4 and info_host (CF_MPPI_INFO_WORDS words) are copied
+ * device->host and the stream is synchronised.  plan_dev / info_dev are device staging as in cf_mppi_iterate. */
+int cf_mppi_iterate_host(cf_sim *sim, const cf_mppi_params *mp, const float *x0_host, void *nominal_dev,
+                         void *plan_host, void *info_host, void *plan_dev, void *info_dev, void *scratch_dev,
+                         size_t scratch_bytes);
+
 const char *cf_last_error(void);
 /* Host-side Philox4x32-10 of this library, for the bit-exact check against the oracle's (C9). */
 int cf_debug_philox(uint64_t seed, const uint32_t ctr[4], uint32_t out[4]);

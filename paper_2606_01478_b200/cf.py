@@ -101,6 +101,7 @@ def lib():
         "cf_mppi_scratch_bytes": (sz, [vp, C.POINTER(MppiParams)]),
         "cf_mppi_update": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, sz]),
         "cf_mppi_iterate": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, sz]),
+        "cf_mppi_iterate_host": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, vp, sz]),
         "cf_last_error": (C.c_char_p, []),
         "cf_debug_philox": (C.c_int, [C.c_uint64, C.POINTER(C.c_uint32 * 4), C.POINTER(C.c_uint32 * 4)]),
         "cf_debug_philox_dev": (C.c_int, [vp, C.c_uint64, vp, C.c_int, vp, vp, vp]),
@@ -116,7 +117,7 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_set_stream", "cf_reset", "cf_set_state", "cf_set_full", "cf_step", "cf_staging_bytes", "cf_step_host",
            "cf_get_state", "cf_get_state_host", "cf_get_aux", "cf_get_aux_host", "cf_step_counter", "cf_sync_counters",
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
-           "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate"]
+           "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host"]
 
 
 def _check(rc: int):
@@ -377,6 +378,14 @@ class Sim:
         _check(lib().cf_mppi_iterate(self._h, C.byref(mp), _dptr(x0), _dptr(nominal), _dptr(self._mppi_plan),
                                      _dptr(self._mppi_info), el, sp, need))
         return self._mppi_result(nominal, want_elites)
+
+    def mppi_iterate_host(self, mp: MppiParams, x0_host, nominal, plan_host, info_host):
+        """End-to-end iteration: x0_host [D], plan_host [H][4], info_host [4 n_ctrl + 4] are (pinned) CPU tensors."""
+        sp, need, _ = self._mppi_buffers(mp, False)
+        _check(lib().cf_mppi_iterate_host(self._h, C.byref(mp), C.c_void_p(x0_host.data_ptr()), _dptr(nominal),
+                                          C.c_void_p(plan_host.data_ptr()), C.c_void_p(info_host.data_ptr()),
+                                          _dptr(self._mppi_plan), _dptr(self._mppi_info), sp, need))
+        return plan_host, info_host
 
     def rec_table(self):
         return self._aux(AUX_REC_TABLE, (REC_TABLE_CAP,), _torch().int32).cpu().numpy().view(np.uint32)

@@ -323,3 +323,24 @@ extern "C" int cf_mppi_iterate(cf_sim *sim, const cf_mppi_params *mp, const floa
   if (rc != CF_OK) return rc;
   return cf_mppi_update(sim, mp, nominal_dev, plan_dev, info_dev, elite_idx_dev, scratch_dev, scratch_bytes);
 }
+
+extern "C" int cf_mppi_iterate_host(cf_sim *sim, const cf_mppi_params *mp, const float *x0_host, void *nominal_dev,
+                                    void *plan_host, void *info_host, void *plan_dev, void *info_dev,
+                                    void *scratch_dev, size_t scratch_bytes) {
+  int rc = check(sim, mp);
+  if (rc != CF_OK) return rc;
+  if (!x0_host || !plan_host || !info_host || !plan_dev || !info_dev) return fail(CF_E_ARG, "NULL argument");
+  // the broadcast start state is parked in the workspace and consumed by the rollout launch (lazy cf_set_state)
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_mppi_iterate_host needs a prior cf_reset (world parameters)");
+  CF_CUDA(cudaMemcpyAsync(sim->bcast_buf, x0_host, sizeof(float) * sim->D, cudaMemcpyHostToDevice, sim->stream));
+  sim->pending_bcast = true; sim->rearmed = true; sim->md_valid = false; sim->cost_valid = false;   // = cf_set_state(broadcast)
+  rc = cf_step(sim, nominal_dev, mp->horizon, mp->cmd_hold, mp->horizon * mp->cmd_hold, 0, nullptr, 0);
+  if (rc != CF_OK) return rc;
+  rc = cf_mppi_update(sim, mp, nominal_dev, plan_dev, info_dev, nullptr, scratch_dev, scratch_bytes);
+  if (rc != CF_OK) return rc;
+  CF_CUDA(cudaMemcpyAsync(plan_host, plan_dev, sizeof(float4) * mp->horizon, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaMemcpyAsync(info_host, info_dev, sizeof(float) * CF_MPPI_INFO_WORDS(sim->p.n_ctrl), cudaMemcpyDeviceToHost,
+                          sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  return CF_OK;
+}
