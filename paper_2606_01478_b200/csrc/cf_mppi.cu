@@ -3,24 +3,33 @@
 // the elites' command sequences (regenerated from the Philox counters -- the 500 k x H sampled commands are never
 // stored), controller score; then the best controller's plan and the warm-started nominal sequences.
 //
-// One CTA per controller does everything for its K_c rollouts (K_c = 100 000 costs = 400 kB, L2 resident):
+// One thread-block CLUSTER of 8 CTAs per controller does everything for its K_c rollouts (K_c = 100 000 costs = 400 kB,
+// L2 resident); CTA r of the cluster owns the contiguous slice [r S, (r+1) S) of the costs.  The CTAs exchange
+// histograms, counts and partial sums through distributed shared memory (cluster.map_shared_rank) between
+// cluster barriers -- no global atomics, no extra launches:
 //   1. radix select (4 passes x 8 bits, MSB first) of the n_elite-th smallest cost key -> threshold key T and the number
-//      r of keys equal to T that are admitted (ties go to the lowest world index, R28);
-//   2. ordered compaction of the elites (one block scan over per-thread segment counts) -> ascending index list;
-//   3. one thread per elite: weight, regenerate eps / commands for the H knots with the rollout kernel's own
-//      arithmetic (bit-identical commands), write w * u rows to scratch;
-//   4. fixed-order two-stage column sums (deterministic), mean, score;
-//   5. the last CTA to finish picks the best controller, writes the plan and shifts the nominal sequences.
+//      r of keys equal to T that are admitted (ties go to the lowest world index, R28); per-CTA shared-memory histograms
+//      (warp-aggregated atomics, double-buffered so one cluster barrier per pass suffices), summed by every CTA;
+//   2. ordered compaction of the elites: per-CTA counts exchanged over DSMEM + one block scan over per-thread segment
+//      counts -> ascending index list;
+//   3. one thread per elite (spread over the 8 CTAs): weight, regenerate eps / commands for the H knots with the
+//      rollout kernel's own arithmetic (bit-identical commands), write w * u rows to scratch;
+//   4. fixed-order column sums (per CTA, then over the 8 CTAs in rank order: deterministic), mean, score;
+//   5. the last cluster to finish picks the best controller, writes the plan and shifts the nominal sequences.
 #include "cf_internal.h"
 
 #include <cmath>
+#include <cooperative_groups.h>
+
+namespace cg = cooperative_groups;
 
 using namespace cf;
 
 namespace {
 
 constexpr int kThreads = 1024;
-constexpr int kWarps = kThreads / 32;
+constexpr int kCluster = 8;      // CTAs per controller (portable cluster size)
+constexpr int kRegKeys = 16;     // cost keys a thread keeps in registers
 
 struct MppiArgs {
   const float *cost;        // [n_ctrl][K_c] rollout costs (world order)
@@ -71,45 +80,74 @@ __device__ __forceinline__ unsigned block_exscan(unsigned v, unsigned *warp_sums
   return ex;
 }
 
-__global__ void __launch_bounds__(kThreads, 1)
+// what a CTA publishes to the other CTAs of its cluster (read through DSMEM)
+struct Shared {
+  unsigned hist[2][256];      // radix-pass histogram of this CTA's slice, double-buffered over passes
+  unsigned n_less, n_eq;      // keys below / equal to the threshold in this CTA's slice
+  uint32_t kmin;              // smallest key of the slice
+  float colsum[kThreads];     // this CTA's partial column sums (first 4 (H + 1) entries)
+};
+
+__global__ void __cluster_dims__(kCluster, 1, 1) __launch_bounds__(kThreads, 1)
 mppi_update_kernel(const __grid_constant__ MppiArgs A, const __grid_constant__ DevParams P) {
-  __shared__ unsigned hist[kWarps][256];
+  __shared__ Shared sh;
+  __shared__ unsigned tot[256];
   __shared__ unsigned warp_sums[33];
   __shared__ unsigned sh_prefix, sh_rank;
   __shared__ float sh_part[kThreads];
   __shared__ float sh_sum[2];
-  const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  __shared__ bool is_last;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int c = blockIdx.x / kCluster, rk = (int)cluster.block_rank();
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const long long K = A.K_c;
   const float *cost = A.cost + (long long)c * K;
+  // slice of this CTA: S keys (a multiple of kThreads so that thread segments tile it exactly)
+  const long long S = ((K + kCluster - 1) / kCluster + kThreads - 1) / kThreads * kThreads;
+  const long long s_lo = (long long)rk * S < K ? (long long)rk * S : K;
+  const long long s_hi = s_lo + S < K ? s_lo + S : K;
+
+  // thread t owns the contiguous segment [lo, hi) of the slice.  Its first kRegKeys keys are read ONCE (all loads in
+  // flight together) and stay in registers for the four radix passes and the compaction; a longer segment (more than
+  // kCluster * kThreads * kRegKeys = 131 072 rollouts per controller) re-reads its tail from L2 in every pass.
+  const long long seg = S / kThreads;
+  const long long lo = s_lo + (long long)tid * seg < s_hi ? s_lo + (long long)tid * seg : s_hi;
+  const long long hi = lo + seg < s_hi ? lo + seg : s_hi;
+  const int n_reg = (int)(hi - lo < kRegKeys ? hi - lo : kRegKeys);
+  uint32_t keys[kRegKeys];
+#pragma unroll
+  for (int j = 0; j < kRegKeys; ++j) keys[j] = j < n_reg ? cost_key(__ldg(cost + lo + j)) : 0xFFFFFFFFu;
 
   // ---- 1. radix select of the n_elite-th smallest key ---------------------------------------------------------
   uint32_t prefix = 0, mask = 0;
   unsigned rank = (unsigned)A.n_elite;        // 1-based rank inside the current candidate set
   for (int pass = 0; pass < 4; ++pass) {
-    const int sh = 24 - 8 * pass;
-    for (int b = lane; b < 256; b += 32) hist[wid][b] = 0;
+    const int shf = 24 - 8 * pass, buf = pass & 1;
+    if (tid < 256) sh.hist[buf][tid] = 0;     // last read by the other CTAs two passes ago (a cluster barrier since)
     __syncthreads();
-    for (long long base = 0; base < K; base += kThreads) {
-      long long i = base + tid;
-      unsigned bin = 256;
-      if (i < K) {
-        uint32_t k = cost_key(__ldg(cost + i));
-        if ((k & mask) == prefix) bin = (k >> sh) & 255u;
-      }
+    auto count = [&](bool valid, uint32_t k) {
+      unsigned bin = (valid && (k & mask) == prefix) ? (k >> shf) & 255u : 256u;
       unsigned peers = __match_any_sync(0xffffffffu, bin);            // warp-aggregated shared-memory atomics
-      if (bin < 256 && lane == __ffs(peers) - 1) atomicAdd(&hist[wid][bin], (unsigned)__popc(peers));
+      if (bin < 256 && lane == __ffs(peers) - 1) atomicAdd(&sh.hist[buf][bin], (unsigned)__popc(peers));
+    };
+#pragma unroll
+    for (int j = 0; j < kRegKeys; ++j) count(j < n_reg, keys[j]);
+    for (long long j = kRegKeys; j < seg; ++j) {                      // (uniform trip count: warp-collective inside)
+      bool valid = lo + j < hi;
+      count(valid, valid ? cost_key(__ldg(cost + lo + j)) : 0u);
     }
-    __syncthreads();
-    if (tid < 256) {                                                  // fold the per-warp histograms
+    cluster.sync();                                                   // every CTA's histogram is complete
+    if (tid < 256) {                                                  // every CTA sums all 8 (same result everywhere)
       unsigned s = 0;
-      for (int w = 0; w < kWarps; ++w) s += hist[w][tid];
-      hist[0][tid] = s;
+#pragma unroll
+      for (int r = 0; r < kCluster; ++r) s += cluster.map_shared_rank(&sh, r)->hist[buf][tid];
+      tot[tid] = s;
     }
     __syncthreads();
     if (wid == 0) {                                                   // find the bucket that holds the rank
       unsigned cnt[8], sum = 0;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) { cnt[j] = hist[0][lane * 8 + j]; sum += cnt[j]; }
+      for (int j = 0; j < 8; ++j) { cnt[j] = tot[lane * 8 + j]; sum += cnt[j]; }
       unsigned inc = sum;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) { unsigned t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
@@ -118,44 +156,57 @@ mppi_update_kernel(const __grid_constant__ MppiArgs A, const __grid_constant__ D
         unsigned r = rank - below;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          if (r != 0 && r <= cnt[j]) { sh_prefix = prefix | ((uint32_t)(lane * 8 + j) << sh); sh_rank = r; r = 0; }
+          if (r != 0 && r <= cnt[j]) { sh_prefix = prefix | ((uint32_t)(lane * 8 + j) << shf); sh_rank = r; r = 0; }
           else if (r != 0) r -= cnt[j];
         }
       }
     }
     __syncthreads();
-    prefix = sh_prefix; rank = sh_rank; mask |= 0xFFu << sh;
+    prefix = sh_prefix; rank = sh_rank; mask |= 0xFFu << shf;
     __syncthreads();
   }
   const uint32_t T = prefix;                  // threshold key; `rank` of the keys equal to T are admitted (lowest indices)
 
-  // ---- 2. ordered compaction: thread t owns the contiguous segment [t seg, (t+1) seg) ------------------------------
-  const long long seg = (K + kThreads - 1) / kThreads;
-  const long long lo = (long long)tid * seg, hi = lo + seg < K ? lo + seg : K;
+  // ---- 2. ordered compaction: thread t owns the contiguous segment [s_lo + t seg, s_lo + (t+1) seg) ---------------
   unsigned n_less = 0, n_eq = 0;
   uint32_t kmin = 0xFFFFFFFFu;
-  for (long long i = lo; i < hi; ++i) {
+#pragma unroll
+  for (int j = 0; j < kRegKeys; ++j) {
+    if (j < n_reg) { uint32_t k = keys[j]; n_less += k < T; n_eq += k == T; kmin = k < kmin ? k : kmin; }
+  }
+  for (long long i = lo + kRegKeys; i < hi; ++i) {
     uint32_t k = cost_key(__ldg(cost + i));
     n_less += k < T; n_eq += k == T; kmin = k < kmin ? k : kmin;
   }
   unsigned tot_less, tot_eq;
   unsigned ex_less = block_exscan(n_less, warp_sums, &tot_less);
   unsigned ex_eq = block_exscan(n_eq, warp_sums, &tot_eq);
-  // block minimum of the keys = J_min of the elites (the best rollout is always an elite)
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) { uint32_t t = __shfl_xor_sync(0xffffffffu, kmin, o); kmin = t < kmin ? t : kmin; }
   if (lane == 0) warp_sums[wid] = kmin;
   __syncthreads();
-  kmin = warp_sums[lane];
+  if (wid == 0) {
+    kmin = warp_sums[lane];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) { uint32_t t = __shfl_xor_sync(0xffffffffu, kmin, o); kmin = t < kmin ? t : kmin; }
-  __syncthreads();
-  const float J_min = key_cost(kmin);
+    for (int o = 16; o > 0; o >>= 1) { uint32_t t = __shfl_xor_sync(0xffffffffu, kmin, o); kmin = t < kmin ? t : kmin; }
+    if (lane == 0) { sh.n_less = tot_less; sh.n_eq = tot_eq; sh.kmin = kmin; }
+  }
+  cluster.sync();                                                     // counts and minima of all slices are published
+  unsigned less_before = 0, eq_before = 0;
+  uint32_t kmin_all = 0xFFFFFFFFu;
+#pragma unroll
+  for (int r = 0; r < kCluster; ++r) {
+    const Shared *o = cluster.map_shared_rank(&sh, r);
+    unsigned nl = o->n_less, ne = o->n_eq; uint32_t km = o->kmin;
+    if (r < rk) { less_before += nl; eq_before += ne; }
+    kmin_all = km < kmin_all ? km : kmin_all;
+  }
+  const float J_min = key_cost(kmin_all);     // the best rollout is always an elite
   int32_t *eidx = A.elite_idx + (long long)c * A.n_elite;
   {
-    unsigned eq_seen = ex_eq, pos = ex_less + (ex_eq < rank ? ex_eq : rank);
-    for (long long i = lo; i < hi; ++i) {
-      uint32_t k = cost_key(__ldg(cost + i));
+    unsigned eq_seen = eq_before + ex_eq;
+    unsigned pos = less_before + ex_less + (eq_seen < rank ? eq_seen : rank);
+    auto admit = [&](long long i, uint32_t k) {
       bool take = k < T || (k == T && eq_seen < rank);
       eq_seen += k == T;
       if (take) {
@@ -163,17 +214,22 @@ mppi_update_kernel(const __grid_constant__ MppiArgs A, const __grid_constant__ D
         if (A.elite_out) A.elite_out[(long long)c * A.n_elite + pos] = (int32_t)i;
         ++pos;
       }
-    }
+    };
+#pragma unroll
+    for (int j = 0; j < kRegKeys; ++j) if (j < n_reg) admit(lo + j, keys[j]);
+    for (long long i = lo + kRegKeys; i < hi; ++i) admit(i, cost_key(__ldg(cost + i)));
   }
-  __threadfence_block();
-  __syncthreads();
+  __threadfence();
+  cluster.sync();                                                     // the elite list (written by all 8 CTAs) is complete
 
   // ---- 3. one thread per elite: weight, regenerated commands (R25, R26 with the rollout kernel's arithmetic) -----
   const int H = A.H, RW = H + 1;
   float4 *rows = A.rows + (long long)c * A.n_elite * RW;
   const float4 *nom = A.nominal + (long long)c * H;
-  for (int e = tid; e < A.n_elite; e += kThreads) {
-    const int k = eidx[e];
+  const int E = (A.n_elite + kCluster - 1) / kCluster;                // elites per CTA
+  const int e_lo = rk * E < A.n_elite ? rk * E : A.n_elite, e_hi = e_lo + E < A.n_elite ? e_lo + E : A.n_elite;
+  for (int e = e_lo + tid; e < e_hi; e += kThreads) {
+    const int k = __ldcg(eidx + e);
     const float J = __ldg(cost + k);
     const float w = expf(-(J - J_min) * A.inv_lambda);                // R29
     const uint32_t wg = (uint32_t)(A.world0 + (long long)c * K + k);
@@ -199,33 +255,45 @@ mppi_update_kernel(const __grid_constant__ MppiArgs A, const __grid_constant__ D
   __threadfence_block();
   __syncthreads();
 
-  // ---- 4. deterministic column sums: column j of 4 RW, partial p sums elites p, p + NP, ... in order ---------------
+  // ---- 4. deterministic column sums: per CTA (column j of 4 RW, partial p sums its elites p, p + NP, ... in order),
+  //         then over the 8 CTAs in rank order by the cluster's CTA 0 ---------------------------------------------------
   const int ncol = 4 * RW, NP = kThreads / ncol;                     // host guarantees ncol <= kThreads
   const float *rowsf = reinterpret_cast<const float *>(rows);
   if (tid < NP * ncol) {
     const int j = tid % ncol, p = tid / ncol;
     float s = 0.f;
-    for (int e = p; e < A.n_elite; e += NP) s += rowsf[(long long)e * ncol + j];
+#pragma unroll 4
+    for (int e = e_lo + p; e < e_hi; e += NP) s += __ldcg(rowsf + (long long)e * ncol + j);
     sh_part[tid] = s;
   }
   __syncthreads();
-  float colsum = 0.f;
   if (tid < ncol) {
-    for (int p = 0; p < NP; ++p) colsum += sh_part[p * ncol + tid];
-    if (tid == 4 * H) sh_sum[0] = colsum;                             // sum of weights
-    if (tid == 4 * H + 1) sh_sum[1] = colsum;                         // sum of w J
+    float s = 0.f;
+    for (int p = 0; p < NP; ++p) s += sh_part[p * ncol + tid];
+    sh.colsum[tid] = s;
   }
-  __syncthreads();
-  if (tid < 4 * H) reinterpret_cast<float *>(A.mean + (long long)c * H)[tid] = colsum / sh_sum[0];      // R30
-  if (tid == 0) {
-    A.info[4 * c + 0] = sh_sum[1] / sh_sum[0];                        // R31 score
-    A.info[4 * c + 1] = J_min;
-    A.info[4 * c + 2] = sh_sum[0];
-    A.info[4 * c + 3] = key_cost(T);
+  cluster.sync();                                                     // all 8 partial column sums are published
+  if (rk == 0) {
+    float colsum = 0.f;
+    if (tid < ncol) {
+#pragma unroll
+      for (int r = 0; r < kCluster; ++r) colsum += cluster.map_shared_rank(&sh, r)->colsum[tid];
+      if (tid == 4 * H) sh_sum[0] = colsum;                           // sum of weights
+      if (tid == 4 * H + 1) sh_sum[1] = colsum;                       // sum of w J
+    }
+    __syncthreads();
+    if (tid < 4 * H) reinterpret_cast<float *>(A.mean + (long long)c * H)[tid] = colsum / sh_sum[0];      // R30
+    if (tid == 0) {
+      A.info[4 * c + 0] = sh_sum[1] / sh_sum[0];                      // R31 score
+      A.info[4 * c + 1] = J_min;
+      A.info[4 * c + 2] = sh_sum[0];
+      A.info[4 * c + 3] = key_cost(T);
+    }
   }
+  cluster.sync();                             // nobody leaves while CTA 0 may still read its shared memory
+  if (rk != 0) return;
 
-  // ---- 5. last CTA: best controller, plan, warm start (R31, R32) ------------------------------------------------
-  __shared__ bool is_last;
+  // ---- 5. last cluster: best controller, plan, warm start (R31, R32) ---------------------------------------------
   __threadfence();
   __syncthreads();
   if (tid == 0) is_last = atomicAdd(A.done, 1u) == (unsigned)A.n_ctrl - 1;
@@ -307,7 +375,7 @@ extern "C" int cf_mppi_update(cf_sim *sim, const cf_mppi_params *mp, void *nomin
   const uint32_t lo = (uint32_t)(sim->seed & 0xFFFFFFFFu), hi = (uint32_t)(sim->seed >> 32);
   for (int r = 0; r < 10; ++r) { A.rk[2 * r] = lo + (uint32_t)r * 0x9E3779B9u; A.rk[2 * r + 1] = hi + (uint32_t)r * 0xBB67AE85u; }
   CF_CUDA(cudaMemsetAsync(A.done, 0, sizeof(unsigned int), sim->stream));
-  mppi_update_kernel<<<A.n_ctrl, kThreads, 0, sim->stream>>>(A, sim->dp);
+  mppi_update_kernel<<<A.n_ctrl * kCluster, kThreads, 0, sim->stream>>>(A, sim->dp);     // one 8-CTA cluster per controller
   CF_CUDA(cudaGetLastError());
   return CF_OK;
 }

@@ -144,6 +144,20 @@ def test_r28_elite_selection_is_bit_exact_on_the_gpu_costs(cf, W, mp, n_elite):
     assert np.array_equal(info[3:12:4], thr) and np.array_equal(info[1:12:4], cost.reshape(3, -1).min(1))
 
 
+def test_r28_selection_with_more_keys_than_the_register_resident_path_holds(cf, W, mp):
+    """150 001 rollouts per controller: each thread's segment is longer than the 16 register-resident keys."""
+    import torch
+    wl = W.mppi(seed=12, n_ctrl=2, worlds_per_ctrl=150_001, horizon=3, cmd_hold=2, n_elite=1500)
+    g = cf.Sim(wl.M, 1, wl.model, wl.params)
+    g.reset(wl.seed)
+    nom = torch.as_tensor(random_nominal(wl, 4), device="cuda")
+    _rollout(g, wl, nom.clone())
+    cost = g.cost().cpu().numpy()
+    for n_elite in (1500, 4096):
+        out = g.mppi_update(g.mppi_params(3, 2, n_elite, 0.5), nom.clone(), want_elites=True)
+        assert np.array_equal(out["elites"].cpu().numpy(), mp.elite_select(cost, 2, n_elite))
+
+
 def test_r28_ties_nan_and_infinities_follow_the_bit_pattern_rule(cf, W, mp):
     import torch
     wl = W.mppi(seed=6, n_ctrl=2, worlds_per_ctrl=1500, horizon=3, cmd_hold=2, n_elite=40)
