@@ -681,7 +681,6 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // chunk c is row c/8 (component), columns 4(c%8)..+3 (drones), so successive chunks of a lane are 4 rows apart
     float *rec_tile = wp_s + (threadIdx.x >> 5) * (D * 32);
     float *rec_ptr = A.record + (size_t)(lane >> 3) * MN + (i - lane) + 4 * (lane & 7);
-    int cmd_cd = 0;
     const bool noise = (OPT & OPT_NOISE) != 0 && P.use_noise;   // compiled in AND requested
     // next command to prefetch; in noise mode the nominal sequence of this world's controller (R26)
     const float4 *cp = noise ? A.cmds + (A.worlds_per_ctrl > 0 ? (long long)(wg / (uint32_t)A.worlds_per_ctrl) * A.n_cmds : 0)
@@ -690,11 +689,10 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     int cmds_left = (A.n_steps + A.cmd_hold - 1) / A.cmd_hold;  // commands this call consumes
     float4 next_cmd = __ldg(cp);
 
-    for (int t = 0; t < A.n_steps; ++t) {
-      // (1) command fetch (prefetched one segment ahead)
-      if (cmd_cd == 0) {
+    // (1) command fetch (prefetched one segment ahead)
+    auto fetch_command = [&]() {
+      {
         float4 c4 = next_cmd;
-        cmd_cd = A.cmd_hold;
         if (--cmds_left > 0) { cp += cstride; next_cmd = __ldg(cp); }
         float c[4] = { c4.x, c4.y, c4.z, c4.w };
         if (noise) {
@@ -724,7 +722,9 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           mixer<OPT>(P, c[3], c, rpm_cmd);
         }
       }
-      --cmd_cd;
+    };
+    // (2)-(8) of one physics step
+    auto physics_step = [&]() {
       // (2) position controller tick
       if (HAS_POS) {
         if (pos_phase == 0) {
@@ -815,6 +815,19 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           }
           ++rec_slot;
         }
+      }
+    };
+    // The call starts at a command boundary (C8), so a run of cmd_hold steps starts with ONE command fetch.  With held
+    // commands the loop is two-level and the inner loop carries no command logic (mppi rollout kernel 705 -> 691 us,
+    // cfg4 +3 %); with a fresh command every step (cmd_hold == 1, configs[2]) the flat loop is 2 % faster.
+    if (A.cmd_hold == 1) {
+      for (int t = 0; t < A.n_steps; ++t) { fetch_command(); physics_step(); }
+    } else {
+      for (int t = 0; t < A.n_steps;) {
+        fetch_command();
+        const int run = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;
+        t += run;
+        for (int k = 0; k < run; ++k) physics_step();
       }
     }
     // final store
