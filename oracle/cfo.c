@@ -505,9 +505,25 @@ int cfo_set_plan_state(cfo_sim *S, const double *eps, const double *cost_run) {
 /* C8: one cf_step call = n_steps physics steps, per drone, in this order:
  *  (1) command fetch  (2) position tick  (3) attitude tick + mixer  (4) disturbance draw
  *  (5) integrate      (6) s += 1         (7) obstacle minima        (8) record */
+static int step_impl(cfo_sim *S, const float *cmds, const double *cmds64, int n_cmds, int cmd_hold, int n_steps,
+                     int record_every, double *record, size_t record_len);
+
 int cfo_step(cfo_sim *S, const float *cmds, int n_cmds, int cmd_hold, int n_steps, int record_every,
              double *record, size_t record_len) {
-  if (!S || n_steps < 1 || cmd_hold < 1 || record_every < 0 || !cmds) return -1;
+  if (!cmds) return -1;
+  return step_impl(S, cmds, NULL, n_cmds, cmd_hold, n_steps, record_every, record, record_len);
+}
+
+/* The same step with float64 commands [K][MN][4] (CFO_CMD_BUFFER only): used by oracle/grad.py, whose finite
+ * differences perturb a command by less than float32 resolves. */
+int cfo_step_f64cmd(cfo_sim *S, const double *cmds64, int n_cmds, int cmd_hold, int n_steps) {
+  if (!S || !cmds64 || S->p.cmd_source != CFO_CMD_BUFFER) return -1;
+  return step_impl(S, NULL, cmds64, n_cmds, cmd_hold, n_steps, 0, NULL, 0);
+}
+
+static int step_impl(cfo_sim *S, const float *cmds, const double *cmds64, int n_cmds, int cmd_hold, int n_steps,
+                     int record_every, double *record, size_t record_len) {
+  if (!S || n_steps < 1 || cmd_hold < 1 || record_every < 0 || (!cmds && !cmds64)) return -1;
   if (!S->have_state) return -3;
   if ((int64_t)n_cmds * cmd_hold < n_steps) return -2;
   const cfo_params *p = &S->p;
@@ -544,7 +560,8 @@ int cfo_step(cfo_sim *S, const float *cmds, int n_cmds, int cmd_hold, int n_step
       if (t % cmd_hold == 0) {
         int k = t / cmd_hold;
         if (p->cmd_source == CFO_CMD_BUFFER) {
-          for (int j = 0; j < 4; ++j) cmd[j] = (double)cmds[((size_t)k * MN + i) * 4 + j];
+          for (int j = 0; j < 4; ++j)
+            cmd[j] = cmds64 ? cmds64[((size_t)k * MN + i) * 4 + j] : (double)cmds[((size_t)k * MN + i) * 4 + j];
         } else {   /* nominal + sigma .* z, clipped; NOISE stream indexed by the global step */
           uint32_t r[4]; double z[4];
           philox_at(S->seed, wg, n, s, STREAM_NOISE, r);

@@ -91,6 +91,7 @@ int  cfo_set_full(cfo_sim *s, const double *state, const double *ctrl, const dou
 int  cfo_set_plan_state(cfo_sim *s, const double *eps, const double *cost_run);
 int  cfo_step(cfo_sim *s, const float *cmds, int n_cmds, int cmd_hold, int n_steps, int record_every,
               double *record, size_t record_len /* doubles */);
+int  cfo_step_f64cmd(cfo_sim *s, const double *cmds64, int n_cmds, int cmd_hold, int n_steps);
 int  cfo_get_state(cfo_sim *s, double *out);
 int  cfo_get_aux(cfo_sim *s, int which, void *out);
 void cfo_philox(uint64_t seed, const uint32_t ctr[4], uint32_t out[4]);

@@ -81,6 +81,7 @@ def lib():
         L.cfo_set_full.argtypes = [vp, vp, vp, vp, vp, C.c_int64]
         L.cfo_set_plan_state.argtypes = [vp, vp, vp]
         L.cfo_step.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, C.c_size_t]
+        L.cfo_step_f64cmd.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int]
         L.cfo_get_state.argtypes = [vp, vp]
         L.cfo_get_aux.argtypes = [vp, C.c_int, vp]
         L.cfo_philox.argtypes = [C.c_uint64, C.POINTER(C.c_uint32 * 4), C.POINTER(C.c_uint32 * 4)]
@@ -195,6 +196,14 @@ class OracleSim:
         if check and rc != 0:
             raise RuntimeError(f"cfo_step: {rc}")
         return rec if check else (rc, rec)
+
+    def step_f64(self, cmds64, n_steps: int, cmd_hold: int = 1):
+        """cmds64: float64 [K][M*N][4], command-buffer source only (oracle/grad.py)."""
+        cm = np.ascontiguousarray(cmds64, dtype=np.float64)
+        assert cm.size % (4 * self.MN) == 0
+        rc = lib().cfo_step_f64cmd(self._h, _ptr(cm), cm.size // (4 * self.MN), cmd_hold, n_steps)
+        if rc != 0:
+            raise RuntimeError(f"cfo_step_f64cmd: {rc}")
 
     def get_state(self):
         out = np.empty((self.D, self.MN), dtype=np.float64)
