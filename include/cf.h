@@ -236,6 +236,24 @@ int cf_mppi_iterate_host(cf_sim *sim, const cf_mppi_params *mp, const float *x0_
                          void *plan_host, void *info_host, void *plan_dev, void *info_dev, void *scratch_dev,
                          size_t scratch_bytes);
 
+/* ---- Gradient of a goal distance w.r.t. the command sequence (Fig. 3D) -------------------------
+ * "Measuring throughput over ten simulation steps by differentiating a goal distance with respect to the control
+ *  inputs"; "differentiating through high-fidelity dynamics, the full onboard controller stack".
+ *   L_i = | p_i(after n_steps) - goal |   for every drone i, from the simulator's CURRENT state (which is not modified:
+ *   neither the planes nor the step counter), driven by cmds_dev [n_cmds][MN] float4 exactly as cf_step would be;
+ *   grad_dev [n_cmds][MN] float4 receives dL_i / d cmds[k][i][0..3]  (commands beyond the last used one: 0);
+ *   loss_dev [MN] receives L_i.
+ * One hand-written reverse-mode kernel: forward sweep parking each step's state in scratch_dev
+ * (cf_grad_scratch_bytes = n_steps * HD * MN floats, HD = 24 first-principles / 13 abstracted, 16-byte aligned), backward
+ * sweep through normalisation, RK4 / Euler, Eqs. (1)-(4), (6) or (7)-(10), mixer and attitude controller.  Where a
+ * clip of the method is active (rotor thrust / speed limits, controller integral, rotor-interface command limits) the
+ * derivative is taken as 0 (reading R33); the controller tick schedule follows the global step counter.
+ * Supported: CF_CMD_BUFFER; rotor and attitude interface (first-principles), attitude (abstracted); Euler and RK4; per-world
+ * randomised parameters; no disturbances, no fidelity extras (CF_E_UNSUPPORTED otherwise).  goal: 3 floats on the HOST. */
+size_t cf_grad_scratch_bytes(const cf_sim *sim, int n_steps);
+int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
+            float *loss_dev, void *grad_dev, void *scratch_dev, size_t scratch_bytes);
+
 const char *cf_last_error(void);
 /* Host-side Philox4x32-10 of this library, for the bit-exact check against the oracle's (C9). */
 int cf_debug_philox(uint64_t seed, const uint32_t ctr[4], uint32_t out[4]);

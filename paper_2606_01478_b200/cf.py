@@ -102,6 +102,8 @@ def lib():
         "cf_mppi_update": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, sz]),
         "cf_mppi_iterate": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, sz]),
         "cf_mppi_iterate_host": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, vp, sz]),
+        "cf_grad_scratch_bytes": (sz, [vp, C.c_int]),
+        "cf_grad": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float * 3), vp, vp, vp, sz]),
         "cf_last_error": (C.c_char_p, []),
         "cf_debug_philox": (C.c_int, [C.c_uint64, C.POINTER(C.c_uint32 * 4), C.POINTER(C.c_uint32 * 4)]),
         "cf_debug_philox_dev": (C.c_int, [vp, C.c_uint64, vp, C.c_int, vp, vp, vp]),
@@ -117,7 +119,8 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_set_stream", "cf_reset", "cf_set_state", "cf_set_full", "cf_step", "cf_staging_bytes", "cf_step_host",
            "cf_get_state", "cf_get_state_host", "cf_get_aux", "cf_get_aux_host", "cf_step_counter", "cf_sync_counters",
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
-           "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host"]
+           "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host", "cf_grad_scratch_bytes",
+           "cf_grad"]
 
 
 def _check(rc: int):
@@ -334,6 +337,27 @@ class Sim:
         assert e is None or e.numel() == 4 * self.MN
         assert c is None or c.numel() == self.MN
         _check(lib().cf_set_plan_state(self._h, _dptr(e), _dptr(c)))
+
+    # -- gradient of the goal distance w.r.t. the commands (cf_grad) --------------------------------------------------
+    def grad(self, cmds, n_steps: int, goal, cmd_hold: int = 1, loss=None, grad=None):
+        """cmds: float32 [K][MN][4] (device).  Returns (loss [MN], grad [K][MN][4]) device tensors; the simulator state
+        is left unchanged."""
+        torch = _torch()
+        cm = self._dev(cmds, torch.float32)
+        assert cm.numel() % (4 * self.MN) == 0
+        K = cm.numel() // (4 * self.MN)
+        need = lib().cf_grad_scratch_bytes(self._h, int(n_steps))
+        if getattr(self, "_grad_scratch", None) is None or self._grad_scratch.numel() < need + 16:
+            self._grad_scratch = torch.empty(need + 16, dtype=torch.uint8, device=self.device)
+        sp = self._grad_scratch.data_ptr() + (-self._grad_scratch.data_ptr()) % 16
+        if loss is None:
+            loss = torch.empty(self.MN, dtype=torch.float32, device=self.device)
+        if grad is None:
+            grad = torch.empty((K, self.MN, 4), dtype=torch.float32, device=self.device)
+        g3 = (C.c_float * 3)(*[float(v) for v in goal])
+        _check(lib().cf_grad(self._h, _dptr(cm), K, int(cmd_hold), int(n_steps), C.byref(g3), _dptr(loss), _dptr(grad),
+                             C.c_void_p(sp), need))
+        return loss, grad
 
     # -- sampling-based planner (cf_mppi_*) --------------------------------------------------------------------------
     def mppi_params(self, horizon: int, cmd_hold: int, n_elite: int, lam: float, shift: int = 1) -> MppiParams:

@@ -464,6 +464,8 @@ static int launch_set_state(cf_sim *sim, const float *src, int broadcast) {
 
 // A broadcast cf_set_state is lazy: the D floats are parked in the workspace and the next cf_step starts every drone
 // from them in registers (no 35-plane write + re-read).  Anything else that touches the planes materialises it first.
+static int materialise(cf_sim *sim);
+int cf_materialise(cf_sim *sim) { return materialise(sim); }
 static int materialise(cf_sim *sim) {
   if (!sim->pending_bcast) return CF_OK;
   sim->pending_bcast = false;

@@ -1,0 +1,451 @@
+// cf_grad.cu -- reverse-mode differentiation of the fused rollout (Fig. 3D: "differentiating a goal
+// distance with respect to the control inputs" through n consecutive steps, dynamics AND onboard controller stack).
+//
+//   L(u) = || p_n(u) - goal ||,   g[k] = dL / du[k]   for the command sequence u[k] (each held cmd_hold steps),
+//
+// as ONE hand-written adjoint kernel (no tape, no autodiff framework): thread = drone.  Forward sweep: the production
+// step (same device functions as the rollout kernel: deriv_fp / deriv_ab, attitude_tick, mixer) with the pre-step state
+// of every step parked in a caller-provided history buffer [n_steps][HD][MN] (SoA, coalesced).  Backward sweep: for
+// t = n-1 .. 0 the step is recomputed from its parked state and the cotangent is pulled back through quaternion
+// normalisation, RK4 / Euler (stage states recomputed in registers), the derivative (hand-derived VJPs of Eqs. (1)-(4),
+// (6) and (7)-(10)), the motor mixer (sqrt and clips: derivative 0 where a clip is active, reading R33) and the attitude
+// controller (rotation-matrix error, clipped integral, desired rotation from the commanded Euler angles).  The adjoint
+// of a held command accumulates over the steps / ticks that used it and is written when its fetch step is reached.
+// The simulator state is not modified.
+#include "cf_internal.h"
+
+using namespace cf;
+
+namespace {
+
+struct GradArgs {
+  const float *state, *ctrl, *wparam;
+  const float4 *cmds;      // [n_cmds][MN]
+  float4 *grad;            // [n_cmds][MN]
+  float *loss;             // [MN]
+  float *hist;             // [n_steps][HD][MN]
+  long long MN, M, N;
+  int n_steps, cmd_hold, n_cmds;
+  uint32_t s0;
+  float goal[3];
+};
+
+template <int MODEL> struct Dim { static constexpr int D = MODEL == MODEL_FP ? 17 : 13; };
+
+// ---- VJP of the first-principles derivative (lean form: Eq. (6) with one time constant, pure-quadratic curves) -------
+// cotangent a[17] of dx -> gx[17] (accumulated into), gu[4] (accumulated into)
+__device__ __forceinline__ void vjp_deriv_fp(const DevParams &P, const Plant<MODEL_FP, 0> &pl, const float *x,
+                                             const float *a, float *gx, float *gu) {
+  const float *q = x + 3, *w = x + 10, *Om = x + 13;
+  const float *a_p = a, *a_q = a + 3, *a_v = a + 7, *a_w = a + 10, *a_Om = a + 13;
+  float *g_q = gx + 3, *g_v = gx + 7, *g_w = gx + 10, *g_Om = gx + 13;
+#pragma unroll
+  for (int j = 0; j < 3; ++j) g_v[j] += a_p[j];                                       // Eq. (1)
+  // Eq. (3): dv = zB F/m - g e_z
+  float w2s = Om[0] * Om[0] + Om[1] * Om[1] + Om[2] * Om[2] + Om[3] * Om[3];
+  float acc = pl.kf2 * w2s * pl.inv_m;
+  float zx = 2.0f * (q[0] * q[2] + q[3] * q[1]), zy = 2.0f * (q[1] * q[2] - q[3] * q[0]);
+  float zz = 1.0f - 2.0f * (q[0] * q[0] + q[1] * q[1]);
+  float gF = (zx * a_v[0] + zy * a_v[1] + zz * a_v[2]) * pl.inv_m;
+  float gzx = a_v[0] * acc, gzy = a_v[1] * acc, gzz = a_v[2] * acc;
+  g_q[0] += 2.0f * (q[2] * gzx - q[3] * gzy) - 4.0f * q[0] * gzz;
+  g_q[1] += 2.0f * (q[3] * gzx + q[2] * gzy) - 4.0f * q[1] * gzz;
+  g_q[2] += 2.0f * (q[0] * gzx + q[1] * gzy);
+  g_q[3] += 2.0f * (q[1] * gzx - q[0] * gzy);
+  // Eq. (4): dw = tau/J + cJ (w x w terms); tau from the mixing matrix C1
+  float gt[3] = { a_w[0] * pl.inv_J[0], a_w[1] * pl.inv_J[1], a_w[2] * pl.inv_J[2] };
+  const float lk = P.lever * pl.kf2;
+  const float sx[4] = { -1, -1, 1, 1 }, sy[4] = { -1, 1, 1, -1 }, sz[4] = { -1, 1, -1, 1 };
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    float g_w2 = pl.kf2 * gF + lk * (sx[k] * gt[0] + sy[k] * gt[1]) + pl.km2 * sz[k] * gt[2];
+    g_Om[k] += 2.0f * Om[k] * g_w2 - pl.cv * a_Om[k];                                 // Eq. (6): dOm = cv (u - Om)
+    gu[k] += pl.cv * a_Om[k];
+  }
+  g_w[1] += pl.cJ[0] * w[2] * a_w[0]; g_w[2] += pl.cJ[0] * w[1] * a_w[0];
+  g_w[2] += pl.cJ[1] * w[0] * a_w[1]; g_w[0] += pl.cJ[1] * w[2] * a_w[1];
+  g_w[0] += pl.cJ[2] * w[1] * a_w[2]; g_w[1] += pl.cJ[2] * w[0] * a_w[2];
+  // Eq. (2): dq = 1/2 q (x) (w, 0)
+  float bx = 0.5f * a_q[0], by = 0.5f * a_q[1], bz = 0.5f * a_q[2], bw = 0.5f * a_q[3];
+  g_q[3] += w[0] * bx + w[1] * by + w[2] * bz;
+  g_q[0] += -w[2] * by + w[1] * bz - w[0] * bw;
+  g_q[1] += w[2] * bx - w[0] * bz - w[1] * bw;
+  g_q[2] += -w[1] * bx + w[0] * by - w[2] * bw;
+  g_w[0] += q[3] * bx + q[2] * by - q[1] * bz - q[0] * bw;
+  g_w[1] += -q[2] * bx + q[3] * by + q[0] * bz - q[1] * bw;
+  g_w[2] += q[1] * bx - q[0] * by + q[3] * bz - q[2] * bw;
+}
+
+// ---- VJP of the abstracted derivative, Eqs. (7)-(10) -------------------------------------------------------------------
+__device__ __forceinline__ void vjp_deriv_ab(const DevParams &P, const Plant<MODEL_AB, 0> &pl, const float *x,
+                                             const float *a, float *gx, float *gu) {
+  float sn[3], cs[3];
+  sincos3_step(x + 3, sn, cs);
+  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
+  const float *a_p = a, *a_ps = a + 3, *a_v = a + 6, *a_dps = a + 9;
+  const float a_f = a[12];
+  float zx = cy * sp * cr + sy * sr, zy = sy * sp * cr - cy * sr, zz = cp * cr;
+  float acc = (P.ab_cf * x[12]) * pl.inv_m;
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    gx[6 + j] += a_p[j];                                                              // dp = v
+    gx[9 + j] += a_ps[j] + pl.b[j] * a_dps[j];                                        // dPsi = dPsi ; Eq. (10)
+    gx[3 + j] += pl.a[j] * a_dps[j];
+    gu[j] += pl.c[j] * a_dps[j];
+  }
+  // dv = zB cf f/m - g e_z : angles through zB, thrust state through acc
+  float dzr[3] = { -cy * sp * sr + sy * cr, -sy * sp * sr - cy * cr, -cp * sr };
+  float dzp[3] = { cy * cp * cr, sy * cp * cr, -sp * cr };
+  float dzy[3] = { -sy * sp * cr + cy * sr, cy * sp * cr + sy * sr, 0.0f };
+  gx[3] += (dzr[0] * a_v[0] + dzr[1] * a_v[1] + dzr[2] * a_v[2]) * acc;
+  gx[4] += (dzp[0] * a_v[0] + dzp[1] * a_v[1] + dzp[2] * a_v[2]) * acc;
+  gx[5] += (dzy[0] * a_v[0] + dzy[1] * a_v[1]) * acc;
+  gx[12] += (zx * a_v[0] + zy * a_v[1] + zz * a_v[2]) * (P.ab_cf * pl.inv_m) - pl.ctau * a_f;   // Eq. (9)
+  gu[3] += pl.ctau * a_f;
+}
+
+template <int MODEL>
+__device__ __forceinline__ void vjp_deriv(const DevParams &P, const Plant<MODEL, 0> &pl, const float *x, const float *a,
+                                          float *gx, float *gu) {
+  if constexpr (MODEL == MODEL_FP) vjp_deriv_fp(P, pl, x, a, gx, gu);
+  else vjp_deriv_ab(P, pl, x, a, gx, gu);
+}
+
+// ---- VJP of the attitude controller tick + mixer (C5, C6) -----------------------------------------------------------
+// inputs of the tick: q, w (state), cmd = (roll, pitch, yaw, F), iR (integral before the tick).
+// cotangents in: g_rpm[4] (of the rotor command), g_iRn[3] (of the integral after the tick).
+// out: accumulates into g_q[4], g_w[3], g_cmd[4]; g_iR[3] = cotangent of the integral before the tick.
+__device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const float *q, const float *w, const float *cmd,
+                                                  const float *iR, const float *g_rpm, const float *g_iRn,
+                                                  float *g_q, float *g_w, float *g_cmd, float *g_iR) {
+  float R[3][3], Rd[3][3];
+  quat_to_R(q, R);
+  euler_to_R(cmd[0], cmd[1], cmd[2], Rd);
+  auto Mij = [&](int i, int j) { return Rd[0][i] * R[0][j] + Rd[1][i] * R[1][j] + Rd[2][i] * R[2][j]; };
+  float eR[3] = { 0.5f * (Mij(2, 1) - Mij(1, 2)), 0.5f * (Mij(0, 2) - Mij(2, 0)), 0.5f * (Mij(1, 0) - Mij(0, 1)) };
+  float pre[3], iRn[3], tau[3];
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    pre[j] = fmaf(eR[j], P.h_att, iR[j]);
+    iRn[j] = clipf(pre[j], -P.iR_max, P.iR_max);
+    tau[j] = P.Jnom[j] * (-P.kR[j] * eR[j] - P.kW[j] * w[j] - P.kI[j] * iRn[j]);
+  }
+  // mixer forward (to know which clips are active), then its reverse
+  float a = 0.25f * cmd[3], bx = tau[0] * P.inv_4lever, by = tau[1] * P.inv_4lever, bz = tau[2] * P.inv_4kappa;
+  float f[4] = { a - bx - by - bz, a - bx + by + bz, a + bx + by - bz, a + bx - by + bz };
+  float gf[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    float fk = clipf(f[k], 0.0f, P.f_rotor_max);
+    float r = sqrtf(fk * P.inv_kf2);
+    bool live = f[k] > 0.0f && f[k] < P.f_rotor_max && r > P.rpm_min && r < P.rpm_max;     // R33: 0 where a clip is active
+    gf[k] = live ? g_rpm[k] * (0.5f * P.inv_kf2 / r) : 0.0f;                               // d sqrt(f/kf)/df = 1/(2 kf r)
+  }
+  float g_a = (gf[0] + gf[1]) + (gf[2] + gf[3]);
+  float g_bx = (gf[2] + gf[3]) - (gf[0] + gf[1]);
+  float g_by = (gf[1] + gf[2]) - (gf[0] + gf[3]);
+  float g_bz = (gf[1] + gf[3]) - (gf[0] + gf[2]);
+  g_cmd[3] += 0.25f * g_a;
+  float g_tau[3] = { g_bx * P.inv_4lever, g_by * P.inv_4lever, g_bz * P.inv_4kappa };
+  float g_eR[3];
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    float gt = P.Jnom[j] * g_tau[j];
+    g_eR[j] = -P.kR[j] * gt;
+    g_w[j] += -P.kW[j] * gt;
+    float g_in = g_iRn[j] - P.kI[j] * gt;                          // cotangent of the integral after the tick
+    float g_pre = (pre[j] > -P.iR_max && pre[j] < P.iR_max) ? g_in : 0.0f;
+    g_iR[j] = g_pre;
+    g_eR[j] += P.h_att * g_pre;
+  }
+  // e_R = 1/2 (M21 - M12, M02 - M20, M10 - M01),  M = Rd^T R
+  float G[3][3] = { { 0.0f, -0.5f * g_eR[2], 0.5f * g_eR[1] },
+                    { 0.5f * g_eR[2], 0.0f, -0.5f * g_eR[0] },
+                    { -0.5f * g_eR[1], 0.5f * g_eR[0], 0.0f } };        // G[i][j] = dL/dM_ij
+  float GR[3][3], GD[3][3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      GR[k][j] = Rd[k][0] * G[0][j] + Rd[k][1] * G[1][j] + Rd[k][2] * G[2][j];     // dL/dR_kj
+      GD[k][j] = R[k][0] * G[j][0] + R[k][1] * G[j][1] + R[k][2] * G[j][2];        // dL/dRd_kj
+    }
+  const float x = q[0], y = q[1], z = q[2], ww = q[3];
+  g_q[0] += 2.0f * (y * (GR[0][1] + GR[1][0]) + z * (GR[0][2] + GR[2][0]) + ww * (GR[2][1] - GR[1][2])) - 4.0f * x * (GR[1][1] + GR[2][2]);
+  g_q[1] += 2.0f * (x * (GR[0][1] + GR[1][0]) + z * (GR[1][2] + GR[2][1]) + ww * (GR[0][2] - GR[2][0])) - 4.0f * y * (GR[0][0] + GR[2][2]);
+  g_q[2] += 2.0f * (x * (GR[0][2] + GR[2][0]) + y * (GR[1][2] + GR[2][1]) + ww * (GR[1][0] - GR[0][1])) - 4.0f * z * (GR[0][0] + GR[1][1]);
+  g_q[3] += 2.0f * (x * (GR[2][1] - GR[1][2]) + y * (GR[0][2] - GR[2][0]) + z * (GR[1][0] - GR[0][1]));
+  // Rd = Rz(yaw) Ry(pitch) Rx(roll): d/droll rotates columns 1, 2; d/dyaw rotates rows 0, 1; d/dpitch written out
+  float sr, cr, sp, cp, sy, cy;
+  sincosf(cmd[0], &sr, &cr); sincosf(cmd[1], &sp, &cp); sincosf(cmd[2], &sy, &cy);
+  g_cmd[0] += GD[0][1] * Rd[0][2] - GD[0][2] * Rd[0][1] + GD[1][1] * Rd[1][2] - GD[1][2] * Rd[1][1] + GD[2][1] * Rd[2][2] - GD[2][2] * Rd[2][1];
+  g_cmd[1] += GD[0][0] * (-cy * sp) + GD[0][1] * (cy * cp * sr) + GD[0][2] * (cy * cp * cr)
+            + GD[1][0] * (-sy * sp) + GD[1][1] * (sy * cp * sr) + GD[1][2] * (sy * cp * cr)
+            + GD[2][0] * (-cp) + GD[2][1] * (-sp * sr) + GD[2][2] * (-sp * cr);
+  g_cmd[2] += -GD[0][0] * Rd[1][0] - GD[0][1] * Rd[1][1] - GD[0][2] * Rd[1][2]
+            + GD[1][0] * Rd[0][0] + GD[1][1] * Rd[0][1] + GD[1][2] * Rd[0][2];
+}
+
+// ---- one step forward (C4) from x with the inputs held; returns the un-normalised quaternion norm for the FP model ----
+template <int MODEL, int INTEG>
+__device__ __forceinline__ void step_forward(const DevParams &P, const Plant<MODEL, 0> &pl, float *x, const float *u) {
+  constexpr int D = Dim<MODEL>::D;
+  const float fd[3] = { 0.f, 0.f, 0.f };
+  float k[D];
+  if constexpr (INTEG == INTEG_EULER) {
+    deriv<MODEL, 0>(P, pl, x, u, fd, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) x[j] = fmaf(P.h, k[j], x[j]);
+  } else {
+    float xs[D], acc[D];
+    deriv<MODEL, 0>(P, pl, x, u, fd, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { acc[j] = k[j]; xs[j] = fmaf(P.half_h, k[j], x[j]); }
+    deriv<MODEL, 0>(P, pl, xs, u, fd, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { acc[j] = fmaf(2.0f, k[j], acc[j]); xs[j] = fmaf(P.half_h, k[j], x[j]); }
+    deriv<MODEL, 0>(P, pl, xs, u, fd, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { acc[j] = fmaf(2.0f, k[j], acc[j]); xs[j] = fmaf(P.h, k[j], x[j]); }
+    deriv<MODEL, 0>(P, pl, xs, u, fd, k);
+#pragma unroll
+    for (int j = 0; j < D; ++j) x[j] = fmaf(P.h_sixth, acc[j] + k[j], x[j]);
+  }
+  if constexpr (MODEL == MODEL_FP) {
+    float *q = x + 3;
+    float inv = rsqrtf(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) q[j] *= inv;
+  }
+}
+
+// ---- pull the cotangent lam (of the post-step state) back through one step that started at x with held inputs u -----
+// on return lam = cotangent of x, gu accumulates the cotangent of u
+template <int MODEL, int INTEG>
+__device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MODEL, 0> &pl, const float *x,
+                                              const float *u, float *lam, float *gu) {
+  constexpr int D = Dim<MODEL>::D;
+  const float fd[3] = { 0.f, 0.f, 0.f };
+  float k1[D], x2[D], x3[D], x4[D], kk[D];
+  deriv<MODEL, 0>(P, pl, x, u, fd, k1);
+  if constexpr (INTEG == INTEG_RK4) {
+#pragma unroll
+    for (int j = 0; j < D; ++j) x2[j] = fmaf(P.half_h, k1[j], x[j]);
+    deriv<MODEL, 0>(P, pl, x2, u, fd, kk);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { k1[j] = fmaf(2.0f, kk[j], k1[j]); x3[j] = fmaf(P.half_h, kk[j], x[j]); }
+    deriv<MODEL, 0>(P, pl, x3, u, fd, kk);
+#pragma unroll
+    for (int j = 0; j < D; ++j) { k1[j] = fmaf(2.0f, kk[j], k1[j]); x4[j] = fmaf(P.h, kk[j], x[j]); }
+  }
+  if constexpr (MODEL == MODEL_FP) {
+    // q+ = qt / |qt| with qt the integrator's un-normalised quaternion: g_qt = (g - q+ (q+ . g)) / |qt|
+    float qt[4];
+    if constexpr (INTEG == INTEG_RK4) {
+      deriv<MODEL, 0>(P, pl, x4, u, fd, kk);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) qt[j] = fmaf(P.h_sixth, k1[3 + j] + kk[3 + j], x[3 + j]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) qt[j] = fmaf(P.h, k1[3 + j], x[3 + j]);
+    }
+    float inv = rsqrtf(qt[0] * qt[0] + qt[1] * qt[1] + qt[2] * qt[2] + qt[3] * qt[3]);
+    float dot = 0.f;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qt[j] *= inv; dot = fmaf(qt[j], lam[3 + j], dot); }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) lam[3 + j] = (lam[3 + j] - qt[j] * dot) * inv;
+  }
+  float a[D], gx[D];
+  if constexpr (INTEG == INTEG_EULER) {
+#pragma unroll
+    for (int j = 0; j < D; ++j) { a[j] = P.h * lam[j]; gx[j] = 0.f; }
+    vjp_deriv<MODEL>(P, pl, x, a, gx, gu);
+#pragma unroll
+    for (int j = 0; j < D; ++j) lam[j] += gx[j];
+  } else {
+    // x+ = x + h/6 (k1 + 2 k2 + 2 k3 + k4), k2 = f(x + h/2 k1), k3 = f(x + h/2 k2), k4 = f(x + h k3)
+    float tot[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) { a[j] = P.h_sixth * lam[j]; gx[j] = 0.f; tot[j] = 0.f; }
+    vjp_deriv<MODEL>(P, pl, x4, a, gx, gu);                                   // k4
+#pragma unroll
+    for (int j = 0; j < D; ++j) { tot[j] += gx[j]; a[j] = fmaf(P.h, gx[j], 2.0f * P.h_sixth * lam[j]); gx[j] = 0.f; }
+    vjp_deriv<MODEL>(P, pl, x3, a, gx, gu);                                   // k3
+#pragma unroll
+    for (int j = 0; j < D; ++j) { tot[j] += gx[j]; a[j] = fmaf(P.half_h, gx[j], 2.0f * P.h_sixth * lam[j]); gx[j] = 0.f; }
+    vjp_deriv<MODEL>(P, pl, x2, a, gx, gu);                                   // k2
+#pragma unroll
+    for (int j = 0; j < D; ++j) { tot[j] += gx[j]; a[j] = fmaf(P.half_h, gx[j], P.h_sixth * lam[j]); gx[j] = 0.f; }
+    vjp_deriv<MODEL>(P, pl, x, a, gx, gu);                                    // k1
+#pragma unroll
+    for (int j = 0; j < D; ++j) lam[j] += tot[j] + gx[j];
+  }
+}
+
+// history record of one step: pre-step state, and for the first-principles model the controller integral before the
+// step's tick and the rotor command the step integrated with
+template <int MODEL> struct Hist { static constexpr int HD = MODEL == MODEL_FP ? 17 + 3 + 4 : 13; };
+
+template <int MODEL, int INTEG, int IFACE>
+__global__ void __launch_bounds__(128)
+grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParams P, int randp) {
+  constexpr int D = Dim<MODEL>::D, HD = Hist<MODEL>::HD;
+  constexpr bool FP = MODEL == MODEL_FP;
+  constexpr bool HAS_ATT = FP && IFACE == IF_ATTITUDE;
+  const long long MN = A.MN;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= MN) return;
+  Plant<MODEL, 0> pl;
+  pl.load(P, A.wparam, A.M, i / A.N, randp != 0);
+
+  float x[D], iR[3] = { 0, 0, 0 }, rpm_cmd[4] = { 0, 0, 0, 0 }, cmd[4] = { 0, 0, 0, 0 };
+#pragma unroll
+  for (int j = 0; j < D; ++j) x[j] = A.state[j * MN + i];
+  if (FP) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) iR[j] = A.ctrl[j * MN + i];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) rpm_cmd[j] = A.ctrl[(10 + j) * MN + i];
+  }
+  // ---- forward sweep -----------------------------------------------------------------------------------------
+  int att_phase = (int)(A.s0 % (uint32_t)P.att_div);
+  for (int t = 0; t < A.n_steps; ++t) {
+    float *h = A.hist + (size_t)t * HD * MN + i;
+#pragma unroll
+    for (int j = 0; j < D; ++j) __stcs(h + j * MN, x[j]);
+    if (t % A.cmd_hold == 0) {
+      float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
+      cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
+      if (FP && IFACE == IF_ROTOR) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) rpm_cmd[j] = clipf(cmd[j], P.rpm_min, P.rpm_max);
+      }
+    }
+    if (HAS_ATT) {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) __stcs(h + (17 + j) * MN, iR[j]);
+      if (att_phase == 0) {
+        float Rd[3][3];
+        euler_to_R(cmd[0], cmd[1], cmd[2], Rd);
+        attitude_tick<0>(P, x + 3, x + 10, Rd, cmd[3], iR, rpm_cmd);
+      }
+      att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
+    }
+    if (FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) __stcs(h + (20 + j) * MN, rpm_cmd[j]);
+    }
+    step_forward<MODEL, INTEG>(P, pl, x, FP ? rpm_cmd : cmd);
+  }
+  // ---- loss and its cotangent ----------------------------------------------------------------------------------
+  float lam[D];
+#pragma unroll
+  for (int j = 0; j < D; ++j) lam[j] = 0.f;
+  {
+    float ex = x[0] - A.goal[0], ey = x[1] - A.goal[1], ez = x[2] - A.goal[2];
+    float L = sqrtf(ex * ex + ey * ey + ez * ez);
+    A.loss[i] = L;
+    float inv = L > 0.f ? 1.0f / L : 0.f;
+    lam[0] = ex * inv; lam[1] = ey * inv; lam[2] = ez * inv;
+  }
+  // ---- backward sweep ------------------------------------------------------------------------------------------
+  float g_cmd[4] = { 0, 0, 0, 0 };      // cotangent of the held command, until its fetch step is reached
+  float g_rpm[4] = { 0, 0, 0, 0 };      // cotangent of the held rotor command, until the tick / fetch that set it
+  float g_iR[3] = { 0, 0, 0 };          // cotangent of the controller integral
+  att_phase = (int)((A.s0 + (uint32_t)A.n_steps - 1u) % (uint32_t)P.att_div);
+  for (int t = A.n_steps - 1; t >= 0; --t) {
+    const float *h = A.hist + (size_t)t * HD * MN + i;
+#pragma unroll
+    for (int j = 0; j < D; ++j) x[j] = __ldcs(h + j * MN);
+    if (t % A.cmd_hold == A.cmd_hold - 1 || t == A.n_steps - 1) {             // entering the run of command t / hold
+      float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
+      cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
+    }
+    if (FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) rpm_cmd[j] = __ldcs(h + (20 + j) * MN);
+      step_backward<MODEL, INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
+    } else {
+      step_backward<MODEL, INTEG>(P, pl, x, cmd, lam, g_cmd);
+    }
+    if (HAS_ATT) {
+      if (att_phase == 0) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) iR[j] = __ldcs(h + (17 + j) * MN);
+        float g_prev[3];
+        vjp_attitude_tick(P, x + 3, x + 10, cmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_cmd, g_prev);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) g_iR[j] = g_prev[j];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) g_rpm[j] = 0.f;
+      }
+      att_phase = att_phase == 0 ? P.att_div - 1 : att_phase - 1;
+    }
+    if (t % A.cmd_hold == 0) {                                                 // the fetch step of command t / hold
+      if (FP && IFACE == IF_ROTOR) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { g_cmd[j] = (cmd[j] > P.rpm_min && cmd[j] < P.rpm_max) ? g_rpm[j] : 0.f; g_rpm[j] = 0.f; }
+      }
+      A.grad[(size_t)(t / A.cmd_hold) * MN + i] = make_float4(g_cmd[0], g_cmd[1], g_cmd[2], g_cmd[3]);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) g_cmd[j] = 0.f;
+    }
+  }
+}
+
+struct Entry { int model, integ, iface; void (*fn)(const GradArgs, const DevParams, int); };
+#define CF_G(M_, I_, F_) { M_, I_, F_, grad_kernel<M_, I_, F_> }
+const Entry kTable[] = {
+  CF_G(MODEL_FP, INTEG_EULER, IF_ATTITUDE), CF_G(MODEL_FP, INTEG_RK4, IF_ATTITUDE),
+  CF_G(MODEL_FP, INTEG_EULER, IF_ROTOR),    CF_G(MODEL_FP, INTEG_RK4, IF_ROTOR),
+  CF_G(MODEL_AB, INTEG_EULER, IF_ATTITUDE), CF_G(MODEL_AB, INTEG_RK4, IF_ATTITUDE),
+};
+
+int check(const cf_sim *sim, int n_cmds, int cmd_hold, int n_steps) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  if (n_steps < 1 || cmd_hold < 1 || n_cmds < 1) return fail(CF_E_ARG, "n_steps, cmd_hold, n_cmds >= 1");
+  if ((long long)n_cmds * cmd_hold < n_steps) return fail(CF_E_SHAPE, "n_cmds * cmd_hold < n_steps");
+  if (sim->p.cmd_source != CF_CMD_BUFFER || (sim->opt & (OPT_DIST | OPT_NOISE | OPT_EXTRAS)) != 0)
+    return fail(CF_E_UNSUPPORTED, "cf_grad differentiates the command-buffer rollout without disturbances / fidelity extras");
+  return CF_OK;
+}
+
+}  // namespace
+
+extern "C" size_t cf_grad_scratch_bytes(const cf_sim *sim, int n_steps) {
+  if (!sim || n_steps < 1) return 0;
+  size_t hd = sim->model == CF_MODEL_FIRST_PRINCIPLES ? Hist<MODEL_FP>::HD : Hist<MODEL_AB>::HD;
+  return sizeof(float) * hd * (size_t)sim->MN * (size_t)n_steps;
+}
+
+extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
+                       float *loss_dev, void *grad_dev, void *scratch_dev, size_t scratch_bytes) {
+  int rc = check(sim, n_cmds, cmd_hold, n_steps);
+  if (rc != CF_OK) return rc;
+  if (!cmds_dev || !goal || !loss_dev || !grad_dev || !scratch_dev) return fail(CF_E_ARG, "NULL argument");
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_grad before cf_reset");
+  if (((uintptr_t)cmds_dev & 15) || ((uintptr_t)grad_dev & 15) || ((uintptr_t)scratch_dev & 15))
+    return fail(CF_E_BUFFER, "cmds, grad and scratch must be 16-byte aligned");
+  if (scratch_bytes < cf_grad_scratch_bytes(sim, n_steps)) return fail(CF_E_BUFFER, "scratch too small");
+  const Entry *e = nullptr;
+  for (const Entry &c : kTable)
+    if (c.model == sim->model && c.integ == sim->p.integrator && c.iface == sim->p.iface) e = &c;
+  if (!e) return fail(CF_E_UNSUPPORTED, "cf_grad: interface not differentiated (rotor / attitude for the first-principles model, attitude for the abstracted one)");
+  rc = cf_materialise(sim);      // a pending broadcast cf_set_state must be in the planes: the kernel reads them
+  if (rc != CF_OK) return rc;
+  GradArgs A;
+  A.state = sim->state; A.ctrl = sim->ctrl; A.wparam = sim->wparam;
+  A.cmds = (const float4 *)cmds_dev; A.grad = (float4 *)grad_dev; A.loss = loss_dev; A.hist = (float *)scratch_dev;
+  A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.n_cmds = n_cmds;
+  A.s0 = (uint32_t)sim->s_host;
+  for (int j = 0; j < 3; ++j) A.goal[j] = goal[j];
+  const int block = 128;
+  e->fn<<<(unsigned)((sim->MN + block - 1) / block), block, 0, sim->stream>>>(A, sim->dp, (sim->opt & OPT_RANDP) ? 1 : 0);
+  CF_CUDA(cudaGetLastError());
+  // commands beyond the last used one get a zero gradient
+  int used = (n_steps + cmd_hold - 1) / cmd_hold;
+  if (used < n_cmds)
+    CF_CUDA(cudaMemsetAsync((float4 *)grad_dev + (size_t)used * sim->MN, 0, sizeof(float4) * (size_t)(n_cmds - used) * sim->MN, sim->stream));
+  return CF_OK;
+}

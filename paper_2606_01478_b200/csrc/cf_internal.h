@@ -35,6 +35,7 @@ struct cf_sim {
   float hover_rpm;
 };
 
+int cf_materialise(cf_sim *sim);         // cf_api.cu: write a pending broadcast cf_set_state into the planes
 int cf_refresh_cost(cf_sim *sim);        // cf_api.cu: cost_drone <- J of the current planes
 char *cf_err_buf();                      // thread-local, 512 bytes (cf_api.cu)
 inline int fail(int code, const char *fmt, ...) {

@@ -1,0 +1,156 @@
+"""GPU parity of cf_grad (Fig. 3D: goal distance differentiated w.r.t. the control inputs through n steps,
+dynamics and controller stack) against oracle/grad.py, the Richardson-extrapolated central difference of the float64 step.
+
+Tolerance (floating point; north_star states none for gradients, derived in DESIGN.md "Arithmetic and tolerances"): per
+drone |g_gpu - g_oracle| <= 1e-3 * max_k,j |g_oracle| + 1e-9 -- the float32 adjoint carries the 1e-7 rounding of ~10^3
+operations per step and the MUFU approximations of the forward step, the oracle's own rounding floor is 1e-11; measured
+worst 3e-5.  The loss itself is held to the state tolerance 1e-4.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def cf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_01478_b200 import build, cf as m
+    build.build()
+    m.lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def og():
+    from oracle import grad
+    return grad
+
+
+def make_pair(cf, cfo, M, model, params, seed=3, pre_steps=0):
+    g = cf.Sim(M, 1, model, params)
+    o = cfo.OracleSim(M, 1, model, params)
+    g.reset(seed), o.reset(seed)
+    if pre_steps:
+        warm = np.zeros((1, M, 4), dtype=np.float32)
+        warm[..., 3] = 0.27 if params.get("iface", 2) != 0 else 14000.0
+        g.step(warm, pre_steps, cmd_hold=pre_steps), o.step(warm, pre_steps, cmd_hold=pre_steps)
+    return g, o
+
+
+def att_cmds(K, M, seed, amp=0.2):
+    rng = np.random.default_rng(seed)
+    c = np.zeros((K, M, 4), dtype=np.float32)
+    c[..., :2] = rng.uniform(-amp, amp, (K, M, 2))
+    c[..., 2] = rng.uniform(-0.1, 0.1, (K, M))
+    c[..., 3] = rng.uniform(0.2, 0.35, (K, M))
+    return c
+
+
+def compare(g_gpu, L_gpu, L_o, g_o, tol=1e-3):
+    scale = np.abs(g_o).max(axis=(0, 2))                          # per drone
+    err = np.abs(g_gpu.astype(np.float64) - g_o).max(axis=(0, 2))
+    worst = (err / (scale + 1e-30)).max()
+    assert (err <= tol * scale + 1e-9).all(), f"worst relative gradient error {worst:.2e}"
+    assert (np.abs(L_gpu - L_o) <= 1e-4 * np.maximum(L_o, 1.0)).all()
+    return worst
+
+
+FP_TILT = dict(f_phys=1000.0, f_att=500.0, init_mode=1, p0_lo=[-1, -1, 0], p0_hi=[1, 1, 2], tilt0_max=0.4)
+GOAL = [0.5, -0.2, 1.2]
+
+
+@pytest.mark.parametrize("integrator,hold,n,pre", [(1, 1, 10, 0), (1, 1, 10, 1), (0, 3, 11, 0), (0, 2, 10, 3), (1, 4, 12, 0)])
+def test_first_principles_attitude_interface_gradient(cf, cfo, og, integrator, hold, n, pre):
+    M = 257
+    lo, hi = [1.0] * 12, [1.0] * 12
+    for s in (0, 1, 2, 3):
+        lo[s], hi[s] = 0.9, 1.1
+    lo[4], hi[4] = 0.95, 1.05                                      # per-world m, J, k_f (the controller keeps the nominal)
+    params = dict(FP_TILT, integrator=integrator, iface=2, rnd_lo=lo, rnd_hi=hi)
+    g, o = make_pair(cf, cfo, M, 0, params, pre_steps=pre)
+    K = -(-n // hold) + 1                                          # one command more than used: its gradient must be 0
+    cmds = att_cmds(K, M, seed=integrator * 10 + hold)
+    before = g.get_state().cpu().numpy().copy()
+    L_gpu, g_gpu = g.grad(cmds, n, GOAL, cmd_hold=hold)
+    L_o, g_o = og.value_and_grad(o, cmds, n, hold, GOAL)
+    worst = compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
+    assert (g_gpu[-1] == 0).all().item()
+    assert np.array_equal(g.get_state().cpu().numpy(), before) and g.step_counter == pre      # pure: nothing moved
+    assert np.abs(g_o[..., :3]).max() > 0 and np.abs(g_o[..., 3]).max() > 0                   # all four inputs are live
+    print(f"worst relative gradient error {worst:.2e}")
+
+
+@pytest.mark.parametrize("integrator", [0, 1])
+def test_first_principles_rotor_interface_gradient(cf, cfo, og, integrator):
+    M = 96
+    params = dict(FP_TILT, integrator=integrator, iface=0)
+    g, o = make_pair(cf, cfo, M, 0, params)
+    rng = np.random.default_rng(4)
+    cmds = rng.uniform(12000, 17000, (5, M, 4)).astype(np.float32)
+    cmds[2, :7] = 25000.0                                          # beyond rpm_max: clipped, zero gradient there
+    L_gpu, g_gpu = g.grad(cmds, 10, GOAL, cmd_hold=2)
+    L_o, g_o = og.value_and_grad(o, cmds, 10, 2, GOAL)
+    compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
+    assert (g_gpu[2, :7] == 0).all().item() and np.abs(g_o[2, :7]).max() == 0
+
+
+@pytest.mark.parametrize("integrator,hold", [(0, 1), (1, 2)])
+def test_abstracted_model_gradient_with_jittered_coefficients(cf, cfo, og, integrator, hold):
+    M = 300
+    lo, hi = [1.0] * 12, [1.0] * 12
+    for s in (0, 1, 2, 3, 4, 5, 6, 8, 9, 10, 11):
+        lo[s], hi[s] = 0.9, 1.1
+    params = dict(integrator=integrator, iface=2, f_phys=500.0, f_att=500.0, init_mode=1, p0_lo=[-1, -1, 0],
+                  p0_hi=[1, 1, 2], tilt0_max=0.4, rnd_lo=lo, rnd_hi=hi)
+    g, o = make_pair(cf, cfo, M, 1, params)
+    cmds = att_cmds(-(-20 // hold), M, seed=7, amp=0.3)
+    L_gpu, g_gpu = g.grad(cmds, 20, GOAL, cmd_hold=hold)
+    L_o, g_o = og.value_and_grad(o, cmds, 20, hold, GOAL)
+    compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
+
+
+def test_saturated_and_broadcast_start_and_unsupported_configurations(cf, cfo, og):
+    params = dict(f_phys=1000.0, f_att=500.0, init_mode=0, integrator=1, iface=2)
+    g, o = make_pair(cf, cfo, 64, 0, params)
+    x0 = np.zeros(17); x0[2] = 1.0; x0[3:7] = [0.05, -0.03, 0.02, 0.998]; x0[3:7] /= np.linalg.norm(x0[3:7]); x0[13:] = 14000.0
+    g.set_state(x0.astype(np.float32), broadcast=True), o.set_state(x0.astype(np.float32).astype(np.float64), broadcast=True)
+    cmds = att_cmds(5, 64, seed=9)
+    cmds[:, :8, 3] = 2.0                                           # hard saturation of all four rotors
+    L_gpu, g_gpu = g.grad(cmds, 10, GOAL, cmd_hold=2)              # lazy broadcast is materialised first
+    L_o, g_o = og.value_and_grad(o, cmds, 10, 2, GOAL)
+    compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
+    assert (g_gpu[:, :8, 3] == 0).all().item()
+    for bad in (dict(dist_sigma=0.005), dict(Jp=1e-8), dict(iface=3)):
+        s = cf.Sim(4, 1, 0, dict(params, **bad))
+        s.reset(1)
+        with pytest.raises(cf.CfError) as e:
+            s.grad(cmds[:, :4], 10, GOAL, cmd_hold=2)
+        assert e.value.code == cf.E_UNSUPPORTED, bad
+    with pytest.raises(cf.CfError) as e:
+        g.grad(cmds, 11, GOAL, cmd_hold=2)
+    assert e.value.code == cf.E_SHAPE
+
+
+def test_full_size_gradient_batch_sampled_against_the_oracle(cf, cfo, og):
+    """The Fig. 3D shape: 2^20 worlds, first-principles model, RK4, attitude controller, 10 steps, 10 commands."""
+    M = 1 << 20
+    params = dict(FP_TILT, integrator=1, iface=2)
+    g = cf.Sim(M, 1, 0, params)
+    g.reset(11)
+    import torch
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    cmds = torch.zeros((10, M, 4), dtype=torch.float32, device="cuda")
+    cmds[..., :2] = (torch.rand((10, M, 2), generator=gen, device="cuda") - 0.5) * 0.4
+    cmds[..., 3] = 0.2 + 0.15 * torch.rand((10, M), generator=gen, device="cuda")
+    L_gpu, g_gpu = g.grad(cmds, 10, GOAL)
+    assert torch.isfinite(g_gpu).all().item() and torch.isfinite(L_gpu).all().item()
+    rng = np.random.default_rng(0)
+    for w in np.concatenate([[0, 31, 32, M - 1], rng.integers(0, M, 28)]):
+        o = cfo.OracleSim(1, 1, 0, dict(params, world_offset=int(w)))
+        o.reset(11)
+        c = cmds[:, w:w + 1].cpu().numpy()
+        L_o, g_o = og.value_and_grad(o, c, 10, 1, GOAL)
+        compare(g_gpu[:, w:w + 1].cpu().numpy(), L_gpu[w:w + 1].cpu().numpy(), L_o, g_o)
