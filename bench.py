@@ -29,8 +29,8 @@ DEFAULT_WORKLOAD = "cfg3"
 # Algorithmic FP32 operations per drone-step: every add / sub / mul / div / sqrt /
 # trig / log / min / max / clip of the float64 oracle's formulas counts 1 (an FMA is 2); Philox integer work is not
 # counted.  Controller ticks are amortised over their period.
-ALGO_FLOPS = {"mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
-BOUND = {"mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
+ALGO_FLOPS = {"grad": 2120, "mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
+BOUND = {"grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
 SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of the rollout kernel, one launch, from the `ncu --set full` captures
 # summarised in profiles/r1_<workload>_rollout.md (static: ncu never runs inside bench.py)
@@ -61,6 +61,8 @@ def algo_bytes_per_launch(wl) -> int:
     resident = 2 * (wl.D + ctrl_planes) * 4 * MN + (2 * 8 * 4 * MN if wl.params.get("n_obstacles") else 0)
     wparam = (14 if wl.model == 0 else 11) * 4 * wl.M
     plan = (4 + 2 + 1) * 4 * MN if wl.params.get("cost_on") else 0       # eps, cost (running, total), min distance out
+    if wl.name == "grad":     # planes in once, history out and back in, commands in, gradient + loss out
+        return (wl.D + 7) * 4 * MN + 2 * wl.n_steps * 24 * 4 * MN + 2 * wl.n_cmds * 16 * MN + 4 * MN
     return cmd + rec + resident + wparam + plan
 
 
@@ -140,6 +142,12 @@ class Runner:
         self.launches_per_step = 1 + (1 if (self.obst and wl.N > 1) else 0)
         self.kernel, self.grid, self.block = self.sim.describe_launch()
         self.planner = name == "mppi"
+        self.grad = name == "grad"
+        if self.grad:         # one cf_grad launch per step; nothing else moves
+            self.loss = torch.empty(wl.MN, dtype=torch.float32, device=device)
+            self.gout = torch.empty((wl.n_cmds, wl.MN, 4), dtype=torch.float32, device=device)
+            self.kernel = "grad_kernel<FP,INTEG_RK4,IF_ATTITUDE>"
+            self.block, self.grid = 128, -(-wl.MN // 128)
         if self.planner:      # planning iteration: broadcast reset + fused rollout + update (2 kernels per step)
             n = wl.notes
             self.mpar = self.sim.mppi_params(n["horizon"], wl.cmd_hold, n["n_elite"], n["lam"], n["shift"])
@@ -157,6 +165,11 @@ class Runner:
                 self.info_pin = torch.empty(4 * wl.notes["n_ctrl"] + 4, dtype=torch.float32, pin_memory=True)
             self.h2d = self.cmds_pin.numel() * 4 + (0 if self.bstate is None else self.bstate.numel() * 4)
             self.d2h = (self.rec_pin.numel() * 4 if n_rec else self.state_pin.numel() * 4) + (wl.M * 4 if self.obst else 0)
+            if self.grad:
+                self.loss_pin = torch.empty(wl.MN, dtype=torch.float32, pin_memory=True)
+                self.gout_pin = torch.empty((wl.n_cmds, wl.MN, 4), dtype=torch.float32, pin_memory=True)
+                self.h2d = self.cmds_pin.numel() * 4
+                self.d2h = self.loss_pin.numel() * 4 + self.gout_pin.numel() * 4
             if self.planner:
                 self.h2d = self.bstate.numel() * 4
                 self.d2h = self.plan_pin.numel() * 4 + self.info_pin.numel() * 4
@@ -166,6 +179,9 @@ class Runner:
         if self.planner:
             sim.mppi_iterate(self.mpar, self.bstate, self.cmds)
             return
+        if self.grad:
+            sim.grad(self.cmds, wl.n_steps, wl.notes["goal"], cmd_hold=wl.cmd_hold, loss=self.loss, grad=self.gout)
+            return
         if self.bstate is not None:
             sim.set_state(self.bstate, broadcast=True)
         sim.step(self.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every, record=self.record)
@@ -174,6 +190,8 @@ class Runner:
 
     def rollout_only(self):
         wl = self.wl
+        if self.grad:
+            return self.step()
         if self.bstate is not None:
             self.sim.set_state(self.bstate, broadcast=True)      # lazy: folded into the rollout launch
         self.sim.step(self.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every, record=self.record)
@@ -182,6 +200,13 @@ class Runner:
         """The same step through the C ABI with HOST buffers: H2D of this step's inputs and D2H of its results
         (records, or final state + min distance when nothing is recorded) inside the call."""
         wl, sim = self.wl, self.sim
+        if self.grad:         # commands in, loss + gradient out (torch copies around the device call: cf_grad has no
+            self.cmds.copy_(self.cmds_pin, non_blocking=True)         # host-buffer variant)
+            self.step()
+            self.loss_pin.copy_(self.loss, non_blocking=True)
+            self.gout_pin.copy_(self.gout, non_blocking=True)
+            self.torch.cuda.synchronize()
+            return
         if self.planner:      # measured state in (52 B), plan + controller scores out; the nominal stays on the device
             sim.mppi_iterate_host(self.mpar, self.bstate_pin, self.cmds, self.plan_pin, self.info_pin)
             return
@@ -281,6 +306,8 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
         cfo.set_num_threads(threads)
     if name == "mppi":
         return oracle_sample_mppi(target_seconds)
+    if name == "grad":
+        return oracle_sample_grad(target_seconds)
     small = dict(cfg1=dict(M=1, n_steps=1000), cfg2=dict(M=64, n_steps=200), cfg3=dict(M=512, n_steps=100),
                  cfg3b=dict(M=512, n_steps=100), cfg4=dict(M=1, N=512, n_steps=100), cfg5=dict(M=64, n_steps=200),
                  cfg5e=dict(M=64, n_steps=200))[name]
@@ -305,6 +332,26 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
     rate, wl = run(kw)
     sample = f"{wl.M} worlds x {wl.N} drones x {wl.n_steps} steps of {name} (same recipe, reduced M)"
     return rate, cfo.num_threads(), sample, wl
+
+
+def oracle_sample_grad(target_seconds):
+    """The gradient oracle as it stands (161 forward runs of the float64 step per batch) on a reduced number of worlds."""
+    from oracle import cfo, grad as ograd
+    from paper_2606_01478_b200 import workloads as W
+
+    def run(M):
+        wl = W.grad(M=M)
+        sim = cfo.OracleSim(wl.M, 1, wl.model, wl.params)
+        sim.reset(wl.seed)
+        t0 = time.perf_counter()
+        ograd.value_and_grad(sim, wl.cmds, wl.n_steps, wl.cmd_hold, wl.notes["goal"])
+        return wl.drone_steps / (time.perf_counter() - t0), wl
+
+    rate, wl = run(256)
+    M = int(min(1 << 20, max(256, rate * target_seconds / wl.n_steps)))
+    rate, wl = run(M)
+    return rate, cfo.num_threads(), (f"{wl.M} worlds x {wl.n_steps} steps of grad: value and gradient w.r.t. 40 inputs by "
+                                     f"Richardson central differences (same recipe, fewer worlds)"), wl
 
 
 def oracle_sample_mppi(target_seconds):
@@ -426,7 +473,7 @@ def main():
     main_res = measure(name, args.steps, args.warmup, not args.no_e2e)
     others = {}
     if not args.no_others and world == 1:
-        for nm in ("mppi", "cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"):
+        for nm in ("grad", "mppi", "cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"):
             if nm == name:
                 continue
             r = measure(nm, 5, 3, False)
@@ -447,6 +494,10 @@ def main():
                                 l2="flushed between timed steps (256 MiB write)", parallelism=f"worlds sharded x{world}, no collective"),
                     roofline=main_res["roofline"], cpu_baseline=cpu, e2e=main_res.get("e2e"), clocks=main_res["clocks"],
                     gpu_launches=main_res["gpu_launches"], workloads=others)
+        if name == "grad":      # the paper's unit for Fig. 3D: one gradient = dL/d(all commands) of one world through n steps
+            line["config"]["world_gradients_per_sec"] = main_res["value"] / main_res["sub_steps"]
+        if name == "mppi":      # plans per second (the paper's requirement: 50 Hz)
+            line["config"]["plans_per_sec"] = 1e3 / main_res["ms_per_step"]
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -120,7 +120,11 @@ __device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const floa
                                                   float *g_q, float *g_w, float *g_cmd, float *g_iR) {
   float R[3][3], Rd[3][3];
   quat_to_R(q, R);
-  euler_to_R(cmd[0], cmd[1], cmd[2], Rd);
+  float sr, cr, sp, cp, sy, cy;                                   // one evaluation serves Rd and its angle derivatives
+  sincosf(cmd[0], &sr, &cr); sincosf(cmd[1], &sp, &cp); sincosf(cmd[2], &sy, &cy);
+  Rd[0][0] = cy * cp; Rd[0][1] = cy * sp * sr - sy * cr; Rd[0][2] = cy * sp * cr + sy * sr;      // reading R13, as euler_to_R
+  Rd[1][0] = sy * cp; Rd[1][1] = sy * sp * sr + cy * cr; Rd[1][2] = sy * sp * cr - cy * sr;
+  Rd[2][0] = -sp;     Rd[2][1] = cp * sr;                Rd[2][2] = cp * cr;
   auto Mij = [&](int i, int j) { return Rd[0][i] * R[0][j] + Rd[1][i] * R[1][j] + Rd[2][i] * R[2][j]; };
   float eR[3] = { 0.5f * (Mij(2, 1) - Mij(1, 2)), 0.5f * (Mij(0, 2) - Mij(2, 0)), 0.5f * (Mij(1, 0) - Mij(0, 1)) };
   float pre[3], iRn[3], tau[3];
@@ -176,8 +180,6 @@ __device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const floa
   g_q[2] += 2.0f * (x * (GR[0][2] + GR[2][0]) + y * (GR[1][2] + GR[2][1]) + ww * (GR[1][0] - GR[0][1])) - 4.0f * z * (GR[0][0] + GR[1][1]);
   g_q[3] += 2.0f * (x * (GR[2][1] - GR[1][2]) + y * (GR[0][2] - GR[2][0]) + z * (GR[1][0] - GR[0][1]));
   // Rd = Rz(yaw) Ry(pitch) Rx(roll): d/droll rotates columns 1, 2; d/dyaw rotates rows 0, 1; d/dpitch written out
-  float sr, cr, sp, cp, sy, cy;
-  sincosf(cmd[0], &sr, &cr); sincosf(cmd[1], &sp, &cp); sincosf(cmd[2], &sy, &cy);
   g_cmd[0] += GD[0][1] * Rd[0][2] - GD[0][2] * Rd[0][1] + GD[1][1] * Rd[1][2] - GD[1][2] * Rd[1][1] + GD[2][1] * Rd[2][2] - GD[2][2] * Rd[2][1];
   g_cmd[1] += GD[0][0] * (-cy * sp) + GD[0][1] * (cy * cp * sr) + GD[0][2] * (cy * cp * cr)
             + GD[1][0] * (-sy * sp) + GD[1][1] * (sy * cp * sr) + GD[1][2] * (sy * cp * cr)
@@ -285,10 +287,13 @@ __device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MO
 
 // history record of one step: pre-step state, and for the first-principles model the controller integral before the
 // step's tick and the rotor command the step integrated with
+#ifndef GRAD_MIN_BLOCKS
+#define GRAD_MIN_BLOCKS 4
+#endif
 template <int MODEL> struct Hist { static constexpr int HD = MODEL == MODEL_FP ? 17 + 3 + 4 : 13; };
 
 template <int MODEL, int INTEG, int IFACE>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, GRAD_MIN_BLOCKS)
 grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParams P, int randp) {
   constexpr int D = Dim<MODEL>::D, HD = Hist<MODEL>::HD;
   constexpr bool FP = MODEL == MODEL_FP;

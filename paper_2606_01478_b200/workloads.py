@@ -211,7 +211,17 @@ def mppi(seed=REPORT_SEED, n_ctrl=5, worlds_per_ctrl=100_000, horizon=25, cmd_ho
                     notes=dict(horizon=horizon, n_elite=n_elite, lam=0.5, shift=1, n_ctrl=n_ctrl))
 
 
-REGISTRY = {"mppi": mppi, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
+def grad(seed=REPORT_SEED, M=1 << 20, n_steps=10, host_cmds=True) -> Workload:
+    """Fig. 3D: 2^20 worlds, first-principles model + attitude controller, RK4, the goal distance
+    after 10 steps differentiated w.r.t. the 10 attitude commands."""
+    cmds = _attitude_cmds(_rng(seed, 6), n_steps, M, 0.2, 0.2, 0.35) if host_cmds else None
+    return Workload("grad", M, 1, MODEL_FP,
+                    dict(integrator=RK4, iface=IF_ATTITUDE, f_phys=1000.0, f_att=500.0, init_mode=1,
+                         p0_lo=[-1, -1, 0], p0_hi=[1, 1, 2], tilt0_max=0.4),
+                    seed, n_steps, 1, 0, cmds, notes=dict(goal=[0.5, -0.2, 1.2]))
+
+
+REGISTRY = {"grad": grad, "mppi": mppi, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
 
 
 def make(name: str, **kw) -> Workload:
