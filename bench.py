@@ -29,8 +29,9 @@ DEFAULT_WORKLOAD = "cfg3"
 # Algorithmic FP32 operations per drone-step: every add / sub / mul / div / sqrt /
 # trig / log / min / max / clip of the float64 oracle's formulas counts 1 (an FMA is 2); Philox integer work is not
 # counted.  Controller ticks are amortised over their period.
-ALGO_FLOPS = {"grad": 2120, "mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
-BOUND = {"grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
+ALGO_FLOPS = {"depth": 4096 * 555,      # per frame: 64 x 64 rays x (16 spheres x 14 + 16 boxes x 19 + plane, direction 27)
+               "grad": 2120, "mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
+BOUND = {"depth": "alu", "grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
 SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of the rollout kernel, one launch, from the `ncu --set full` captures
 # summarised in profiles/r1_<workload>_rollout.md (static: ncu never runs inside bench.py)
@@ -61,6 +62,9 @@ def algo_bytes_per_launch(wl) -> int:
     resident = 2 * (wl.D + ctrl_planes) * 4 * MN + (2 * 8 * 4 * MN if wl.params.get("n_obstacles") else 0)
     wparam = (14 if wl.model == 0 else 11) * 4 * wl.M
     plan = (4 + 2 + 1) * 4 * MN if wl.params.get("cost_on") else 0       # eps, cost (running, total), min distance out
+    if wl.name == "depth":    # images out, poses in
+        sc = wl.notes["scene"]
+        return 4 * MN * sc["width"] * sc["height"] + 7 * 4 * MN
     if wl.name == "grad":     # planes in once, history out and back in, commands in, gradient + loss out
         return (wl.D + 7) * 4 * MN + 2 * wl.n_steps * 24 * 4 * MN + 2 * wl.n_cmds * 16 * MN + 4 * MN
     return cmd + rec + resident + wparam + plan
@@ -117,6 +121,8 @@ class Runner:
         from paper_2606_01478_b200 import cf, workloads as W
         self.torch, self.name = torch, name
         host_cmds = name != "cfg3b"
+        if name == "depth":
+            return self._init_depth(W.make(name), device, cf, e2e)
         wl = W.make(name, **({} if host_cmds else dict(host_cmds=False)))
         self.wl = wl
         prm = dict(wl.params, world_offset=rank * wl.M)          # disjoint global worlds per rank (weak scaling)
@@ -174,8 +180,31 @@ class Runner:
                 self.h2d = self.bstate.numel() * 4
                 self.d2h = self.plan_pin.numel() * 4 + self.info_pin.numel() * 4
 
+    def _init_depth(self, wl, device, cf, e2e):
+        """PAPER.md:L71 workload: one cf_depth launch per step renders every environment's 64 x 64 depth image."""
+        torch = self.torch
+        self.wl, self.planner, self.grad, self.depth = wl, False, False, True
+        self.sim = cf.Sim(wl.M, 1, wl.model, wl.params, device=device)
+        self.sim.reset(wl.seed)
+        sc = wl.notes["scene"]
+        self.dp = self.sim.depth_params(**sc)
+        self.img = torch.empty((wl.M, sc["height"], sc["width"]), dtype=torch.float32, device=device)
+        self.rays = wl.M * sc["height"] * sc["width"]
+        self.kernel, self.block, self.grid = "depth_kernel", 256, wl.M * -(-sc["height"] * sc["width"] // 256)
+        self.launches_per_step, self.record, self.obst, self.bstate = 1, None, False, None
+        self.e2e_ok = e2e
+        if e2e:
+            self.img_pin = torch.empty(self.img.shape, dtype=torch.float32, pin_memory=True)
+            self.state_pin = self.sim.get_state().cpu().pin_memory()
+            self.h2d, self.d2h = self.state_pin.numel() * 4, self.img_pin.numel() * 4
+
+    depth = False
+
     def step(self):
         wl, sim = self.wl, self.sim
+        if self.depth:
+            sim.depth(self.dp, out=self.img)
+            return
         if self.planner:
             sim.mppi_iterate(self.mpar, self.bstate, self.cmds)
             return
@@ -190,7 +219,7 @@ class Runner:
 
     def rollout_only(self):
         wl = self.wl
-        if self.grad:
+        if self.grad or self.depth:
             return self.step()
         if self.bstate is not None:
             self.sim.set_state(self.bstate, broadcast=True)      # lazy: folded into the rollout launch
@@ -200,6 +229,12 @@ class Runner:
         """The same step through the C ABI with HOST buffers: H2D of this step's inputs and D2H of its results
         (records, or final state + min distance when nothing is recorded) inside the call."""
         wl, sim = self.wl, self.sim
+        if self.depth:        # poses in (the state planes), images out
+            sim.set_state(self.state_pin.to(self.img.device, non_blocking=True))
+            sim.depth(self.dp, out=self.img)
+            self.img_pin.copy_(self.img, non_blocking=True)
+            self.torch.cuda.synchronize()
+            return
         if self.grad:         # commands in, loss + gradient out (torch copies around the device call: cf_grad has no
             self.cmds.copy_(self.cmds_pin, non_blocking=True)         # host-buffer variant)
             self.step()
@@ -308,6 +343,8 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
         return oracle_sample_mppi(target_seconds)
     if name == "grad":
         return oracle_sample_grad(target_seconds)
+    if name == "depth":
+        return oracle_sample_depth(target_seconds)
     small = dict(cfg1=dict(M=1, n_steps=1000), cfg2=dict(M=64, n_steps=200), cfg3=dict(M=512, n_steps=100),
                  cfg3b=dict(M=512, n_steps=100), cfg4=dict(M=1, N=512, n_steps=100), cfg5=dict(M=64, n_steps=200),
                  cfg5e=dict(M=64, n_steps=200))[name]
@@ -332,6 +369,28 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
     rate, wl = run(kw)
     sample = f"{wl.M} worlds x {wl.N} drones x {wl.n_steps} steps of {name} (same recipe, reduced M)"
     return rate, cfo.num_threads(), sample, wl
+
+
+def oracle_sample_depth(target_seconds):
+    """The numpy depth oracle as it stands on a reduced number of environments (frames per second)."""
+    import numpy as np
+    from oracle import cfo, depth as odepth
+    from paper_2606_01478_b200 import workloads as W
+
+    def run(M):
+        wl = W.depth(M=M)
+        sim = cfo.OracleSim(wl.M, 1, wl.model, wl.params)
+        sim.reset(wl.seed)
+        sc = wl.notes["scene"]
+        st = sim.get_state()
+        t0 = time.perf_counter()
+        odepth.render(st, wl.model, sc["width"], sc["height"], sc["fov_x"], spheres=sc["spheres"], boxes=sc["boxes"],
+                      ground_plane=sc["ground_plane"], cam_offset=sc["cam_offset"], t_max=sc["t_max"])
+        return wl.M / (time.perf_counter() - t0), wl
+
+    rate, wl = run(8)
+    rate, wl = run(int(min(1024, max(8, rate * target_seconds))))
+    return rate, 1, f"{wl.M} environments x 64 x 64 rays of depth (same scene, fewer environments; numpy, one thread)", wl
 
 
 def oracle_sample_grad(target_seconds):
@@ -473,7 +532,7 @@ def main():
     main_res = measure(name, args.steps, args.warmup, not args.no_e2e)
     others = {}
     if not args.no_others and world == 1:
-        for nm in ("grad", "mppi", "cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"):
+        for nm in ("depth", "grad", "mppi", "cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"):
             if nm == name:
                 continue
             r = measure(nm, 5, 3, False)
@@ -496,6 +555,9 @@ def main():
                     gpu_launches=main_res["gpu_launches"], workloads=others)
         if name == "grad":      # the paper's unit for Fig. 3D: one gradient = dL/d(all commands) of one world through n steps
             line["config"]["world_gradients_per_sec"] = main_res["value"] / main_res["sub_steps"]
+        if name == "depth":     # the paper's unit: frames per second; a "drone-step" here is one frame
+            line["metric"], line["unit"] = "depth_frames_per_sec", "frames/s"
+            line["config"]["rays_per_sec"] = main_res["value"] * 4096
         if name == "mppi":      # plans per second (the paper's requirement: 50 Hz)
             line["config"]["plans_per_sec"] = 1e3 / main_res["ms_per_step"]
         print(json.dumps(line))

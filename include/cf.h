@@ -254,6 +254,28 @@ size_t cf_grad_scratch_bytes(const cf_sim *sim, int n_steps);
 int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
             float *loss_dev, void *grad_dev, void *scratch_dev, size_t scratch_bytes);
 
+/* ---- Batched depth ray casting -------------------------------------------------------------
+ * "parallel rendering of depth images ... 350k frames per second at a 64x64 ray resolution across 1,024 environments".
+ * The paper inherits this from MJX's ray-cast pipeline; its camera model and test scene (MuJoCo XML) are not available, so
+ * this is reading R34 on a synthetic scene.  For every drone i (from the CURRENT state planes):
+ *   camera origin o = p_i + R_i cam_offset; optical axis = body +x, image right = body -y, image down = body -z;
+ *   pixel (row v, column u): d = R_i normalise(1, -(u + 1/2 - W/2) s, -(v + 1/2 - H/2) s),  s = 2 tan(fov_x/2) / W;
+ *   depth_dev[i][v][u] = smallest t in (0, t_max] with o + t d on a sphere, an axis-aligned box or the plane z = 0
+ *   (distance along the unit ray; a ray starting inside a primitive hits it from the inside), or -1 if there is none.
+ * The scene is shared by all worlds.  One kernel launch, thread = ray; arithmetic only (no graphics API). */
+#define CF_DEPTH_MAX_PRIMS 32
+typedef struct cf_depth_params {
+  uint32_t struct_size;
+  int32_t  width, height;
+  int32_t  n_spheres, n_boxes, ground_plane;
+  float    fov_x;                               /* horizontal field of view [rad], (0, 3.1) */
+  float    t_max;                               /* <= 0: unlimited */
+  float    cam_offset[3];                       /* camera position in the body frame [m] */
+  float    spheres[CF_DEPTH_MAX_PRIMS][4];      /* cx cy cz r */
+  float    boxes[CF_DEPTH_MAX_PRIMS][6];        /* cx cy cz hx hy hz (half extents) */
+} cf_depth_params;
+int cf_depth(cf_sim *sim, const cf_depth_params *dp, float *depth_dev /* [MN][height][width] */);
+
 const char *cf_last_error(void);
 /* Host-side Philox4x32-10 of this library, for the bit-exact check against the oracle's (C9). */
 int cf_debug_philox(uint64_t seed, const uint32_t ctr[4], uint32_t out[4]);

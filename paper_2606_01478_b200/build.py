@@ -8,7 +8,7 @@ from concurrent.futures import ThreadPoolExecutor
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libcf.so")
-SOURCES = ["cf_api.cu", "cf_rollout_fp.cu", "cf_rollout_ab.cu", "cf_mppi.cu", "cf_grad.cu"]
+SOURCES = ["cf_api.cu", "cf_rollout_fp.cu", "cf_rollout_ab.cu", "cf_mppi.cu", "cf_grad.cu", "cf_depth.cu"]
 HEADERS = [os.path.join(CSRC, "cf_device.cuh"), os.path.join(CSRC, "cf_internal.h"),
            os.path.join(os.path.dirname(_HERE), "include", "cf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

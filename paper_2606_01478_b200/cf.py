@@ -57,6 +57,16 @@ class MppiParams(C.Structure):
                 ("shift", C.c_int32), ("lam", f)]
 
 
+DEPTH_MAX_PRIMS = 32
+
+
+class DepthParams(C.Structure):
+    """Mirror of `cf_depth_params` (include/cf.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("width", C.c_int32), ("height", C.c_int32), ("n_spheres", C.c_int32),
+                ("n_boxes", C.c_int32), ("ground_plane", C.c_int32), ("fov_x", f), ("t_max", f), ("cam_offset", f * 3),
+                ("spheres", (f * 4) * DEPTH_MAX_PRIMS), ("boxes", (f * 6) * DEPTH_MAX_PRIMS)]
+
+
 class CfError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"cf status {code}: {msg}")
@@ -104,6 +114,7 @@ def lib():
         "cf_mppi_iterate_host": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, vp, sz]),
         "cf_grad_scratch_bytes": (sz, [vp, C.c_int]),
         "cf_grad": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float * 3), vp, vp, vp, sz]),
+        "cf_depth": (C.c_int, [vp, C.POINTER(DepthParams), vp]),
         "cf_last_error": (C.c_char_p, []),
         "cf_debug_philox": (C.c_int, [C.c_uint64, C.POINTER(C.c_uint32 * 4), C.POINTER(C.c_uint32 * 4)]),
         "cf_debug_philox_dev": (C.c_int, [vp, C.c_uint64, vp, C.c_int, vp, vp, vp]),
@@ -120,7 +131,7 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_get_state", "cf_get_state_host", "cf_get_aux", "cf_get_aux_host", "cf_step_counter", "cf_sync_counters",
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
            "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host", "cf_grad_scratch_bytes",
-           "cf_grad"]
+           "cf_grad", "cf_depth"]
 
 
 def _check(rc: int):
@@ -337,6 +348,34 @@ class Sim:
         assert e is None or e.numel() == 4 * self.MN
         assert c is None or c.numel() == self.MN
         _check(lib().cf_set_plan_state(self._h, _dptr(e), _dptr(c)))
+
+    # -- depth ray casting (cf_depth) ------------------------------------------------------------------------------
+    def depth_params(self, width: int, height: int, fov_x: float, spheres=(), boxes=(), ground_plane=False,
+                     cam_offset=(0.0, 0.0, 0.0), t_max=0.0) -> DepthParams:
+        dp = DepthParams()
+        dp.struct_size = C.sizeof(DepthParams)
+        dp.width, dp.height, dp.fov_x, dp.t_max, dp.ground_plane = int(width), int(height), float(fov_x), float(t_max), int(ground_plane)
+        sp = np.asarray(spheres, dtype=np.float32).reshape(-1, 4)
+        bx = np.asarray(boxes, dtype=np.float32).reshape(-1, 6)
+        dp.n_spheres, dp.n_boxes = len(sp), len(bx)
+        if len(sp) > DEPTH_MAX_PRIMS or len(bx) > DEPTH_MAX_PRIMS:
+            raise ValueError("too many primitives")
+        for r, row in enumerate(sp):
+            for c_, v in enumerate(row):
+                dp.spheres[r][c_] = float(v)
+        for r, row in enumerate(bx):
+            for c_, v in enumerate(row):
+                dp.boxes[r][c_] = float(v)
+        for j in range(3):
+            dp.cam_offset[j] = float(cam_offset[j])
+        return dp
+
+    def depth(self, dp: DepthParams, out=None):
+        """Depth images [MN][H][W] (device tensor) of every drone's camera at the current state."""
+        if out is None:
+            out = _torch().empty((self.MN, dp.height, dp.width), dtype=_torch().float32, device=self.device)
+        _check(lib().cf_depth(self._h, C.byref(dp), _dptr(out)))
+        return out
 
     # -- gradient of the goal distance w.r.t. the commands (cf_grad) --------------------------------------------------
     def grad(self, cmds, n_steps: int, goal, cmd_hold: int = 1, loss=None, grad=None):

@@ -221,7 +221,25 @@ def grad(seed=REPORT_SEED, M=1 << 20, n_steps=10, host_cmds=True) -> Workload:
                     seed, n_steps, 1, 0, cmds, notes=dict(goal=[0.5, -0.2, 1.2]))
 
 
-REGISTRY = {"grad": grad, "mppi": mppi, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
+def depth(seed=REPORT_SEED, M=1024, model=MODEL_FP, width=64, height=64) -> Workload:
+    """depth images, 64 x 64 rays x 1024 environments.  The paper's MuJoCo test scene is not available: a
+    synthetic room of 16 spheres, 16 axis-aligned boxes and the ground plane stands in for it; every environment's drone
+    hovers at a random pose (position box + tilt <= 0.4 rad), its camera looks along body +x."""
+    rng = _rng(seed, 7)
+    sph = np.column_stack([rng.uniform(2.0, 7.0, 16), rng.uniform(-3.0, 3.0, 16), rng.uniform(0.3, 2.5, 16),
+                           rng.uniform(0.15, 0.6, 16)])
+    box = np.column_stack([rng.uniform(2.0, 8.0, 16), rng.uniform(-3.5, 3.5, 16), rng.uniform(0.2, 2.0, 16),
+                           rng.uniform(0.1, 0.5, (16, 3))])
+    scene = dict(width=width, height=height, fov_x=1.2, spheres=sph.astype(np.float32).astype(np.float64),
+                 boxes=box.astype(np.float32).astype(np.float64), ground_plane=True, cam_offset=(0.03, 0.0, 0.0), t_max=20.0)
+    fp = model == MODEL_FP
+    return Workload("depth", M, 1, model,
+                    dict(integrator=EULER, iface=IF_ATTITUDE, f_phys=1000.0 if fp else 500.0, f_att=500.0, init_mode=1,
+                         p0_lo=[-1, -1, 0.5], p0_hi=[1, 1, 2], tilt0_max=0.4),
+                    seed, 1, 1, 0, None, notes=dict(scene=scene))
+
+
+REGISTRY = {"depth": depth, "grad": grad, "mppi": mppi, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
 
 
 def make(name: str, **kw) -> Workload:
