@@ -578,6 +578,9 @@ __device__ __forceinline__ void position_tick(const DevParams &P, const float *p
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+struct NoSmem { static constexpr bool value = false; };
+struct InSmem { static constexpr bool value = true; };
+
 // The rollout kernel.  One thread = one drone; the state, controller state, held commands and plant parameters stay
 // in registers for all n_steps; HBM is touched for command loads, recorded states and the final store only.
 template <int MODEL, int INTEG, int IFACE, int OPT>
@@ -590,6 +593,14 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   constexpr bool HAS_POS = IFACE == IF_POSITION;
   extern __shared__ __align__(128) float wp_s[];             // [NP][span] per-world parameters of this block (N > 1);
                                                              // afterwards [warps][D][32] record staging tiles
+
+  // obstacle table in shared memory for the held-command loop: one LDS.128 per sphere and step instead of two LDC.64
+  // (sm_100a takes no constant-bank operands in FFMA, and the uniform registers are taken by the Philox keys and command
+  // limits): mppi rollout 692 -> 653 us.  The flat per-step-command loop (configs[2]) is 7 % SLOWER with it (measured)
+  // and keeps reading the table from the constant bank.
+  __shared__ float4 obst_s[kMaxObst];
+  if ((OPT & OPT_OBST) && threadIdx.x < kMaxObst) obst_s[threadIdx.x] = P.obst_q[threadIdx.x];
+  if (OPT & OPT_OBST) __syncthreads();
 
   const long long MN = A.MN;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -724,7 +735,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       }
     };
     // (2)-(8) of one physics step
-    auto physics_step = [&]() {
+    auto physics_step = [&](auto obst_in_smem) {
       // (2) position controller tick
       if (HAS_POS) {
         if (pos_phase == 0) {
@@ -774,7 +785,9 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         float pp = fmaf(x[2], x[2], fmaf(x[1], x[1], x[0] * x[0]));
 #pragma unroll
         for (int j = 0; j < kMaxObst; ++j) {
-          float tq = fmaf(P.obst_q[j].z, x[2], fmaf(P.obst_q[j].y, x[1], fmaf(P.obst_q[j].x, x[0], P.obst_q[j].w)));
+          float4 oq;
+          if constexpr (decltype(obst_in_smem)::value) oq = obst_s[j]; else oq = P.obst_q[j];
+          float tq = fmaf(oq.z, x[2], fmaf(oq.y, x[1], fmaf(oq.x, x[0], oq.w)));
           md2[j] = fminf(md2[j], tq + pp);
         }
       }
@@ -821,13 +834,13 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // commands the loop is two-level and the inner loop carries no command logic (mppi rollout kernel 705 -> 691 us,
     // cfg4 +3 %); with a fresh command every step (cmd_hold == 1, configs[2]) the flat loop is 2 % faster.
     if (A.cmd_hold == 1) {
-      for (int t = 0; t < A.n_steps; ++t) { fetch_command(); physics_step(); }
+      for (int t = 0; t < A.n_steps; ++t) { fetch_command(); physics_step(NoSmem{}); }
     } else {
       for (int t = 0; t < A.n_steps;) {
         fetch_command();
         const int run = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;
         t += run;
-        for (int k = 0; k < run; ++k) physics_step();
+        for (int k = 0; k < run; ++k) physics_step(InSmem{});
       }
     }
     // final store
