@@ -35,7 +35,10 @@ BOUND = {"depth": "alu", "grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "a
 SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of the rollout kernel, one launch, from the `ncu --set full` captures
 # summarised in profiles/r1_<workload>_rollout.md (static: ncu never runs inside bench.py)
-TRAFFIC_NCU = {"cfg2": 5.9e6, "cfg3": 201.0e6, "cfg4": 2.725e9, "cfg5": 4.415e9, "cfg5e": 4.415e9}
+TRAFFIC_NCU = {"cfg2": 5.9e6, "cfg3": 99.1e6, "cfg4": 2.725e9, "cfg5": 4.415e9, "cfg5e": 4.415e9, "mppi": 30.9e6,
+               "grad": 1.680e9, "depth": 0.05e6}
+# (cfg3 / mppi / depth: below the algorithmic bytes because the written planes were still in the 126 MB L2 when the
+#  kernel ended; the figures are what DRAM saw during the launch)
 
 
 def peaks():
