@@ -146,6 +146,13 @@ int cf_set_stream(cf_sim *sim, void *cuda_stream);
  * controller integrals, set the held commands to hover, re-arm the minimum distance, s = 0.  (C9) */
 int cf_reset(cf_sim *sim, uint64_t seed);
 
+/* Continuous environment resets ("trivially handle continuous environment resets"): the worlds with
+ * mask_dev[w] != 0 (uint8 [M], device) start a new episode -- initial state re-drawn from the INIT stream keyed by
+ * episode_seed (same distributions as cf_reset), controller integrals 0, held commands = hover, minimum distance, noise
+ * chain and rollout cost re-armed -- while every other world, the per-world parameters, the step counter and the seed of
+ * the disturbance / noise streams stay untouched.  Needs a prior cf_reset. */
+int cf_reset_masked(cf_sim *sim, const uint8_t *mask_dev, uint64_t episode_seed);
+
 /* Overwrite the drone states: state_dev is [D][MN], or [D] broadcast to every drone when broadcast != 0 (the MPPI
  * "all rollouts start from the measured state" reset).  Keeps s and the world parameters; zeroes the
  * controller integrals, re-arms the minimum distance, held commands = hover.  Needs a prior cf_reset. */

@@ -375,20 +375,22 @@ void cfo_destroy(cfo_sim *S) {
   free(S->x); free(S->ctrl); free(S->wp); free(S->mind2); free(S->eps); free(S->cost); free(S);
 }
 
-static void rearm_controllers(cfo_sim *S) {
+static void rearm_drone(cfo_sim *S, int64_t i) {
   /* integrals 0, held commands = hover of the nominal model, min distance +inf (R20) */
   const cfo_params *p = &S->p;
   double wh = S->model == CFO_MODEL_FIRST_PRINCIPLES ? hover_rpm(p) : 0.0;
-  for (int64_t i = 0; i < S->MN; ++i) {
-    for (int c = 0; c < 6; ++c) S->ctrl[c * S->MN + i] = 0.0;
-    S->ctrl[6 * S->MN + i] = 0.0; S->ctrl[7 * S->MN + i] = 0.0; S->ctrl[8 * S->MN + i] = 0.0;
-    S->ctrl[9 * S->MN + i] = p->mass * p->g;
-    for (int k = 0; k < 4; ++k) S->ctrl[(10 + k) * S->MN + i] = wh;
-    for (int j = 0; j < 8; ++j) S->mind2[j * S->MN + i] = INFINITY;
-    for (int j = 0; j < 4; ++j) S->eps[j * S->MN + i] = NAN;   /* R25: the next command starts a fresh noise chain */
-    S->cost[i] = 0.0;                                          /* R27 */
-  }
+  for (int c = 0; c < 9; ++c) S->ctrl[c * S->MN + i] = 0.0;
+  S->ctrl[9 * S->MN + i] = p->mass * p->g;
+  for (int k = 0; k < 4; ++k) S->ctrl[(10 + k) * S->MN + i] = wh;
+  for (int j = 0; j < 8; ++j) S->mind2[j * S->MN + i] = INFINITY;
+  for (int j = 0; j < 4; ++j) S->eps[j * S->MN + i] = NAN;   /* R25: the next command starts a fresh noise chain */
+  S->cost[i] = 0.0;                                          /* R27 */
 }
+static void rearm_controllers(cfo_sim *S) {
+  for (int64_t i = 0; i < S->MN; ++i) rearm_drone(S, i);
+}
+
+static void reset_world_state(cfo_sim *S, uint64_t seed, int64_t w);
 
 /* C9 reset: PARAM stream (world params) + INIT stream (initial state) */
 int cfo_reset(cfo_sim *S, uint64_t seed) {
@@ -423,7 +425,33 @@ int cfo_reset(cfo_sim *S, uint64_t seed) {
       wp[10 * M + w] = p->ab_ctau * fac[11];
     }
   }
-  for (int64_t w = 0; w < M; ++w) {
+  for (int64_t w = 0; w < M; ++w) reset_world_state(S, seed, w);
+  rearm_controllers(S);
+  S->s = 0; S->att_ticks = 0; S->pos_ticks = 0; S->n_rec_total = 0;
+  memset(S->rec_table, 0, sizeof(S->rec_table));
+  S->have_state = 1;
+  return 0;
+}
+
+/* Continuous environment resets: the worlds with mask[w] != 0 start a new episode -- initial state
+ * re-drawn from the INIT stream of `episode_seed`, controllers re-armed -- while the other worlds, the per-world
+ * parameters, the step counter and the seed of the disturbance / noise streams stay as they are. */
+int cfo_reset_masked(cfo_sim *S, const uint8_t *mask, uint64_t episode_seed) {
+  if (!S || !mask) return -1;
+  if (!S->have_state) return -3;
+  for (int64_t w = 0; w < S->M; ++w) {
+    if (!mask[w]) continue;
+    reset_world_state(S, episode_seed, w);
+    for (int64_t n = 0; n < S->N; ++n) rearm_drone(S, w * S->N + n);
+  }
+  return 0;
+}
+
+/* INIT stream -> initial state of the drones of world w (C9) */
+static void reset_world_state(cfo_sim *S, uint64_t seed, int64_t w) {
+  const cfo_params *p = &S->p;
+  const int64_t N = S->N, MN = S->MN;
+  {
     int64_t wg = w + p->world_offset;
     for (int64_t n = 0; n < N; ++n) {
       int64_t i = w * N + n;
@@ -465,11 +493,6 @@ int cfo_reset(cfo_sim *S, uint64_t seed) {
       }
     }
   }
-  rearm_controllers(S);
-  S->s = 0; S->att_ticks = 0; S->pos_ticks = 0; S->n_rec_total = 0;
-  memset(S->rec_table, 0, sizeof(S->rec_table));
-  S->have_state = 1;
-  return 0;
 }
 
 int cfo_set_state(cfo_sim *S, const double *state, int broadcast) {

@@ -84,6 +84,7 @@ int  cfo_world_param_dim(int model);           /* 14 / 11 */
 int  cfo_create(cfo_sim **out, int64_t M, int64_t N, int model, const cfo_params *p);
 void cfo_destroy(cfo_sim *s);
 int  cfo_reset(cfo_sim *s, uint64_t seed);
+int  cfo_reset_masked(cfo_sim *s, const uint8_t *mask /* [M] */, uint64_t episode_seed);
 int  cfo_set_state(cfo_sim *s, const double *state, int broadcast);
 /* teacher forcing: overwrite everything a step depends on (any pointer may be NULL = keep) */
 int  cfo_set_full(cfo_sim *s, const double *state, const double *ctrl, const double *wparam,

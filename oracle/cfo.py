@@ -78,6 +78,7 @@ def lib():
         L.cfo_destroy.restype = None
         L.cfo_reset.argtypes = [vp, C.c_uint64]
         L.cfo_set_state.argtypes = [vp, vp, C.c_int]
+        L.cfo_reset_masked.argtypes = [vp, vp, C.c_uint64]
         L.cfo_set_full.argtypes = [vp, vp, vp, vp, vp, C.c_int64]
         L.cfo_set_plan_state.argtypes = [vp, vp, vp]
         L.cfo_step.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, C.c_size_t]
@@ -160,6 +161,12 @@ class OracleSim:
 
     def reset(self, seed: int):
         rc = lib().cfo_reset(self._h, seed)
+        assert rc == 0, rc
+
+    def reset_masked(self, mask, episode_seed: int):
+        m = np.ascontiguousarray(mask, dtype=np.uint8)
+        assert m.size == self.M
+        rc = lib().cfo_reset_masked(self._h, _ptr(m), int(episode_seed))
         assert rc == 0, rc
 
     def set_state(self, state, broadcast: bool = False):

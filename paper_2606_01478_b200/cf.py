@@ -96,6 +96,7 @@ def lib():
         "cf_set_stream": (C.c_int, [vp, vp]),
         "cf_reset": (C.c_int, [vp, C.c_uint64]),
         "cf_set_state": (C.c_int, [vp, vp, C.c_int]),
+        "cf_reset_masked": (C.c_int, [vp, vp, C.c_uint64]),
         "cf_set_full": (C.c_int, [vp, vp, vp, vp, vp, i64]),
         "cf_step": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, sz]),
         "cf_staging_bytes": (sz, [vp, C.c_int, C.c_int, C.c_int]),
@@ -131,7 +132,7 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_get_state", "cf_get_state_host", "cf_get_aux", "cf_get_aux_host", "cf_step_counter", "cf_sync_counters",
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
            "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host", "cf_grad_scratch_bytes",
-           "cf_grad", "cf_depth"]
+           "cf_grad", "cf_depth", "cf_reset_masked"]
 
 
 def _check(rc: int):
@@ -234,6 +235,12 @@ class Sim:
     # -- the four calls ------------------------------------------------------------------------------------------
     def reset(self, seed: int):
         _check(lib().cf_reset(self._h, int(seed)))
+
+    def reset_masked(self, mask, episode_seed: int):
+        """mask: [M] (bool / uint8, host or device): worlds that start a new episode."""
+        m = self._dev(np.asarray(mask, dtype=np.uint8) if not isinstance(mask, _torch().Tensor) else mask, _torch().uint8)
+        assert m.numel() == self.M
+        _check(lib().cf_reset_masked(self._h, _dptr(m), int(episode_seed)))
 
     def set_state(self, state, broadcast: bool = False):
         t = self._dev(state, _torch().float32)

@@ -244,10 +244,11 @@ __device__ __forceinline__ void rearm(const RearmPlanes &rp, long long MN, long 
   }
 }
 
-__global__ void reset_state_kernel(float *state, RearmPlanes rp, const __grid_constant__ ResetArgs R) {
+__global__ void reset_state_kernel(float *state, RearmPlanes rp, const uint8_t *mask, const __grid_constant__ ResetArgs R) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= R.MN) return;
   long long w = i / R.N, n = i - w * R.N;
+  if (mask != nullptr && mask[w] == 0) return;             // cf_reset_masked: this world keeps running
   uint32_t wg = (uint32_t)(w + R.world_offset), nn = (uint32_t)n;
   float pos[3], q[4] = { 0.f, 0.f, 0.f, 1.f };
   uint32_t r[4];
@@ -420,10 +421,8 @@ extern "C" int cf_set_stream(cf_sim *sim, void *cuda_stream) {
 static int grid_for(long long n, int block) { return (int)((n + block - 1) / block); }
 static RearmPlanes rearm_planes(const cf_sim *sim) { return RearmPlanes{ sim->ctrl, sim->min_d2, sim->eps, sim->cost_run }; }
 
-extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
-  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+static void fill_reset_args(const cf_sim *sim, uint64_t seed, ResetArgs &R) {
   const cf_params &p = sim->p;
-  ResetArgs R;
   memset(&R, 0, sizeof(R));
   for (int j = 0; j < 12; ++j) { R.rnd_lo[j] = p.rnd_lo[j]; R.rnd_hi[j] = p.rnd_hi[j]; }
   if (sim->model == CF_MODEL_FIRST_PRINCIPLES) {
@@ -443,13 +442,31 @@ extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
   R.hover_rpm = sim->hover_rpm; R.hover_thrust = (float)((double)p.mass * p.g);
   R.M = sim->M; R.N = sim->N; R.MN = sim->MN; R.world_offset = p.world_offset;
   R.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu); R.seed_hi = (uint32_t)(seed >> 32);
+}
+
+extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  ResetArgs R;
+  fill_reset_args(sim, seed, R);
   reset_params_kernel<<<grid_for(sim->M, 128), 128, 0, sim->stream>>>(sim->wparam, R);
-  reset_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(sim->state, rearm_planes(sim), R);
+  reset_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(sim->state, rearm_planes(sim), nullptr, R);
   set_counters_kernel<<<1, 1, 0, sim->stream>>>(sim->counters, 0u, 1);
   CF_CUDA(cudaMemsetAsync(sim->rec_table, 0, sizeof(uint32_t) * kRecTableCap, sim->stream));
   CF_CUDA(cudaGetLastError());
   sim->seed = seed; sim->s_host = 0; sim->n_rec_host = 0; sim->have_state = true;
   sim->pending_bcast = false; sim->md_valid = false; sim->cost_valid = false; sim->rearmed = true;
+  return CF_OK;
+}
+
+extern "C" int cf_reset_masked(cf_sim *sim, const uint8_t *mask_dev, uint64_t episode_seed) {
+  if (!sim || !mask_dev) return fail(CF_E_ARG, "NULL argument");
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_reset_masked needs a prior cf_reset (world parameters)");
+  { int rc = cf_materialise(sim); if (rc != CF_OK) return rc; }
+  ResetArgs R;
+  fill_reset_args(sim, episode_seed, R);
+  reset_state_kernel<<<grid_for(sim->MN, 128), 128, 0, sim->stream>>>(sim->state, rearm_planes(sim), mask_dev, R);
+  CF_CUDA(cudaGetLastError());
+  sim->md_valid = false; sim->cost_valid = false; sim->rearmed = false;
   return CF_OK;
 }
 

@@ -409,3 +409,26 @@ def test_lazy_broadcast_reset_and_fused_min_distance(cf, cfo, W):
     assert_state_close(b.get_state().cpu().numpy(), o.get_state(), wl.model, 2e-4, "second iteration")
     np.testing.assert_allclose(b.min_dist().cpu().numpy(), o.min_dist(), rtol=0, atol=1e-4)
     assert list(b.counters()) == list(o.counters())
+
+
+def test_masked_reset_matches_the_oracle(cf, cfo):
+    lo, hi = [1.0] * 12, [1.0] * 12
+    lo[0], hi[0] = 0.9, 1.1
+    ov = dict(integrator=1, iface=2, f_phys=1000.0, f_att=500.0, init_mode=1, p0_lo=[-1, -1, 0], p0_hi=[1, 1, 2],
+              tilt0_max=0.5, rnd_lo=lo, rnd_hi=hi, dist_sigma=0.004)
+    M, N = 70, 3
+    g, o = cf.Sim(M, N, 0, ov), cfo.OracleSim(M, N, 0, ov)
+    g.reset(7), o.reset(7)
+    cm = np.zeros((1, M * N, 4), dtype=np.float32); cm[..., 0] = 0.1; cm[..., 3] = 0.27
+    g.step(cm, 25, cmd_hold=25), o.step(cm, 25, cmd_hold=25)
+    mask = (np.random.default_rng(0).random(M) < 0.4).astype(np.uint8)
+    before = g.get_state().cpu().numpy()
+    g.reset_masked(mask, 99), o.reset_masked(mask, 99)
+    x, dm = g.get_state().cpu().numpy(), np.repeat(mask.astype(bool), N)
+    assert np.array_equal(x[:, ~dm], before[:, ~dm])                       # untouched worlds: bit-identical
+    assert_state_close(x[:, dm], o.get_state()[:, dm], 0, rtol=2e-6, what="masked reset (T4)")
+    assert_state_close(x[:, ~dm], o.get_state()[:, ~dm], 0, what="worlds that kept running")
+    assert np.abs(g.ctrl().cpu().numpy() - o.ctrl()).max() <= 1e-6 * W_HOVER
+    assert np.array_equal(g.counters(), o.counters()) and g.step_counter == 25
+    g.step(cm, 30, cmd_hold=30), o.step(cm, 30, cmd_hold=30)
+    assert_state_close(g.get_state().cpu().numpy(), o.get_state(), 0, what="after a masked reset")
