@@ -159,6 +159,7 @@ static void fill_dev_params(cf_sim *s) {
     } else {
       d.obst_q[j] = make_float4(0.f, 0.f, 0.f, INFINITY);
     }
+    d.obst_x[j] = d.obst_q[j].x; d.obst_y[j] = d.obst_q[j].y; d.obst_z[j] = d.obst_q[j].z;
   }
   for (int k = 0; k < 4; ++k) { d.noise_sigma[k] = p.noise_sigma[k]; d.cmd_lo[k] = p.cmd_lo[k]; d.cmd_hi[k] = p.cmd_hi[k]; }
   d.noise_beta = p.noise_beta; d.noise_gain = (float)std::sqrt(1.0 - (double)p.noise_beta * p.noise_beta);

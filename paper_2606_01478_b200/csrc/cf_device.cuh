@@ -51,6 +51,7 @@ struct DevParams {
   int   n_obst;
   float obst[kMaxObst][4];        // cx cy cz r (read-out)
   float4 obst_q[kMaxObst];        // (-2cx, -2cy, -2cz, c.c): d^2 = |p|^2 + q.(p,1); unused slots (0,0,0,+inf)
+  float obst_x[kMaxObst], obst_y[kMaxObst], obst_z[kMaxObst];   // the same -2c components as three constant-bank rows
   float noise_sigma[4], cmd_lo[4], cmd_hi[4];
   float noise_beta, noise_gain;    // R25: AR(1) coefficient and sqrt(1 - beta^2)
   float cost_goal[3], cost_hw_pos, cost_hw_vel;   // R27: h w_pos, h w_vel (running), and the read-out terms:
@@ -676,7 +677,8 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       }
       if (obst) {
 #pragma unroll
-        for (int j = 0; j < kMaxObst; ++j) md2[j] = A.min_d2[j * MN + i];
+        for (int j = 0; j < kMaxObst; ++j)      // registers hold min_t(|p|^2 - 2 c.p); |c|^2 is added back at the end
+        md2[j] = j < P.n_obst ? A.min_d2[j * MN + i] - P.obst_q[j].w : __int_as_float(0x7f800000);
       }
     }
     float Rd[3][3];
@@ -780,15 +782,16 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       ++s;
       // (7) obstacle minima (squared centre distance; the square roots are taken once, at read-out)
       if (obst) {
-        // |p - c_j|^2 = |p|^2 + (c_j.c_j - 2 c_j.p): 3 FFMA + FADD + FMNMX per sphere, constants straight from the
-        // uniform bank; unused slots hold (0,0,0,+inf) and never win the minimum
+        // |p - c_j|^2 = (|p|^2 - 2 c_j.p) + |c_j|^2, and the constant |c_j|^2 commutes with the minimum over time: the
+        // registers track min_t(|p|^2 - 2 c_j.p) with 3 FFMA + FMNMX per sphere and step, |c_j|^2 is added once when
+        // the minima leave the registers (unused slots: + inf, they never win)
         float pp = fmaf(x[2], x[2], fmaf(x[1], x[1], x[0] * x[0]));
 #pragma unroll
         for (int j = 0; j < kMaxObst; ++j) {
-          float4 oq;
-          if constexpr (decltype(obst_in_smem)::value) oq = obst_s[j]; else oq = P.obst_q[j];
-          float tq = fmaf(oq.z, x[2], fmaf(oq.y, x[1], fmaf(oq.x, x[0], oq.w)));
-          md2[j] = fminf(md2[j], tq + pp);
+          float qx, qy, qz;
+          if constexpr (decltype(obst_in_smem)::value) { const float4 oq = obst_s[j]; qx = oq.x; qy = oq.y; qz = oq.z; }
+          else { qx = P.obst_x[j]; qy = P.obst_y[j]; qz = P.obst_z[j]; }
+          md2[j] = fminf(md2[j], fmaf(qz, x[2], fmaf(qy, x[1], fmaf(qx, x[0], pp))));
         }
       }
       // (7b) running rollout cost on the post-step state (R27): h w_pos |p - goal|^2 + h w_vel |v|^2
@@ -865,7 +868,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     float d_min = __int_as_float(0x7f800000);
     if (obst) {
 #pragma unroll
-      for (int j = 0; j < kMaxObst; ++j) A.min_d2[j * MN + i] = md2[j];
+      for (int j = 0; j < kMaxObst; ++j) { md2[j] += P.obst_q[j].w; A.min_d2[j * MN + i] = md2[j]; }
       if (A.md_drone != nullptr || costing) {   // C10 read-out fused into the epilogue: min_j sqrt(min_t d2_j) - r_j
 #pragma unroll
         for (int j = 0; j < kMaxObst; ++j)
