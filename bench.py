@@ -123,6 +123,7 @@ class Runner:
         import torch
         from paper_2606_01478_b200 import cf, workloads as W
         self.torch, self.name = torch, name
+        self.rank, self.world = rank, int(os.environ.get("WORLD_SIZE", 1))
         host_cmds = name != "cfg3b"
         if name == "depth":
             return self._init_depth(W.make(name), device, cf, e2e)
@@ -209,7 +210,11 @@ class Runner:
             sim.depth(self.dp, out=self.img)
             return
         if self.planner:
-            sim.mppi_iterate(self.mpar, self.bstate, self.cmds)
+            out = sim.mppi_iterate(self.mpar, self.bstate, self.cmds)
+            if self.world > 1:      # the planner's one exchange step: all ranks agree on the best controller's plan
+                from paper_2606_01478_b200 import planner
+                self.global_plan = planner.select_global_plan(
+                    planner.pack_local_best(out["info"], out["plan"], wl.notes["n_ctrl"], self.rank))
             return
         if self.grad:
             sim.grad(self.cmds, wl.n_steps, wl.notes["goal"], cmd_hold=wl.cmd_hold, loss=self.loss, grad=self.gout)

@@ -115,7 +115,8 @@ typedef struct cf_params {
                                         eps <- beta eps + sqrt(1 - beta^2) z;  command = clip(nominal + sigma eps) */
   int32_t n_ctrl;                    /* R26: number of nominal sequences (independent controllers), >= 1;
                                         the command buffer of cf_step is then [n_ctrl][n_cmds] float4 */
-  int64_t worlds_per_ctrl;           /* controller of a world = global world index / worlds_per_ctrl (0: controller 0) */
+  int64_t worlds_per_ctrl;           /* controller of a world = LOCAL world index / worlds_per_ctrl (0: controller 0): the
+                                        buffer holds this shard's controllers; the noise is keyed by the global world */
   int32_t cost_on;                   /* R27: accumulate the rollout cost (needs N == 1) */
   float cost_goal[3];                /* running cost per step: h (w_pos |p - goal|^2 + w_vel |v|^2), post-step state */
   float cost_w_pos, cost_w_vel;

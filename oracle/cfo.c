@@ -551,7 +551,7 @@ static int step_impl(cfo_sim *S, const float *cmds, const double *cmds64, int n_
   if ((int64_t)n_cmds * cmd_hold < n_steps) return -2;
   const cfo_params *p = &S->p;
   if (p->cmd_source == CFO_CMD_NOMINAL_PLUS_NOISE && p->worlds_per_ctrl > 0 &&
-      (p->world_offset + S->M - 1) / p->worlds_per_ctrl >= p->n_ctrl) return -2;
+      (S->M - 1) / p->worlds_per_ctrl >= p->n_ctrl) return -2;
   const int D = S->D;
   const int64_t MN = S->MN, N = S->N;
   const uint32_t s0 = S->s;
@@ -595,8 +595,9 @@ static int step_impl(cfo_sim *S, const float *cmds, const double *cmds64, int n_
           const int fresh = isnan(eps[0]);
           const double gain = sqrt(1.0 - p->noise_beta * p->noise_beta);
           for (int j = 0; j < 4; ++j) eps[j] = fresh ? z[j] : p->noise_beta * eps[j] + gain * z[j];
-          /* R26: one nominal sequence per controller, controller = global world / worlds_per_ctrl */
-          const int64_t cidx = p->worlds_per_ctrl > 0 ? wg / p->worlds_per_ctrl : 0;
+          /* R26: one nominal sequence per controller of this shard, controller = local world / worlds_per_ctrl
+           * (the noise stays keyed by the GLOBAL world index wg, so a controller's rollouts do not depend on the shard) */
+          const int64_t cidx = p->worlds_per_ctrl > 0 ? w / p->worlds_per_ctrl : 0;
           const float *nom = cmds + ((size_t)cidx * (size_t)n_cmds + (size_t)k) * 4;
           for (int j = 0; j < 4; ++j)
             cmd[j] = clipd((double)nom[j] + p->noise_sigma[j] * eps[j], p->cmd_lo[j], p->cmd_hi[j]);

@@ -70,7 +70,7 @@ typedef struct cfo_params {
   double noise_sigma[4], cmd_lo[4], cmd_hi[4];
   /* planning rollouts for the MPPI / iCEM sampler (readings R25-R27) */
   double noise_beta;              /* AR(1) coefficient of the temporally correlated command noise, 0 = white */
-  int64_t worlds_per_ctrl;        /* controller of a world = global world index / worlds_per_ctrl (0: one controller) */
+  int64_t worlds_per_ctrl;        /* controller of a world = local world index / worlds_per_ctrl (0: one controller) */
   int32_t n_ctrl;                 /* number of nominal sequences in the command buffer [n_ctrl][n_cmds][4] */
   int32_t cost_on;                /* accumulate the running rollout cost */
   double cost_goal[3], cost_w_pos, cost_w_vel, cost_w_term, cost_w_obs, cost_d_safe, cost_w_coll;

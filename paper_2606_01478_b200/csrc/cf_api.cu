@@ -95,8 +95,8 @@ static int validate(long long M, long long N, int model, const cf_params *p) {
   if (!(p->noise_beta >= 0.f && p->noise_beta < 1.f)) return fail(CF_E_ARG, "noise_beta must be in [0, 1)");
   if (p->n_ctrl < 1 || p->worlds_per_ctrl < 0) return fail(CF_E_ARG, "n_ctrl >= 1 and worlds_per_ctrl >= 0");
   if (p->cmd_source == CF_CMD_NOMINAL_PLUS_NOISE && p->worlds_per_ctrl > 0 &&
-      (p->world_offset + M - 1) / p->worlds_per_ctrl >= p->n_ctrl)
-    return fail(CF_E_SHAPE, "worlds %lld.. need more than n_ctrl = %d nominal sequences", (long long)p->world_offset, p->n_ctrl);
+      (M - 1) / p->worlds_per_ctrl >= p->n_ctrl)
+    return fail(CF_E_SHAPE, "%lld worlds need more than n_ctrl = %d nominal sequences", (long long)M, p->n_ctrl);
   if (p->cost_on && N != 1) return fail(CF_E_UNSUPPORTED, "the rollout cost needs N == 1");
   if (p->world_offset < 0 || p->world_offset + M > ((long long)1 << 32)) return fail(CF_E_SHAPE, "world_offset out of range");
   return CF_OK;

@@ -71,7 +71,7 @@ struct StepArgs {
   float *eps;              // [4][MN] or nullptr: AR(1) command-noise state (kept when noise_beta != 0)
   float *cost_run;         // [MN] or nullptr: running rollout cost
   float *cost_drone;       // [MN] or nullptr: total rollout cost J (epilogue, R27)
-  long long worlds_per_ctrl;   // R26: nominal sequence of a world = cmds + (global world / worlds_per_ctrl) * n_cmds
+  long long worlds_per_ctrl;   // R26: nominal sequence of a world = cmds + (local world / worlds_per_ctrl) * n_cmds
   int n_cmds;
   Counters *counters;
   uint32_t *rec_table;     // [kRecTableCap]
@@ -753,7 +753,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     float *rec_ptr = A.record + (size_t)(lane >> 3) * MN + (i - lane) + 4 * (lane & 7);
     const bool noise = (OPT & OPT_NOISE) != 0 && P.use_noise;   // compiled in AND requested
     // next command to prefetch; in noise mode the nominal sequence of this world's controller (R26)
-    const float4 *cp = noise ? A.cmds + (A.worlds_per_ctrl > 0 ? (long long)(wg / (uint32_t)A.worlds_per_ctrl) * A.n_cmds : 0)
+    const float4 *cp = noise ? A.cmds + (A.worlds_per_ctrl > 0 ? (w / A.worlds_per_ctrl) * A.n_cmds : 0)
                              : A.cmds + i;
     const long long cstride = noise ? 1 : MN;
     int cmds_left = (A.n_steps + A.cmd_hold - 1) / A.cmd_hold;  // commands this call consumes

@@ -332,8 +332,8 @@ int check(const cf_sim *sim, const cf_mppi_params *mp) {
   const cf_params &p = sim->p;
   if (sim->N != 1 || p.cmd_source != CF_CMD_NOMINAL_PLUS_NOISE || !p.cost_on)
     return fail(CF_E_UNSUPPORTED, "the planner needs N == 1, CF_CMD_NOMINAL_PLUS_NOISE and cost_on");
-  if (p.worlds_per_ctrl < 1 || sim->M != (long long)p.n_ctrl * p.worlds_per_ctrl || p.world_offset % p.worlds_per_ctrl != 0)
-    return fail(CF_E_SHAPE, "M must equal n_ctrl * worlds_per_ctrl and world_offset be a multiple of worlds_per_ctrl");
+  if (p.worlds_per_ctrl < 1 || sim->M != (long long)p.n_ctrl * p.worlds_per_ctrl)
+    return fail(CF_E_SHAPE, "M must equal n_ctrl * worlds_per_ctrl");
   if (mp->horizon < 1 || mp->cmd_hold < 1 || 4 * (mp->horizon + 1) > kThreads) return fail(CF_E_ARG, "horizon out of range (1..255)");
   if (mp->n_elite < 1 || mp->n_elite > p.worlds_per_ctrl || mp->n_elite > 4096) return fail(CF_E_ARG, "n_elite out of range");
   if (mp->shift < 0 || mp->shift > mp->horizon) return fail(CF_E_ARG, "shift out of range");

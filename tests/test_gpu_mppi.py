@@ -235,6 +235,35 @@ def test_closed_loop_iterations_track_the_oracle_chain(cf, cfo, W, mp):
     assert g.step_counter == 5 * wl.n_steps and scores[-1] < scores[0]
 
 
+def test_a_shard_of_controllers_reproduces_its_slice_of_the_full_run(cf, W):
+    """Sharding by controllers (planner.py): rank 1 of 2 runs controllers 2, 3 with world_offset = 2 K_c and must get
+    bit-identical costs, elite sets and warm-started nominals, and packing + selecting gives the full run's plan."""
+    import torch
+    from paper_2606_01478_b200 import planner
+    full = W.mppi(seed=21, n_ctrl=4, worlds_per_ctrl=320, horizon=5, cmd_hold=3, n_elite=10)
+    nom_np = random_nominal(full, 6)
+    x0 = torch.as_tensor(full.broadcast_state.astype(np.float32), device="cuda")
+    gf = cf.Sim(full.M, 1, full.model, full.params)
+    gf.reset(full.seed)
+    nom_f = torch.as_tensor(nom_np, device="cuda")
+    of = gf.mppi_iterate(gf.mppi_params(5, 3, 10, 0.5, 1), x0, nom_f, want_elites=True)
+    cost_f, el_f, plan_f = gf.cost().cpu().numpy(), of["elites"].cpu().numpy().copy(), of["plan"].cpu().numpy().copy()
+    best_f = int(of["info"].cpu().numpy().view(np.int32)[16])
+    rows = []
+    for rank in range(2):
+        gs = cf.Sim(640, 1, full.model, dict(full.params, n_ctrl=2, world_offset=rank * 640))
+        gs.reset(full.seed)
+        nom_s = torch.as_tensor(nom_np[2 * rank:2 * rank + 2].copy(), device="cuda")
+        os_ = gs.mppi_iterate(gs.mppi_params(5, 3, 10, 0.5, 1), x0, nom_s, want_elites=True)
+        sl = slice(rank * 640, (rank + 1) * 640)
+        assert np.array_equal(gs.cost().cpu().numpy(), cost_f[sl])
+        assert np.array_equal(os_["elites"].cpu().numpy(), el_f[2 * rank:2 * rank + 2])
+        assert np.array_equal(nom_s.cpu().numpy(), nom_f.cpu().numpy()[2 * rank:2 * rank + 2])
+        rows.append(planner.pack_local_best(os_["info"], os_["plan"], 2, rank).clone())
+    win = int(torch.argmin(torch.stack(rows)[:, 0]))
+    assert int(rows[win][1]) == best_f and np.array_equal(rows[win][2:].reshape(-1, 4).cpu().numpy(), plan_f)
+
+
 def test_planner_argument_and_state_errors(cf, W):
     import torch
     wl = W.mppi(seed=9, n_ctrl=2, worlds_per_ctrl=64, horizon=4, cmd_hold=2, n_elite=4)
@@ -290,10 +319,11 @@ def test_full_size_planner_iteration_sampled_against_the_oracle(cf, cfo, W, mp):
     sample = np.concatenate([[0, 31, 32, wl.M - 1, 99_999, 100_000], rng.integers(0, wl.M, 42),
                              ref["elites"][3][:8] + 300_000])
     for w in sample:
-        o = cfo.OracleSim(1, 1, wl.model, dict(wl.params, world_offset=int(w)))
+        o = cfo.OracleSim(1, 1, wl.model, dict(wl.params, world_offset=int(w), n_ctrl=1))   # a one-world shard ...
         o.reset(wl.seed)
         o.set_state(wl.broadcast_state, broadcast=True)
-        o.step(nom_np, wl.n_steps, cmd_hold=wl.cmd_hold)
+        c = int(w) // wl.params["worlds_per_ctrl"]                                           # ... of controller c
+        o.step(nom_np[c:c + 1].copy(), wl.n_steps, cmd_hold=wl.cmd_hold)
         assert rel_state_err(state[:, w:w + 1], o.get_state()) <= 1e-4, w
         Jo = o.cost()[0]
         assert abs(cost[w] - Jo) <= 1e-4 * max(abs(Jo), 1.0), w

@@ -123,14 +123,20 @@ def test_r26_regenerated_commands_equal_the_commands_the_rollout_applied(cfo, mp
     assert np.array_equal(sim2.eps(), sim.eps())
 
 
-def test_r26_controller_index_uses_the_global_world_and_is_range_checked(cfo):
-    sim = plan_sim(cfo, 4, n_ctrl=2, worlds_per_ctrl=4, world_offset=4, noise_sigma=[0, 0, 0, 0])
+def test_r26_controller_index_is_local_to_the_shard_noise_is_global_and_the_range_is_checked(cfo):
+    sim = plan_sim(cfo, 8, n_ctrl=2, worlds_per_ctrl=4, world_offset=40, noise_sigma=[0, 0, 0, 0])
     sim.reset(1)
     nom = hover_nominal(2, 1)
-    nom[1, 0, 0] = 0.25                                        # local worlds 0..3 are global 4..7 = controller 1
+    nom[1, 0, 0] = 0.25                                        # local worlds 4..7 = this shard's controller 1
     sim.step(nom, 1, cmd_hold=1)
-    np.testing.assert_allclose(sim.ctrl()[6], 0.25)
-    bad = plan_sim(cfo, 4, n_ctrl=2, worlds_per_ctrl=4, world_offset=6)
+    np.testing.assert_allclose(sim.ctrl()[6], [0, 0, 0, 0, 0.25, 0.25, 0.25, 0.25])
+    # a shard reproduces the slice of the full run: the noise is keyed by the global world index
+    full = plan_sim(cfo, 16, n_ctrl=4, worlds_per_ctrl=4); full.reset(2)
+    part = plan_sim(cfo, 8, n_ctrl=2, worlds_per_ctrl=4, world_offset=8); part.reset(2)
+    nom4 = hover_nominal(4, 3); nom4[:, :, 1] = 0.1 * np.arange(4)[:, None]
+    full.step(nom4, 3, cmd_hold=1); part.step(nom4[2:].copy(), 3, cmd_hold=1)
+    assert np.array_equal(full.get_state()[:, 8:], part.get_state()) and np.array_equal(full.eps()[:, 8:], part.eps())
+    bad = plan_sim(cfo, 9, n_ctrl=2, worlds_per_ctrl=4)
     bad.reset(1)
     rc, _ = bad.step(nom, 1, cmd_hold=1, check=False)
     assert rc == -2
