@@ -101,11 +101,12 @@ def test_t4_reset_parity(cf, cfo, W, name):
 
 
 # ------------------------------------------------------------------------------------------------ T1 teacher-forced
+@pytest.mark.parametrize("seed", [1, 3, 20260601])
 @pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg3b", "cfg4", "cfg5", "cfg5e"])
-def test_t1_teacher_forced_single_steps(cf, cfo, W, name):
+def test_t1_teacher_forced_single_steps(cf, cfo, W, name, seed):
     """At >= 20 sampled steps (including controller-tick and command-change steps): widen the GPU's own float32
     state / controller planes / world parameters / obstacle minima, advance oracle and GPU one step, compare."""
-    wl = W.make(name, seed=1, **SMALL[name])
+    wl = W.make(name, seed=seed, **SMALL[name])
     g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
     fl, rate = floors(wl.model)
     h = 1.0 / wl.params["f_phys"]
