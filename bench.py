@@ -456,6 +456,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-others", action="store_true", help="skip the secondary workloads and the CPU baseline")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="Fig. 3B shape (PAPER.md:L63): single drone x 2^k worlds, 50 executions of 50 steps each, "
+                         "first-principles model + attitude controller, RK4; prints one JSON line with the table")
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
@@ -537,6 +540,23 @@ def main():
         torch.cuda.empty_cache()
         return out
 
+    if args.sweep:
+        from paper_2606_01478_b200 import cf, workloads as W
+        import numpy as np
+        rows = []
+        for k in range(0, 21, 2):
+            wl = W.cfg2(M=1 << k, n_steps=50)
+            sim = cf.Sim(wl.M, 1, wl.model, wl.params, device=device)
+            sim.reset(wl.seed)
+            cm = torch.from_numpy(np.ascontiguousarray(wl.cmds)).to(device)
+            ms = time_steps(lambda: sim.step(cm, 50, cmd_hold=wl.cmd_hold), torch, 50, 3, None)
+            mean, sd = float(np.mean(ms)), float(np.std(ms))
+            rows.append(dict(worlds=wl.M, ms_per_50_steps=mean, sigma_ms=sd, drone_steps_per_sec=wl.M * 50 / (mean * 1e-3)))
+            del sim
+        if rank == 0:
+            print(json.dumps(dict(sweep="FP + attitude controller, RK4 1 kHz, 50 executions x 50 steps (PAPER.md:L63 protocol), "
+                                        "state resident, no L2 flush (the paper's loop re-runs the same buffers)", rows=rows)))
+        return 0
     main_res = measure(name, args.steps, args.warmup, not args.no_e2e)
     others = {}
     if not args.no_others and world == 1:
