@@ -472,7 +472,9 @@ def main():
         full = W.make(name) if name != "cfg3b" else W.make(name, host_cmds=False)
         rates = []
         for i in range(args.warmup + args.steps):
-            r, cores, sample, wl = oracle_sample(name, target_seconds=max(2.0, 60.0 / max(1, args.steps)))
+            # the whole arm stays within a few minutes whatever K is: ~120 s of oracle time shared by the K + W steps
+            budget = min(10.0, max(0.15, 120.0 / max(1, args.steps + args.warmup)))
+            r, cores, sample, wl = oracle_sample(name, target_seconds=budget)
             if i >= args.warmup:
                 rates.append((r, wl.drone_steps))
         tot = sum(d for _, d in rates)
