@@ -252,7 +252,7 @@ int cf_mppi_iterate_host(cf_sim *sim, const cf_mppi_params *mp, const float *x0_
  *   grad_dev [n_cmds][MN] float4 receives dL_i / d cmds[k][i][0..3]  (commands beyond the last used one: 0);
  *   loss_dev [MN] receives L_i.
  * One hand-written reverse-mode kernel: forward sweep parking each step's state in scratch_dev
- * (cf_grad_scratch_bytes = n_steps * HD * MN floats, HD = 24 first-principles / 13 abstracted, 16-byte aligned), backward
+ * (cf_grad_scratch_bytes = n_steps * HD * MN floats, HD = 24 first-principles / 16 abstracted, 16-byte aligned), backward
  * sweep through normalisation, RK4 / Euler, Eqs. (1)-(4), (6) or (7)-(10), mixer and attitude controller.  Where a
  * clip of the method is active (rotor thrust / speed limits, controller integral, rotor-interface command limits) the
  * derivative is taken as 0 (reading R33); the controller tick schedule follows the global step counter.

@@ -23,7 +23,7 @@ struct GradArgs {
   const float4 *cmds;      // [n_cmds][MN]
   float4 *grad;            // [n_cmds][MN]
   float *loss;             // [MN]
-  float *hist;             // [n_steps][HD][MN]
+  float4 *hist;            // [n_steps][HD / 4][MN] float4
   long long MN, M, N;
   int n_steps, cmd_hold, n_cmds;
   uint32_t s0;
@@ -120,8 +120,9 @@ __device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const floa
                                                   float *g_q, float *g_w, float *g_cmd, float *g_iR) {
   float R[3][3], Rd[3][3];
   quat_to_R(q, R);
-  float sr, cr, sp, cp, sy, cy;                                   // one evaluation serves Rd and its angle derivatives
-  sincosf(cmd[0], &sr, &cr); sincosf(cmd[1], &sp, &cp); sincosf(cmd[2], &sy, &cy);
+  float sn[3], cs[3];                                             // one evaluation serves Rd and its angle derivatives;
+  sincos3_step(cmd, sn, cs);                                      // MUFU (abs err 5e-7): a linearisation point, not the forward value
+  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
   Rd[0][0] = cy * cp; Rd[0][1] = cy * sp * sr - sy * cr; Rd[0][2] = cy * sp * cr + sy * sr;      // reading R13, as euler_to_R
   Rd[1][0] = sy * cp; Rd[1][1] = sy * sp * sr + cy * cr; Rd[1][2] = sy * sp * cr - cy * sr;
   Rd[2][0] = -sp;     Rd[2][1] = cp * sr;                Rd[2][2] = cp * cr;
@@ -193,6 +194,10 @@ template <int MODEL, int INTEG>
 __device__ __forceinline__ void step_forward(const DevParams &P, const Plant<MODEL, 0> &pl, float *x, const float *u) {
   constexpr int D = Dim<MODEL>::D;
   const float fd[3] = { 0.f, 0.f, 0.f };
+  if constexpr (MODEL == MODEL_FP) {          // the rollout kernel's own lean step (closed-form rotor lag, factored rates)
+    integrate<MODEL_FP, INTEG, 0>(P, pl, x, u, fd);
+    return;
+  }
   float k[D];
   if constexpr (INTEG == INTEG_EULER) {
     deriv<MODEL, 0>(P, pl, x, u, fd, k);
@@ -290,7 +295,8 @@ __device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MO
 #ifndef GRAD_MIN_BLOCKS
 #define GRAD_MIN_BLOCKS 4
 #endif
-template <int MODEL> struct Hist { static constexpr int HD = MODEL == MODEL_FP ? 17 + 3 + 4 : 13; };
+// (float4 planes: a warp writes 512 contiguous bytes per plane with one STG.128 per lane; the abstracted model pads 13 -> 16)
+template <int MODEL> struct Hist { static constexpr int HD = MODEL == MODEL_FP ? 17 + 3 + 4 : 16; };
 
 template <int MODEL, int INTEG, int IFACE>
 __global__ void __launch_bounds__(128, GRAD_MIN_BLOCKS)
@@ -316,9 +322,10 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   // ---- forward sweep -----------------------------------------------------------------------------------------
   int att_phase = (int)(A.s0 % (uint32_t)P.att_div);
   for (int t = 0; t < A.n_steps; ++t) {
-    float *h = A.hist + (size_t)t * HD * MN + i;
+    float4 *h = A.hist + (size_t)t * (HD / 4) * MN + i;
+    float rec[HD];                                          // the step's record: x, [iR before the tick, rotor command]
 #pragma unroll
-    for (int j = 0; j < D; ++j) __stcs(h + j * MN, x[j]);
+    for (int j = 0; j < HD; ++j) rec[j] = j < D ? x[j] : 0.f;
     if (t % A.cmd_hold == 0) {
       float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
       cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
@@ -329,7 +336,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     }
     if (HAS_ATT) {
 #pragma unroll
-      for (int j = 0; j < 3; ++j) __stcs(h + (17 + j) * MN, iR[j]);
+      for (int j = 0; j < 3; ++j) rec[17 + j] = iR[j];
       if (att_phase == 0) {
         float Rd[3][3];
         euler_to_R(cmd[0], cmd[1], cmd[2], Rd);
@@ -339,8 +346,10 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     }
     if (FP) {
 #pragma unroll
-      for (int j = 0; j < 4; ++j) __stcs(h + (20 + j) * MN, rpm_cmd[j]);
+      for (int j = 0; j < 4; ++j) rec[20 + j] = rpm_cmd[j];
     }
+#pragma unroll
+    for (int j = 0; j < HD / 4; ++j) __stcs(h + (size_t)j * MN, make_float4(rec[4 * j], rec[4 * j + 1], rec[4 * j + 2], rec[4 * j + 3]));
     step_forward<MODEL, INTEG>(P, pl, x, FP ? rpm_cmd : cmd);
   }
   // ---- loss and its cotangent ----------------------------------------------------------------------------------
@@ -360,16 +369,22 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   float g_iR[3] = { 0, 0, 0 };          // cotangent of the controller integral
   att_phase = (int)((A.s0 + (uint32_t)A.n_steps - 1u) % (uint32_t)P.att_div);
   for (int t = A.n_steps - 1; t >= 0; --t) {
-    const float *h = A.hist + (size_t)t * HD * MN + i;
+    const float4 *h = A.hist + (size_t)t * (HD / 4) * MN + i;
+    float rec[HD];
 #pragma unroll
-    for (int j = 0; j < D; ++j) x[j] = __ldcs(h + j * MN);
+    for (int j = 0; j < HD / 4; ++j) {
+      const float4 v = __ldcs(h + (size_t)j * MN);
+      rec[4 * j] = v.x; rec[4 * j + 1] = v.y; rec[4 * j + 2] = v.z; rec[4 * j + 3] = v.w;
+    }
+#pragma unroll
+    for (int j = 0; j < D; ++j) x[j] = rec[j];
     if (t % A.cmd_hold == A.cmd_hold - 1 || t == A.n_steps - 1) {             // entering the run of command t / hold
       float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
       cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
     }
     if (FP) {
 #pragma unroll
-      for (int j = 0; j < 4; ++j) rpm_cmd[j] = __ldcs(h + (20 + j) * MN);
+      for (int j = 0; j < 4; ++j) rpm_cmd[j] = rec[20 + j];
       step_backward<MODEL, INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
     } else {
       step_backward<MODEL, INTEG>(P, pl, x, cmd, lam, g_cmd);
@@ -377,7 +392,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     if (HAS_ATT) {
       if (att_phase == 0) {
 #pragma unroll
-        for (int j = 0; j < 3; ++j) iR[j] = __ldcs(h + (17 + j) * MN);
+        for (int j = 0; j < 3; ++j) iR[j] = rec[17 + j];
         float g_prev[3];
         vjp_attitude_tick(P, x + 3, x + 10, cmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_cmd, g_prev);
 #pragma unroll
@@ -441,7 +456,7 @@ extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   if (rc != CF_OK) return rc;
   GradArgs A;
   A.state = sim->state; A.ctrl = sim->ctrl; A.wparam = sim->wparam;
-  A.cmds = (const float4 *)cmds_dev; A.grad = (float4 *)grad_dev; A.loss = loss_dev; A.hist = (float *)scratch_dev;
+  A.cmds = (const float4 *)cmds_dev; A.grad = (float4 *)grad_dev; A.loss = loss_dev; A.hist = (float4 *)scratch_dev;
   A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.n_cmds = n_cmds;
   A.s0 = (uint32_t)sim->s_host;
   for (int j = 0; j < 3; ++j) A.goal[j] = goal[j];
