@@ -194,7 +194,7 @@ class Runner:
         self.dp = self.sim.depth_params(**sc)
         self.img = torch.empty((wl.M, sc["height"], sc["width"]), dtype=torch.float32, device=device)
         self.rays = wl.M * sc["height"] * sc["width"]
-        self.kernel, self.block, self.grid = "depth_kernel", 256, wl.M * -(-sc["height"] * sc["width"] // 4096)
+        self.kernel, self.block, self.grid = "depth_kernel", 256, wl.M * (-(-sc["height"] // 16)) * (-(-sc["width"] // 16))
         self.launches_per_step, self.record, self.obst, self.bstate = 1, None, False, None
         self.e2e_ok = e2e
         if e2e:
