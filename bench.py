@@ -296,6 +296,39 @@ def time_host_steps(fn, torch, steps, warmup):
     return ts
 
 
+def time_host_steps_pipelined(make_runner, torch, steps, warmup):
+    """Two host threads, each with its own simulator, pinned buffers and CUDA stream, call the synchronous host-buffer
+    API back to back: while one call's results cross PCIe the other call's kernel runs.  Every step still moves its
+    inputs host->device and its results device->host inside the timed region; returns ms per step (wall / total steps)."""
+    import threading
+    runners, streams = [], []
+    for _ in range(2):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            R = make_runner()
+            R.sim.bind_stream(st)
+        runners.append(R); streams.append(st)
+
+    def loop(R, st, n):
+        with torch.cuda.stream(st):
+            for _ in range(n):
+                R.step_e2e()
+
+    for R, st in zip(runners, streams):
+        loop(R, st, warmup)
+    torch.cuda.synchronize()
+    th = [threading.Thread(target=loop, args=(R, st, steps)) for R, st in zip(runners, streams)]
+    t0 = time.perf_counter()
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    torch.cuda.synchronize()
+    ms = (time.perf_counter() - t0) * 1e3 / (2 * steps)
+    del runners
+    return ms
+
+
 def interactive_mode(device):
     """configs[0] in single-step-per-launch mode (north_star "interactive stepping"): 1000 launches of n_steps = 1,
     plain and as replays of one captured CUDA graph.  Returns microseconds per step (host wall clock around a
@@ -538,6 +571,11 @@ def main():
                 dist.all_reduce(et, op=dist.ReduceOp.MAX)
             out["e2e"] = dict(value=world * wl.drone_steps / (float(et.item()) * 1e-3), unit=UNIT,
                               h2d_bytes_per_step=R.h2d, d2h_bytes_per_step=R.d2h, ms_per_step=float(et.item()))
+            if world == 1 and nm in ("cfg3", "mppi", "depth"):      # double-buffered host loop (two calls in flight)
+                pms = time_host_steps_pipelined(lambda: Runner(nm, device, rank=rank, e2e=True), torch, 10, 2)
+                out["e2e"]["pipelined"] = dict(value=wl.drone_steps / (pms * 1e-3), ms_per_step=pms,
+                                               note="two host threads, each with its own simulator and stream, same "
+                                                    "synchronous host-buffer calls; value above is the single-call figure")
         del R
         torch.cuda.empty_cache()
         return out
