@@ -433,3 +433,41 @@ def test_masked_reset_matches_the_oracle(cf, cfo):
     assert np.array_equal(g.counters(), o.counters()) and g.step_counter == 25
     g.step(cm, 30, cmd_hold=30), o.step(cm, 30, cmd_hold=30)
     assert_state_close(g.get_state().cpu().numpy(), o.get_state(), 0, what="after a masked reset")
+
+
+@pytest.mark.parametrize("name", ["cfg3", "mppi"])
+def test_full_size_every_world_against_the_oracle(cf, cfo, W, name):
+    """The two planning workloads at their full bench sizes (2^20 x 100 and 500 000 x 250 drone-steps), in the bench's
+    launch configuration, with EVERY world compared: the oracle simulates the whole batch (~1 s on the host cores)."""
+    wl = W.make(name)
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold)
+    o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold)
+    worst = assert_state_close(g.get_state().cpu().numpy(), o.get_state(), wl.model, 1e-4, f"{name} full size")
+    md_g, md_o = g.min_dist().cpu().numpy(), o.min_dist()
+    assert np.abs(md_g - md_o).max() <= 1e-4 * max(1.0, np.abs(md_o).max())
+    assert np.array_equal(g.counters(), o.counters())
+    if name == "mppi":
+        Jg, Jo = g.cost().cpu().numpy().astype(np.float64), o.cost()
+        assert (np.abs(Jg - Jo) / np.maximum(np.abs(Jo), 1.0)).max() <= 1e-4
+    print(f"{name}: {wl.M} worlds x {wl.n_steps} steps, worst relative state error {worst:.2e}")
+
+
+@pytest.mark.parametrize("name", ["cfg5", "cfg5e"])
+def test_full_size_record_mode_every_world_every_100th_record(cf, cfo, W, name):
+    """configs[4] at full size in the bench's launch configuration (65 536 worlds x 1000 steps, record every step,
+    4.46 GB): every world compared at every 100th recorded step and at the end (T2: position drift <= 1e-3 m)."""
+    import torch
+    wl = W.make(name)
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    rg = g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=1)
+    ro = o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=100)
+    assert rg.shape[0] == 1000 and ro.shape[0] == 10
+    for k in range(10):
+        rk = rg[100 * k + 99].cpu().numpy()
+        assert np.abs(rk[0:3] - ro[k, 0:3]).max() <= 1e-3, (name, k)
+        assert_state_close(rk, ro[k], wl.model, 2e-3, f"{name} record {100 * k + 99}")
+    assert np.array_equal(rg[999].cpu().numpy(), g.get_state().cpu().numpy())          # last record = final state
+    assert list(g.counters()) == [1000, 500, 0, 1000]
+    del rg
+    torch.cuda.empty_cache()
