@@ -471,3 +471,18 @@ def test_full_size_record_mode_every_world_every_100th_record(cf, cfo, W, name):
     assert list(g.counters()) == [1000, 500, 0, 1000]
     del rg
     torch.cuda.empty_cache()
+
+
+def test_full_size_cfg2_every_world_every_record(cf, cfo, W):
+    """configs[1] at full size (4096 worlds x 2000 RK4 steps, 40 command segments, every 10th state recorded): all 200
+    records of all worlds against the oracle (T2-style bounds: 1e-3 m on positions, 2e-3 on the other components)."""
+    wl = W.make("cfg2")
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    rg = g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every).cpu().numpy()
+    ro = o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=wl.record_every)
+    assert rg.shape == ro.shape == (200, 17, 4096)
+    assert np.abs(rg[:, 0:3] - ro[:, 0:3]).max() <= 1e-3
+    for k in range(0, 200, 7):
+        assert_state_close(rg[k], ro[k], wl.model, 2e-3, f"cfg2 record {k}")
+    assert_state_close(g.get_state().cpu().numpy(), o.get_state(), wl.model, 2e-3, "cfg2 final")
+    assert np.array_equal(g.counters(), o.counters()) and np.array_equal(g.rec_table(), o.rec_table())
