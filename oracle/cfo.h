@@ -25,6 +25,10 @@
  * conservation laws, quaternion closed form, motor-lag closed forms, mixer round trip, tilted thrust
  * parabola, Eq.(10) linear recurrence, Philox known-answer vectors, distribution moments, brute-force
  * obstacle distance, position/attitude controller special cases, integrator order, fused == split.
+ * tests/test_oracle_pins_switches.py: disturbance step (Newton's law on a force-free body: counter, which normals,
+ * sigma, world frame, per-world mass, hold over RK4 stages, variance), PARAM slot map of both models one slot at a
+ * time, torque interface and thrust-polynomial inverse through the geometry-pinned mixing matrix, simplified
+ * abstracted model (Eq. (8) at level attitude with and without Eq. (9)).
  * The controller structure and gains (C5-C7), limits, reset distributions and stream numbering are
  * readings the paper does not print: for those, parity is pinned only by the special cases above.
  */
