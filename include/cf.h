@@ -212,7 +212,8 @@ int cf_describe_launch(const cf_sim *sim, char *buf, size_t buf_len, int *grid, 
  *   R32 plan = mean of the best controller; warm start nominal_c[t] <- mean_c[min(t + shift, H - 1)].
  * The sampled commands are never stored: the update regenerates the elites' commands from the Philox counters.
  * Requirements: N == 1, cmd_source == CF_CMD_NOMINAL_PLUS_NOISE, cost_on, M == n_ctrl * worlds_per_ctrl on this
- * shard (world_offset a multiple of worlds_per_ctrl), and the last calls on sim were a reset / cf_set_state followed by
+ * shard (a shard that is to reproduce controllers of a larger run starts at a world_offset that is a multiple of
+ * worlds_per_ctrl; nothing else depends on it), and the last calls on sim were a reset / cf_set_state followed by
  * ONE cf_step of horizon * cmd_hold steps with n_cmds == horizon (else CF_E_STATE). */
 typedef struct cf_mppi_params {
   uint32_t struct_size;

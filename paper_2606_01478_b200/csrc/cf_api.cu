@@ -99,6 +99,17 @@ static int validate(long long M, long long N, int model, const cf_params *p) {
     return fail(CF_E_SHAPE, "%lld worlds need more than n_ctrl = %d nominal sequences", (long long)M, p->n_ctrl);
   if (p->cost_on && N != 1) return fail(CF_E_UNSUPPORTED, "the rollout cost needs N == 1");
   if (p->world_offset < 0 || p->world_offset + M > ((long long)1 << 32)) return fail(CF_E_SHAPE, "world_offset out of range");
+  for (int j = 0; j < 12; ++j) {
+    if (!(p->rnd_lo[j] <= p->rnd_hi[j])) return fail(CF_E_ARG, "rnd_lo[%d] > rnd_hi[%d] (or NaN)", j, j);
+    // slots the kernels take reciprocals of: mass and inertia (both models: slot 0; FP: 1-3), motor time constant (FP: 6)
+    bool divides = j == 0 || (model == CF_MODEL_FIRST_PRINCIPLES && (j <= 3 || j == 6));
+    if (divides && !(p->rnd_lo[j] > 0.f)) return fail(CF_E_ARG, "rnd_lo[%d] must be > 0 (the slot is divided by)", j);
+  }
+  for (int j = 0; j < 4; ++j) {
+    if (!(p->cmd_lo[j] <= p->cmd_hi[j])) return fail(CF_E_ARG, "cmd_lo[%d] > cmd_hi[%d] (or NaN)", j, j);
+    if (!(p->noise_sigma[j] >= 0.f)) return fail(CF_E_ARG, "noise_sigma[%d] must be >= 0", j);
+  }
+  if (!(p->dist_sigma >= 0.f)) return fail(CF_E_ARG, "dist_sigma must be >= 0");
   return CF_OK;
 }
 
@@ -522,6 +533,7 @@ extern "C" int cf_set_plan_state(cf_sim *sim, const float *eps_dev, const float 
 extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctrl_dev, const float *wparam_dev,
                            const float *min_d2_dev, int64_t step_counter) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  if (step_counter >= ((int64_t)1 << 32)) return fail(CF_E_SHAPE, "step_counter must be < 2^32");
   { int rc = materialise(sim); if (rc != CF_OK) return rc; }
   sim->md_valid = false; sim->cost_valid = false; sim->rearmed = false;
   const size_t MN = (size_t)sim->MN;
@@ -558,7 +570,14 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
   LaunchCfg L;
   L.block = pick_block(sim->MN);
   L.grid = grid_for(sim->MN, L.block);
-  size_t smem_wp = ((sim->opt & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
+  // the kernel stages the parameter rows whenever ITS compile-time options carry OPT_RANDP and N > 1, and the
+  // dispatcher may pick a superset instantiation: size the staging area from the instantiation, not from the request
+  int opt_used = 0;
+  bool found = sim->model == CF_MODEL_FIRST_PRINCIPLES
+      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, nullptr, nullptr, nullptr, nullptr, &opt_used, true)
+      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
+  if (!found) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
+  size_t smem_wp = ((opt_used & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
   size_t smem_rec = (A && A->rec_tiled) ? sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
   L.smem = smem_wp > smem_rec ? smem_wp : smem_rec;
   L.stream = sim->stream;

@@ -486,3 +486,30 @@ def test_full_size_cfg2_every_world_every_record(cf, cfo, W):
         assert_state_close(rg[k], ro[k], wl.model, 2e-3, f"cfg2 record {k}")
     assert_state_close(g.get_state().cpu().numpy(), o.get_state(), wl.model, 2e-3, "cfg2 final")
     assert np.array_equal(g.counters(), o.counters()) and np.array_equal(g.rec_table(), o.rec_table())
+
+
+@pytest.mark.parametrize("model,integ,iface", [(1, 0, 3), (0, 0, 3), (1, 1, 2), (0, 1, 0), (0, 0, 1)])
+def test_swarms_without_randomisation_on_superset_kernels(cf, cfo, model, integ, iface):
+    """N > 1 with NO per-world randomisation and no record: the dispatcher serves these from instantiations that carry
+    OPT_RANDP (they stage the parameter rows of the block's worlds in shared memory), so the staging area must be sized
+    from the instantiation, not from the request.  Several worlds per block and a ragged tail."""
+    M, N, n = 37, 11, 24
+    prm = dict(integrator=integ, iface=iface, init_mode=1, p0_lo=[-1, -1, 0.5], p0_hi=[1, 1, 2], tilt0_max=0.3)
+    g, o = cf.Sim(M, N, model, prm), cfo.OracleSim(M, N, model, prm)
+    g.reset(4), o.reset(4)
+    rng = np.random.default_rng(1)
+    cm = np.zeros((2, M * N, 4), dtype=np.float32)
+    if iface == 3:
+        cm[..., :3] = rng.uniform(-1, 1, (2, M * N, 3)) + [0, 0, 1.2]
+        cm[..., 3] = rng.uniform(-0.4, 0.4, (2, M * N))
+    elif iface == 2:
+        cm[..., :2] = rng.uniform(-0.3, 0.3, (2, M * N, 2)); cm[..., 3] = rng.uniform(0.2, 0.35, (2, M * N))
+    elif iface == 1:
+        cm[..., :3] = rng.uniform(-2e-4, 2e-4, (2, M * N, 3)); cm[..., 3] = rng.uniform(0.2, 0.35, (2, M * N))
+    else:
+        cm[...] = rng.uniform(12000, 17000, (2, M * N, 4))
+    g.step(cm, n, cmd_hold=12), o.step(cm, n, cmd_hold=12)
+    assert_state_close(g.get_state().cpu().numpy(), o.get_state(), model, 2e-4, f"model {model} integ {integ} iface {iface}")
+    assert np.array_equal(g.counters(), o.counters())
+    g.step(cm, n, cmd_hold=12, record_every=5)          # the same simulator again WITH the tiled-record staging area
+    assert np.isfinite(g.get_state().cpu().numpy()).all()
