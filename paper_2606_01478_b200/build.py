@@ -31,6 +31,8 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    if os.environ.get("CF_LIB"):                     # an explicitly chosen library is used as it is
+        return os.environ["CF_LIB"]
     if not force and not needs_build():
         return LIB_PATH
     objdir = os.path.join(_HERE, "build")

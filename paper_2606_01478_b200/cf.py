@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcf.so")
+LIB_PATH = os.environ.get("CF_LIB") or os.path.join(_HERE, "libcf.so")    # CF_LIB: an alternative build (debug, variant)
 
 MODEL_FP, MODEL_AB = 0, 1
 EULER, RK4 = 0, 1

@@ -187,6 +187,7 @@ static int needed_opt(const cf_sim *s) {
   if (p.dist_sigma > 0.f) opt |= OPT_DIST;
   if (p.n_obstacles > 0) opt |= OPT_OBST;
   if (p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE) opt |= OPT_NOISE;
+  if (wants_eps(&p)) opt |= OPT_AR;
   if (p.cost_on) opt |= OPT_COST;
   bool extras = p.Jp != 0.f || p.Ca[0] != 0.f || p.Ca[1] != 0.f || p.Ca[2] != 0.f;
   if (s->model == CF_MODEL_FIRST_PRINCIPLES)
@@ -405,14 +406,15 @@ extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf
   s->cost_valid = false; s->rearmed = false; s->last_fresh = false; s->last_s0 = 0; s->last_n_steps = s->last_n_cmds = s->last_cmd_hold = 0;
   s->pending_bcast = false; s->md_valid = false;
   s->counters = (Counters *)(base + c.counters); s->rec_table = (uint32_t *)(base + c.rec_table);
+  s->last_rec_mode = REC_NONE;
   s->stream = 0; s->seed = 0; s->s_host = 0; s->n_rec_host = 0; s->have_state = false;
   s->hover_rpm = (float)hover_rpm_nominal(p);
   fill_dev_params(s);
   s->opt = needed_opt(s);
   const char *name = nullptr;
   bool ok = model == CF_MODEL_FIRST_PRINCIPLES
-      ? launch_fp(p->integrator, p->iface, s->opt, nullptr, nullptr, nullptr, &name, nullptr, true)
-      : launch_ab(p->integrator, p->iface, s->opt, nullptr, nullptr, nullptr, &name, nullptr, true);
+      ? launch_fp(p->integrator, p->iface, s->opt, REC_NONE, nullptr, nullptr, nullptr, &name, nullptr, true)
+      : launch_ab(p->integrator, p->iface, s->opt, REC_NONE, nullptr, nullptr, nullptr, &name, nullptr, true);
   if (!ok) { delete s; return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration"); }
   *out = s;
   return CF_OK;
@@ -556,36 +558,67 @@ extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctr
   return CF_OK;
 }
 
+// The record buffer of one cf_step call as a 2-D tensor for the TMA unit: [n_rec * D rows][MN columns] float32, box = 32
+// columns x D rows (one warp's snapshot), no swizzle, no interleave.  cuTensorMapEncodeTiled is a driver-API entry
+// point, fetched through the runtime so that the library links against libcudart only.  false = not available (the
+// caller falls back to one 4-byte store per component).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess) {
+      (void)cudaGetLastError();
+      return nullptr;
+    }
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+static bool encode_record_map(CUtensorMap *map, float *record_dev, long long MN, long long n_rec, int D) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[2] = { (cuuint64_t)MN, (cuuint64_t)(n_rec * D) };
+  const cuuint64_t strides[1] = { (cuuint64_t)MN * sizeof(float) };      // bytes, a multiple of 16 (MN % 32 == 0)
+  const cuuint32_t box[2] = { 32u, (cuuint32_t)D }, elem[2] = { 1u, 1u };
+  return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, record_dev, dims, strides, box, elem, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // launch geometry.  One wave always suffices for the paper's sizes up to ~600k drones (64 warps/SM x 148 SMs), so the
 // block size only decides how evenly the warps spread over the 148 SMs: the fewer warps per SM, the smaller the block.
 static int pick_block(long long MN) {
   const long long sms = 148, warps = (MN + 31) / 32;
   if (warps <= sms * 16) return 32;
   if (warps <= sms * 32) return 64;
-  if (warps <= sms * 64) return 128;
-  return 256;
+  return kMaxBlock;
 }
 
 static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name, int *grid, int *block) {
   LaunchCfg L;
+  const int rec_mode = A ? A->rec_mode : sim->last_rec_mode;    // a dry run describes the kernel of the last cf_step
+  if (A) sim->last_rec_mode = A->rec_mode;
   L.block = pick_block(sim->MN);
   L.grid = grid_for(sim->MN, L.block);
   // the kernel stages the parameter rows whenever ITS compile-time options carry OPT_RANDP and N > 1, and the
   // dispatcher may pick a superset instantiation: size the staging area from the instantiation, not from the request
   int opt_used = 0;
   bool found = sim->model == CF_MODEL_FIRST_PRINCIPLES
-      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, nullptr, nullptr, nullptr, nullptr, &opt_used, true)
-      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
+      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true)
+      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
   if (!found) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
   size_t smem_wp = ((opt_used & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
-  size_t smem_rec = (A && A->rec_tiled) ? sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
+  size_t smem_rec = (A && A->rec_mode == REC_TMA) ? kRecBufs * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
   L.smem = smem_wp > smem_rec ? smem_wp : smem_rec;
   L.stream = sim->stream;
   if (grid) *grid = L.grid;
   if (block) *block = L.block;
   bool ok = sim->model == CF_MODEL_FIRST_PRINCIPLES
-      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, A, &sim->dp, &L, name, nullptr, dry)
-      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, A, &sim->dp, &L, name, nullptr, dry);
+      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, A, &sim->dp, &L, name, nullptr, dry)
+      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, A, &sim->dp, &L, name, nullptr, dry);
   if (!ok) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
   return CF_OK;
 }
@@ -622,7 +655,11 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   A.cmds = (const float4 *)cmds_dev; A.record = record_dev;
   A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.world_offset = sim->p.world_offset;
   A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.record_every = record_every; A.n_rec_cap = (int)n_rec;
-  A.rec_tiled = (n_rec > 0 && sim->MN % 32 == 0 && ((uintptr_t)record_dev & 15) == 0) ? 1 : 0;
+  memset(&A.rec_map, 0, sizeof(A.rec_map));
+  A.rec_mode = n_rec > 0 ? REC_SCALAR : REC_NONE;
+  if (n_rec > 0 && sim->MN % 32 == 0 && ((uintptr_t)record_dev & 15) == 0 &&
+      encode_record_map(&A.rec_map, record_dev, sim->MN, n_rec, sim->D))
+    A.rec_mode = REC_TMA;
   A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);
   for (int r = 0; r < 10; ++r) {      // Philox key schedule: k += (0x9E3779B9, 0xBB67AE85) per round
     A.rk[2 * r] = A.seed_lo + (uint32_t)r * 0x9E3779B9u;

@@ -4,6 +4,7 @@
 // What each piece computes is defined by PAPER.md Eqs. (1)-(10) and the readings in DESIGN.md; citations are at
 // each function.  This file shares nothing with oracle/ (the float64 CPU oracle).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -12,6 +13,8 @@ namespace cf {
 constexpr int kMaxObst = 8;
 constexpr int kCtrlPlanes = 14;
 constexpr int kRecTableCap = 4096;
+constexpr int kRecBufs = 2;       // record staging tiles per warp (TMA path: one in flight, one being filled; 3 and 4
+                                  // measured no faster)
 
 // option bits of a kernel instantiation
 enum : int {
@@ -22,7 +25,8 @@ enum : int {
   OPT_EXTRAS = 16,  // full Eq. (6) (asymmetric + quadratic), thrust/torque polynomials, Eq. (5) gyro, body drag,
                     // simplified AB variant
   OPT_COST = 32,    // rollout cost for the sampling-based planner (reading R27)
-  OPT_ALL = 63
+  OPT_AR = 64,      // OPT_NOISE with temporally correlated noise (AR(1), reading R25): eps kept as simulator state
+  OPT_ALL = 127
 };
 enum : int { MODEL_FP = 0, MODEL_AB = 1 };
 enum : int { INTEG_EULER = 0, INTEG_RK4 = 1 };
@@ -79,10 +83,11 @@ struct StepArgs {
   float *record;           // [n_rec][D][MN]
   long long MN, M, N, world_offset;
   int n_steps, cmd_hold, record_every, n_rec_cap;
-  int rec_tiled;           // 1: records leave as 16-byte stores after a shared-memory transpose (needs MN % 32 == 0,
-                           //    16-byte aligned record buffer); 0: one 4-byte store per component
+  int rec_mode;            // REC_NONE / REC_SCALAR (one 4-byte store per component) / REC_TMA (bulk-tensor store of a
+                           // [D][32] shared-memory tile; needs MN % 32 == 0 and a 16-byte aligned record buffer)
   uint32_t seed_lo, seed_hi;
   uint32_t rk[20];         // Philox round keys (k0_r, k1_r), r = 0..9, precomputed on the host from the seed
+  alignas(64) CUtensorMap rec_map;   // REC_TMA: the record buffer as the 2-D tensor [n_rec * D][MN], box = 32 x D
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -491,9 +496,8 @@ __device__ __forceinline__ void integrate_fp_lean(const DevParams &P, const Plan
 // integrator (algebraically identical restatements are free), ~10 instructions fewer per step.
 template <int OPT>
 __device__ __forceinline__ void integrate_ab_euler_lean(const DevParams &P, const Plant<MODEL_AB, OPT> &pl, float *x,
-                                                        const float *held, const float *fdist) {
-  float sn[3], cs[3];
-  sincos3_step(x + 3, sn, cs);
+                                                        const float *held, const float *fdist, const float *sn,
+                                                        const float *cs) {   // sn, cs: sin / cos of the pre-step Psi
   const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
   const float t = sp * cr;
   const float zx = fmaf(cy, t, sy * sr), zy = fmaf(sy, t, -(cy * sr)), zz = cp * cr;
@@ -518,10 +522,11 @@ __device__ __forceinline__ void integrate_ab_euler_lean(const DevParams &P, cons
 // C4: explicit Euler / classical RK4, inputs held; q renormalised once per step, not inside the stages (R8-R10).
 template <int MODEL, int INTEG, int OPT>
 __device__ __forceinline__ void integrate(const DevParams &P, const Plant<MODEL, OPT> &pl, float *x, const float *u,
-                                          const float *fdist, const float *held = nullptr) {
+                                          const float *fdist, const float *held = nullptr, const float *sn = nullptr,
+                                          const float *cs = nullptr) {
   constexpr int D = MODEL == MODEL_FP ? 17 : 13;
   if constexpr (MODEL == MODEL_AB && INTEG == INTEG_EULER && !(OPT & OPT_EXTRAS)) {
-    integrate_ab_euler_lean<OPT>(P, pl, x, held, fdist);
+    integrate_ab_euler_lean<OPT>(P, pl, x, held, fdist, sn, cs);
     return;
   }
   if constexpr (MODEL == MODEL_FP && !(OPT & OPT_EXTRAS)) {
@@ -625,21 +630,48 @@ __device__ __forceinline__ void position_tick(const DevParams &P, const float *p
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Record stream through the TMA unit (cp.async.bulk.tensor, SASS UTMASTG): the caller's record buffer is the 2-D tensor
+// [n_rec * D rows][MN columns]; a warp parks its snapshot as a [D][32] tile in shared memory and ONE elected lane hands
+// the whole tile to the copy engine.  The tile is double-buffered: the warp goes on computing while the engine drains.
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_tile_2d(const void *tmap, uint32_t smem_addr, int col, int row, int pred) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+               "@p cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];\n\t"
+               "@p cp.async.bulk.commit_group;\n\t}"
+               :: "l"(tmap), "r"(col), "r"(row), "r"(smem_addr), "r"(pred) : "memory");
+}
+template <int N> __device__ __forceinline__ void tma_store_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory");
+}
+
 struct NoSmem { static constexpr bool value = false; };
 struct InSmem { static constexpr bool value = true; };
+template <int V> struct IntC { static constexpr int value = V; };
+enum : int { REC_NONE = 0, REC_SCALAR = 1, REC_TMA = 2, REC_RUNTIME = -1 };
 
 // The rollout kernel.  One thread = one drone; the state, controller state, held commands and plant parameters stay
 // in registers for all n_steps; HBM is touched for command loads, recorded states and the final store only.
-template <int MODEL, int INTEG, int IFACE, int OPT>
-__global__ void __launch_bounds__(256)
+//
+// Lean instantiations (no OPT_EXTRAS) take their compiled-in options as unconditionally ON (the dispatcher hands them
+// only requests with exactly those options; OPT_RANDP alone may be a superset, the parameter planes always hold valid
+// values) and exist once per record mode REC (separate kernels: each gets its own register allocation), so the step
+// loop carries no run-time feature test.  General instantiations (OPT_ALL, REC_RUNTIME) gate everything at run time.
+// Launch bounds (measured on B200, profiles/r2_launch_config.md): blocks of at most 128 threads; abstracted-model lean
+// kernels at >= 5 blocks / SM (<= 96 registers, 20 warps: best of 3..6 blocks and 64 / 128 / 256 threads on configs[2],
+// configs[3] and the planner); first-principles lean kernels at >= 4 blocks (<= 128 registers, so that the 2048
+// one-warp blocks of configs[4] are all resident: at > 146 registers they spill into a second wave, +50 % time).
+constexpr int kMaxBlock = 128;
+template <int MODEL, int INTEG, int IFACE, int OPT, int REC>
+__global__ void __launch_bounds__(kMaxBlock, (OPT & OPT_EXTRAS) ? 1 : (MODEL == MODEL_AB ? 5 : 4))
 rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevParams P) {
   constexpr int D = MODEL == MODEL_FP ? 17 : 13;
   constexpr int NP = MODEL == MODEL_FP ? 14 : 11;
   constexpr bool FP = MODEL == MODEL_FP;
+  constexpr bool GEN = (OPT & OPT_EXTRAS) != 0;
   constexpr bool HAS_ATT = FP && IFACE >= IF_ATTITUDE;       // attitude controller + mixer active
   constexpr bool HAS_POS = IFACE == IF_POSITION;
   extern __shared__ __align__(128) float wp_s[];             // [NP][span] per-world parameters of this block (N > 1);
-                                                             // afterwards [warps][D][32] record staging tiles
+                                                             // afterwards [warps][2][D][32] record staging tiles
 
   // obstacle table in shared memory for the held-command loop: one LDS.128 per sphere and step instead of two LDC.64
   // (sm_100a takes no constant-bank operands in FFMA, and the uniform registers are taken by the Philox keys and command
@@ -652,8 +684,13 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   const long long MN = A.MN;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const bool active = i < MN;
-  const uint32_t s0 = *((volatile uint32_t *)&A.counters->s);
-  const uint32_t rec0 = *((volatile uint32_t *)&A.counters->n_rec_total);
+  // the warp index as a value the compiler can prove warp-uniform (the TMA instruction takes uniform operands)
+  const int warp_u = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+  // the device-side counters, broadcast from lane 0 so that the compiler can prove them (and every phase counter, loop
+  // bound and record slot derived from them) warp-uniform: the step loop's control then runs on the uniform datapath
+  // and the TMA store gets its operands without a per-lane uniformisation loop
+  const uint32_t s0 = __shfl_sync(0xffffffffu, *((volatile uint32_t *)&A.counters->s), 0);
+  const uint32_t rec0 = __shfl_sync(0xffffffffu, *((volatile uint32_t *)&A.counters->n_rec_total), 0);
 
   Plant<MODEL, OPT> pl;
   long long w = 0, n = 0;
@@ -675,15 +712,23 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     pl.load(P, A.wparam, A.M, w, (OPT & OPT_RANDP) != 0);
   }
 
-  uint32_t my_att = 0, my_pos = 0;
+  // record-slot table: slot r of this call holds the state after step (s0 / record_every + 1 + r) * record_every
+  if (i == 0 && A.record_every > 0) {
+    const uint32_t first_mult = s0 / (uint32_t)A.record_every + 1u;
+    for (int r = 0; r < A.n_rec_cap && rec0 + (uint32_t)r < (uint32_t)kRecTableCap; ++r)
+      A.rec_table[rec0 + r] = (first_mult + (uint32_t)r) * (uint32_t)A.record_every;
+  }
+
   if (active) {
     float x[D];
     float iR[3] = { 0, 0, 0 }, ip[3] = { 0, 0, 0 }, att_cmd[4] = { 0, 0, 0, 0 }, rpm_cmd[4] = { 0, 0, 0, 0 };
     float target[4] = { 0, 0, 0, 0 };
     float md2[kMaxObst];
-    const bool obst = (OPT & OPT_OBST) != 0 && A.min_d2 != nullptr;
-    const bool ar = (OPT & OPT_NOISE) != 0 && A.eps != nullptr;              // temporally correlated noise (R25)
-    const bool costing = (OPT & OPT_COST) != 0 && A.cost_run != nullptr;     // R27
+    const bool obst = (OPT & OPT_OBST) != 0 && (!GEN || A.min_d2 != nullptr);
+    const bool ar = (OPT & OPT_AR) != 0 && (!GEN || A.eps != nullptr);                 // temporally correlated noise (R25)
+    const bool costing = (OPT & OPT_COST) != 0 && (!GEN || A.cost_run != nullptr);     // R27
+    const bool noise = (OPT & OPT_NOISE) != 0 && (!GEN || P.use_noise);                // compiled in AND requested
+    const bool dist = (OPT & OPT_DIST) != 0 && (!GEN || P.dist_sigma > 0.0f);
     float eps[4] = { 0, 0, 0, 0 };
     float cost = 0.0f;
     if (A.bcast != nullptr) {
@@ -747,29 +792,59 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     int rec_phase = A.record_every > 0 ? (int)(s0 % (uint32_t)A.record_every) : 0;
     int rec_slot = 0;
     const int lane = threadIdx.x & 31;
-    // record staging: the warp's snapshot is a [D][32] tile = D*8 16-byte chunks; lane L stores chunks L, L+32, ...:
-    // chunk c is row c/8 (component), columns 4(c%8)..+3 (drones), so successive chunks of a lane are 4 rows apart
-    float *rec_tile = wp_s + (threadIdx.x >> 5) * (D * 32);
-    float *rec_ptr = A.record + (size_t)(lane >> 3) * MN + (i - lane) + 4 * (lane & 7);
-    const bool noise = (OPT & OPT_NOISE) != 0 && P.use_noise;   // compiled in AND requested
-    // next command to prefetch; in noise mode the nominal sequence of this world's controller (R26)
+    // record staging (REC_TMA): the warp's snapshot is a [D][32] tile (kRecBufs of them, used in turn); one
+    // cp.async.bulk.tensor.2d of the whole tile by lane 0, box = 32 columns x D rows at (column = first drone of the
+    // warp, row = slot * D) of the [n_rec * D][MN] record tensor
+    float *rec_tile = wp_s + warp_u * (kRecBufs * D * 32);
+    const uint32_t rec_tile_sa = (uint32_t)__cvta_generic_to_shared(wp_s) + (uint32_t)warp_u * (kRecBufs * D * 128);
+    const int rec_col = (int)((long long)blockIdx.x * blockDim.x) + warp_u * 32;
+    int rec_buf = 0;
+    // commands.  Buffer mode: one float4 per drone and command, prefetched one command ahead.  Noise mode: the nominal
+    // sequence of this world's controller (R26), the same 16 bytes for (nearly) every lane: a plain indexed read-only
+    // load at the top of the step, served by L1, with the Philox rounds between it and its use.
     const float4 *cp = noise ? A.cmds + (A.worlds_per_ctrl > 0 ? (w / A.worlds_per_ctrl) * A.n_cmds : 0)
                              : A.cmds + i;
-    const long long cstride = noise ? 1 : MN;
     int cmds_left = (A.n_steps + A.cmd_hold - 1) / A.cmd_hold;  // commands this call consumes
-    float4 next_cmd = __ldg(cp);
+    int cmd_k = 0;
+    float4 next_cmd = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (!noise) next_cmd = __ldg(cp);
+    // Software-pipelined random draws.  A Philox block + Box-Muller is a ~60-instruction serial chain that depends on
+    // nothing but the counter, so the draw for the NEXT step is issued in the same basic block as this step's
+    // integration: two independent chains for the scheduler to interleave (the kernel runs at 3-4 warps per
+    // scheduler, where instruction-level parallelism inside a warp is what fills the issue slots).  zn holds the
+    // normals of the next command (flat loop: a command every step), fdn the disturbance of the next step.
+    const bool flat = A.cmd_hold == 1;
+    float zn[4] = { 0, 0, 0, 0 }, fdn[3] = { 0, 0, 0 };
+    auto draw4 = [&](uint32_t step, int stream, float *z) {
+      uint32_t r[4];
+      philox4x32_10_rk(A.rk, wg, nn, step, stream, r);
+      normal_pair(r[0], r[1], z[0], z[1]);
+      normal_pair(r[2], r[3], z[2], z[3]);
+    };
+    if (noise && flat) draw4(s0, STREAM_NOISE, zn);
+    if (dist) {
+      float z[4];
+      draw4(s0, STREAM_DIST, z);
+#pragma unroll
+      for (int j = 0; j < 3; ++j) fdn[j] = P.dist_sigma * z[j];
+    }
 
-    // (1) command fetch (prefetched one segment ahead)
-    auto fetch_command = [&]() {
+    // (1) command fetch
+    auto fetch_command = [&](auto piped_c) {
       {
-        float4 c4 = next_cmd;
-        if (--cmds_left > 0) { cp += cstride; next_cmd = __ldg(cp); }
-        float c[4] = { c4.x, c4.y, c4.z, c4.w };
+        float c[4];
         if (noise) {
-          uint32_t r[4]; float z[4];
-          philox4x32_10_rk(A.rk, wg, nn, s, STREAM_NOISE, r);
-          normal_pair(r[0], r[1], z[0], z[1]);
-          normal_pair(r[2], r[3], z[2], z[3]);
+          const float4 c4 = __ldg(cp + cmd_k);
+          ++cmd_k;
+          c[0] = c4.x; c[1] = c4.y; c[2] = c4.z; c[3] = c4.w;
+          float z[4];
+          if constexpr (decltype(piped_c)::value) {          // flat loop: drawn one step ahead; draw the next one now
+#pragma unroll
+            for (int j = 0; j < 4; ++j) z[j] = zn[j];
+            draw4(s + 1u, STREAM_NOISE, zn);
+          } else {
+            draw4(s, STREAM_NOISE, z);
+          }
           if (ar) {                                            // eps <- z (fresh chain) or beta eps + sqrt(1-beta^2) z
             const bool fresh = eps[0] != eps[0];
 #pragma unroll
@@ -777,6 +852,17 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           }
 #pragma unroll
           for (int j = 0; j < 4; ++j) c[j] = clipf(fmaf(P.noise_sigma[j], z[j], c[j]), P.cmd_lo[j], P.cmd_hi[j]);
+        } else {
+          const float4 c4 = next_cmd;
+          if (--cmds_left > 0) {
+            cp += MN;
+            next_cmd = __ldg(cp);
+            // a fresh command every step streams 16 bytes per drone and step from HBM (configs[2] variant 3B): one
+            // step of cover does not hide DRAM latency at 16 warps per SM, so the line four commands ahead is pulled
+            // into L2 now and the register prefetch above hits there
+            if (flat && cmds_left > 4) asm volatile("prefetch.global.L2 [%0];" :: "l"(cp + 4 * MN));
+          }
+          c[0] = c4.x; c[1] = c4.y; c[2] = c4.z; c[3] = c4.w;
         }
         if (IFACE == IF_ATTITUDE) {
 #pragma unroll
@@ -795,7 +881,14 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       }
     };
     // (2)-(8) of one physics step
-    auto physics_step = [&](auto obst_in_smem) {
+    auto physics_step = [&](auto obst_in_smem, auto fetch_c) {
+      const int rec_mode = REC == REC_RUNTIME ? A.rec_mode : REC;
+      // sin / cos of the pre-step Euler angles (abstracted model, lean Euler step): taken first -- its range check is the
+      // only data-dependent branch of the step -- and shared by the position tick and the integration
+      float sn[3], cs[3];
+      if constexpr (AB_LEAN) sincos3_step(x + 3, sn, cs);
+      // (1) flat loop: this step's command (formed after the sin / cos so that everything below is one basic block)
+      if constexpr (decltype(fetch_c)::value) fetch_command(IntC<1>{});
       // (2) position controller tick
       if (HAS_POS) {
         if (pos_phase == 0) {
@@ -806,38 +899,33 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
             zB[1] = 2.0f * (q[1] * q[2] - q[3] * q[0]);
             zB[2] = 1.0f - 2.0f * (q[0] * q[0] + q[1] * q[1]);
           } else {
-            float sn[3], cs[3];
-            sincos3_step(x + 3, sn, cs);
+            if constexpr (!AB_LEAN) sincos3_step(x + 3, sn, cs);
             zB[0] = cs[2] * sn[1] * cs[0] + sn[2] * sn[0]; zB[1] = sn[2] * sn[1] * cs[0] - cs[2] * sn[0];
             zB[2] = cs[1] * cs[0];
           }
           position_tick(P, x, FP ? x + 7 : x + 6, zB, target, ip, att_cmd);
           if (HAS_ATT) euler_to_R(att_cmd[0], att_cmd[1], att_cmd[2], Rd);
           fold_command();
-          ++my_pos;
         }
         pos_phase = pos_phase + 1 == P.pos_div ? 0 : pos_phase + 1;
       }
       // (3) attitude controller tick + mixer
       if (HAS_ATT) {
-        if (att_phase == 0) {
-          attitude_tick<OPT>(P, x + 3, x + 10, Rd, att_cmd[3], iR, rpm_cmd);
-          ++my_att;
-        }
+        if (att_phase == 0) attitude_tick<OPT>(P, x + 3, x + 10, Rd, att_cmd[3], iR, rpm_cmd);
         att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
       }
-      // (4) disturbance draw, held over the RK4 stages
+      // (4) disturbance of this step (drawn one step ahead, held over the RK4 stages) and the draw for the next step
       float fdist[3] = { 0, 0, 0 };
-      if ((OPT & OPT_DIST) && P.dist_sigma > 0.0f) {
-        uint32_t r[4]; float z[4];
-        philox4x32_10_rk(A.rk, wg, nn, s, STREAM_DIST, r);
-        normal_pair(r[0], r[1], z[0], z[1]);
-        normal_pair(r[2], r[3], z[2], z[3]);
+      if (dist) {
+        float z[4];
 #pragma unroll
-        for (int j = 0; j < 3; ++j) fdist[j] = P.dist_sigma * z[j];
+        for (int j = 0; j < 3; ++j) fdist[j] = fdn[j];
+        draw4(s + 1u, STREAM_DIST, z);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) fdn[j] = P.dist_sigma * z[j];
       }
       // (5) integrate, (6) count
-      integrate<MODEL, INTEG, OPT>(P, pl, x, FP ? rpm_cmd : att_cmd, fdist, held);
+      integrate<MODEL, INTEG, OPT>(P, pl, x, FP ? rpm_cmd : att_cmd, fdist, held, sn, cs);
       ++s;
       // (7) obstacle minima (squared centre distance; the square roots are taken once, at read-out)
       if (obst) {
@@ -860,33 +948,29 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         float e2 = fmaf(ez, ez, fmaf(ey, ey, ex * ex)), v2 = fmaf(v[2], v[2], fmaf(v[1], v[1], v[0] * v[0]));
         cost = fmaf(P.cost_hw_pos, e2, fmaf(P.cost_hw_vel, v2, cost));
       }
-      // (8) record (streaming stores; a warp writes whole 128-byte lines of each plane)
-      if (A.record_every > 0) {
+      // (8) record
+      if (rec_mode != REC_NONE) {
         if (++rec_phase == A.record_every) {
           rec_phase = 0;
           if (rec_slot < A.n_rec_cap) {
-            if (A.rec_tiled) {
-              __syncwarp();                           // everyone has read the previous snapshot out of the tile
-#pragma unroll
-              for (int j = 0; j < D; ++j) rec_tile[j * 32 + lane] = x[j];
+            if (rec_mode == REC_TMA) {
+              tma_store_wait_read<kRecBufs - 1>();    // the engine has read the tile written kRecBufs records ago
               __syncwarp();
-              constexpr int ROUNDS = (D * 8 + 31) / 32;
-              float *dst = rec_ptr;
+              // slot and buffer index as provably warp-uniform values (one shuffle): the TMA instruction takes its
+              // operands from uniform registers; without this the compiler wraps it in a per-lane uniformisation loop
+              const int sb = __shfl_sync(0xffffffffu, kRecBufs * rec_slot + rec_buf, 0);
+              float *t = rec_tile + (sb % kRecBufs) * (D * 32);
 #pragma unroll
-              for (int m = 0; m < ROUNDS; ++m) {
-                if (m * 32 + lane < D * 8) {
-                  float4 v = *reinterpret_cast<const float4 *>(rec_tile + (m * 32 + lane) * 4);
-                  __stcs(reinterpret_cast<float4 *>(dst), v);
-                }
-                dst += 4 * MN;
-              }
-              rec_ptr += (size_t)D * MN;
-            } else {
+              for (int j = 0; j < D; ++j) t[j * 32 + lane] = x[j];
+              fence_proxy_async_smem();               // generic-proxy writes -> visible to the async proxy
+              __syncwarp();
+              tma_store_tile_2d(&A.rec_map, rec_tile_sa + (sb % kRecBufs) * (D * 128), rec_col, (sb / kRecBufs) * D, lane == 0);
+              rec_buf = (rec_buf + 1) % kRecBufs;
+            } else {                                  // one streaming 4-byte store per component (any MN, any alignment)
               float *r = A.record + (size_t)rec_slot * D * MN + i;
 #pragma unroll
               for (int j = 0; j < D; ++j) __stcs(r + j * MN, x[j]);
             }
-            if (i == 0 && rec0 + (uint32_t)rec_slot < (uint32_t)kRecTableCap) A.rec_table[rec0 + rec_slot] = s;
           }
           ++rec_slot;
         }
@@ -895,16 +979,18 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // The call starts at a command boundary (C8), so a run of cmd_hold steps starts with ONE command fetch.  With held
     // commands the loop is two-level and the inner loop carries no command logic (mppi rollout kernel 705 -> 691 us,
     // cfg4 +3 %); with a fresh command every step (cmd_hold == 1, configs[2]) the flat loop is 2 % faster.
-    if (A.cmd_hold == 1) {
-      for (int t = 0; t < A.n_steps; ++t) { fetch_command(); physics_step(NoSmem{}); }
+    if (flat) {
+#pragma unroll 2
+      for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{});
     } else {
       for (int t = 0; t < A.n_steps;) {
-        fetch_command();
-        const int run = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;
-        t += run;
-        for (int k = 0; k < run; ++k) physics_step(InSmem{});
+        fetch_command(IntC<0>{});
+        const int run_len = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;
+        t += run_len;
+        for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{});
       }
     }
+    if (REC == REC_TMA || (REC == REC_RUNTIME && A.rec_mode == REC_TMA)) { tma_store_wait_read<0>(); __syncwarp(); }   // the tiles must outlive the engine's reads
     // final store
 #pragma unroll
     for (int j = 0; j < D; ++j) A.state[j * MN + i] = x[j];
@@ -948,20 +1034,20 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       if (d_min < 0.0f) J += P.cost_w_coll;
       A.cost_drone[i] = J;
     }
-    if (i == 0) {
-      if (my_att) atomicAdd(&A.counters->att_ticks, my_att);
-      if (my_pos) atomicAdd(&A.counters->pos_ticks, my_pos);
-    }
   }
-  // the last block to finish advances the device-side step counter (every block has read s0 by then), so that a
-  // captured CUDA graph of single-step launches replays correctly
+  // the last block to finish advances the device-side counters (every block has read s0 by then), so that a captured
+  // CUDA graph of single-step launches replays correctly.  Controller ticks happen at the steps s in [s0, s0 + n) with
+  // s % div == 0: a closed form, nothing is counted in the loop.
   if (threadIdx.x == 0) {
     __threadfence();
     uint32_t done = atomicAdd(&A.counters->blocks_done, 1u);
     if (done == gridDim.x - 1) {
-      uint32_t n_rec = A.record_every > 0
-          ? (s0 + (uint32_t)A.n_steps) / (uint32_t)A.record_every - s0 / (uint32_t)A.record_every : 0u;
-      A.counters->s = s0 + (uint32_t)A.n_steps;
+      const uint32_t s1 = s0 + (uint32_t)A.n_steps;
+      uint32_t n_rec = A.record_every > 0 ? s1 / (uint32_t)A.record_every - s0 / (uint32_t)A.record_every : 0u;
+      auto ticks = [&](uint32_t div) { return (s1 + div - 1u) / div - (s0 + div - 1u) / div; };
+      if (HAS_ATT) A.counters->att_ticks += ticks((uint32_t)P.att_div);
+      if (HAS_POS) A.counters->pos_ticks += ticks((uint32_t)P.pos_div);
+      A.counters->s = s1;
       A.counters->n_rec_total = rec0 + n_rec;
       A.counters->blocks_done = 0;
       __threadfence();
@@ -972,9 +1058,24 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
 // launch table entry points, one translation unit per model (cf_rollout_fp.cu / cf_rollout_ab.cu)
 struct LaunchCfg { int grid, block; size_t smem; cudaStream_t stream; };
 // returns false if (integ, iface, opt) has no instantiation that covers it; *name = instantiation label, *opt_used
-bool launch_fp(int integ, int iface, int opt, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
+bool launch_fp(int integ, int iface, int opt, int rec_mode, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
                const char **name, int *opt_used, bool dry);
-bool launch_ab(int integ, int iface, int opt, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
+bool launch_ab(int integ, int iface, int opt, int rec_mode, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
                const char **name, int *opt_used, bool dry);
+
+// shared by the two launch tables: the entry that serves (integ, iface, opt, rec_mode), or nullptr
+struct RolloutEntry { int integ, iface, opt, rec; const char *name; void (*fn)(const StepArgs, const DevParams); };
+inline const RolloutEntry *pick_rollout(const RolloutEntry *tab, int n, int integ, int iface, int opt, int rec_mode) {
+  const RolloutEntry *best = nullptr;
+  for (int k = 0; k < n; ++k) {
+    const RolloutEntry &e = tab[k];
+    if (e.integ != integ || e.iface != iface || (e.opt & opt) != opt) continue;
+    // a lean kernel takes its options as unconditionally on: it serves only requests with exactly its options
+    // (OPT_RANDP may be extra: the parameter planes always hold valid values) and exactly its record mode
+    if (!(e.opt & OPT_EXTRAS) && ((e.opt & ~OPT_RANDP) != (opt & ~OPT_RANDP) || e.rec != rec_mode)) continue;
+    if (!best || __builtin_popcount(e.opt) < __builtin_popcount(best->opt)) best = &e;
+  }
+  return best;
+}
 
 }  // namespace cf

@@ -25,6 +25,7 @@ struct cf_sim {
   bool rearmed;               // no cf_step since the last cf_reset / cf_set_state
   bool last_fresh; long long last_s0; int last_n_steps, last_n_cmds, last_cmd_hold;
   bool pending_bcast, md_valid;
+  int last_rec_mode;          // record mode of the last cf_step launch (cf_describe_launch names that kernel)
   Counters *counters;
   uint32_t *rec_table;
   cudaStream_t stream;

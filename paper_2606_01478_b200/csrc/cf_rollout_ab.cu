@@ -4,33 +4,31 @@
 
 namespace cf {
 
-struct EntryAB { int integ, iface, opt; const char *name; void (*fn)(const StepArgs, const DevParams); };
-
+#define CF_AB1(INTEG, IFACE, OPT, REC) \
+  { INTEG, IFACE, OPT, REC, "rollout<AB," #INTEG "," #IFACE "," #OPT "," #REC ">", rollout_kernel<MODEL_AB, INTEG, IFACE, OPT, REC> }
+// a lean configuration: one kernel per record mode
 #define CF_AB(INTEG, IFACE, OPT) \
-  { INTEG, IFACE, OPT, "rollout<AB," #INTEG "," #IFACE "," #OPT ">", rollout_kernel<MODEL_AB, INTEG, IFACE, OPT> }
+  CF_AB1(INTEG, IFACE, OPT, REC_NONE), CF_AB1(INTEG, IFACE, OPT, REC_SCALAR), CF_AB1(INTEG, IFACE, OPT, REC_TMA)
+#define CF_AB_GEN(INTEG, IFACE) CF_AB1(INTEG, IFACE, OPT_ALL, REC_RUNTIME)
 
-static const EntryAB kTableAB[] = {
+static const RolloutEntry kTableAB[] = {
   // configs[2]: planning rollouts, in-kernel nominal + noise commands, obstacle distance, jittered (a,b,c)
   CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_OBST | OPT_NOISE),
   // sampling-based planner: the same rollout + correlated noise + rollout cost
-  CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_OBST | OPT_NOISE | OPT_COST),
+  CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_OBST | OPT_NOISE | OPT_AR | OPT_COST),
   // variant 3B: the same with a command buffer
   CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_OBST),
   // configs[3]: swarm, position interface, per-world mass
   CF_AB(INTEG_EULER, IF_POSITION, OPT_RANDP),
   CF_AB(INTEG_EULER, IF_ATTITUDE, 0),
   // general kernels
-  CF_AB(INTEG_EULER, IF_ATTITUDE, OPT_ALL), CF_AB(INTEG_RK4, IF_ATTITUDE, OPT_ALL),
-  CF_AB(INTEG_EULER, IF_POSITION, OPT_ALL), CF_AB(INTEG_RK4, IF_POSITION, OPT_ALL),
+  CF_AB_GEN(INTEG_EULER, IF_ATTITUDE), CF_AB_GEN(INTEG_RK4, IF_ATTITUDE),
+  CF_AB_GEN(INTEG_EULER, IF_POSITION), CF_AB_GEN(INTEG_RK4, IF_POSITION),
 };
 
-bool launch_ab(int integ, int iface, int opt, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
+bool launch_ab(int integ, int iface, int opt, int rec_mode, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
                const char **name, int *opt_used, bool dry) {
-  const EntryAB *best = nullptr;
-  for (const EntryAB &e : kTableAB) {
-    if (e.integ != integ || e.iface != iface || (e.opt & opt) != opt) continue;
-    if (!best || __builtin_popcount(e.opt) < __builtin_popcount(best->opt)) best = &e;
-  }
+  const RolloutEntry *best = pick_rollout(kTableAB, (int)(sizeof(kTableAB) / sizeof(kTableAB[0])), integ, iface, opt, rec_mode);
   if (!best) return false;
   if (name) *name = best->name;
   if (opt_used) *opt_used = best->opt;

@@ -4,12 +4,13 @@
 
 namespace cf {
 
-struct EntryFP { int integ, iface, opt; const char *name; void (*fn)(const StepArgs, const DevParams); };
-
+#define CF_FP1(INTEG, IFACE, OPT, REC) \
+  { INTEG, IFACE, OPT, REC, "rollout<FP," #INTEG "," #IFACE "," #OPT "," #REC ">", rollout_kernel<MODEL_FP, INTEG, IFACE, OPT, REC> }
 #define CF_FP(INTEG, IFACE, OPT) \
-  { INTEG, IFACE, OPT, "rollout<FP," #INTEG "," #IFACE "," #OPT ">", rollout_kernel<MODEL_FP, INTEG, IFACE, OPT> }
+  CF_FP1(INTEG, IFACE, OPT, REC_NONE), CF_FP1(INTEG, IFACE, OPT, REC_SCALAR), CF_FP1(INTEG, IFACE, OPT, REC_TMA)
+#define CF_FP_GEN(INTEG, IFACE) CF_FP1(INTEG, IFACE, OPT_ALL, REC_RUNTIME)
 
-static const EntryFP kTableFP[] = {
+static const RolloutEntry kTableFP[] = {
   // configs[0] / configs[1]: attitude interface, nominal plant
   CF_FP(INTEG_EULER, IF_ATTITUDE, 0),
   CF_FP(INTEG_RK4, IF_ATTITUDE, 0),
@@ -17,19 +18,15 @@ static const EntryFP kTableFP[] = {
   CF_FP(INTEG_EULER, IF_ATTITUDE, OPT_RANDP | OPT_DIST),
   CF_FP(INTEG_RK4, IF_ATTITUDE, OPT_RANDP | OPT_DIST),
   // general kernels
-  CF_FP(INTEG_EULER, IF_ROTOR, OPT_ALL),    CF_FP(INTEG_RK4, IF_ROTOR, OPT_ALL),
-  CF_FP(INTEG_EULER, IF_TORQUE, OPT_ALL),   CF_FP(INTEG_RK4, IF_TORQUE, OPT_ALL),
-  CF_FP(INTEG_EULER, IF_ATTITUDE, OPT_ALL), CF_FP(INTEG_RK4, IF_ATTITUDE, OPT_ALL),
-  CF_FP(INTEG_EULER, IF_POSITION, OPT_ALL), CF_FP(INTEG_RK4, IF_POSITION, OPT_ALL),
+  CF_FP_GEN(INTEG_EULER, IF_ROTOR),    CF_FP_GEN(INTEG_RK4, IF_ROTOR),
+  CF_FP_GEN(INTEG_EULER, IF_TORQUE),   CF_FP_GEN(INTEG_RK4, IF_TORQUE),
+  CF_FP_GEN(INTEG_EULER, IF_ATTITUDE), CF_FP_GEN(INTEG_RK4, IF_ATTITUDE),
+  CF_FP_GEN(INTEG_EULER, IF_POSITION), CF_FP_GEN(INTEG_RK4, IF_POSITION),
 };
 
-bool launch_fp(int integ, int iface, int opt, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
+bool launch_fp(int integ, int iface, int opt, int rec_mode, const StepArgs *A, const DevParams *P, const LaunchCfg *L,
                const char **name, int *opt_used, bool dry) {
-  const EntryFP *best = nullptr;
-  for (const EntryFP &e : kTableFP) {
-    if (e.integ != integ || e.iface != iface || (e.opt & opt) != opt) continue;
-    if (!best || __builtin_popcount(e.opt) < __builtin_popcount(best->opt)) best = &e;
-  }
+  const RolloutEntry *best = pick_rollout(kTableFP, (int)(sizeof(kTableFP) / sizeof(kTableFP[0])), integ, iface, opt, rec_mode);
   if (!best) return false;
   if (name) *name = best->name;
   if (opt_used) *opt_used = best->opt;

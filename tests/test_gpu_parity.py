@@ -513,3 +513,33 @@ def test_swarms_without_randomisation_on_superset_kernels(cf, cfo, model, integ,
     assert np.array_equal(g.counters(), o.counters())
     g.step(cm, n, cmd_hold=12, record_every=5)          # the same simulator again WITH the tiled-record staging area
     assert np.isfinite(g.get_state().cpu().numpy()).all()
+
+
+@pytest.mark.parametrize("name,kw,rec_every", [("cfg2", dict(M=256, n_steps=120), 3), ("cfg5", dict(M=96, n_steps=50), 1),
+                                               ("cfg5e", dict(M=2048, n_steps=40), 1), ("cfg4", dict(M=2, N=160, n_steps=60), 7),
+                                               ("cfg1", dict(M=32, n_steps=33), 1)])
+def test_tma_record_path_small_sizes(cf, cfo, W, name, kw, rec_every):
+    """Drone counts that are multiples of 32 take the bulk-tensor (TMA) record store: every record of every drone against
+    the oracle, in one fused call and in a split run whose calls start at odd record slots (tile double-buffering, row
+    coordinate = slot * D of the call's own record buffer), counters and record table bit-exact."""
+    wl = W.make(name, seed=12, **kw)
+    assert wl.MN % 32 == 0
+    g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+    assert "REC_NONE" in g.describe_launch()[0]
+    rg = g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every).cpu().numpy()
+    assert "REC_TMA" in g.describe_launch()[0]
+    ro = o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every)
+    assert rg.shape == ro.shape and rg.shape[0] == wl.n_steps // rec_every
+    for k in range(ro.shape[0]):
+        assert_state_close(rg[k], ro[k], wl.model, 2e-4, f"{name} record {k}")
+    assert np.array_equal(g.counters(), o.counters()) and np.array_equal(g.rec_table(), o.rec_table())
+    b = fresh_gpu(cf, wl)
+    recs = []
+    for cm, n, hold in split_calls(wl, [1, 2, 5, 3, 11]):
+        r = b.step(cm, n, cmd_hold=hold, record_every=rec_every)
+        if r is not None:
+            recs.append(r.cpu().numpy())
+    rb = np.concatenate(recs)
+    fl = floors(wl.model)[0][None, :, None]
+    assert rb.shape == rg.shape and (np.abs(rb - rg) / np.maximum(np.abs(rg), fl)).max() <= 1e-6
+    assert np.array_equal(b.counters(), g.counters()) and np.array_equal(b.rec_table(), g.rec_table())
