@@ -213,8 +213,7 @@ class Runner:
             out = sim.mppi_iterate(self.mpar, self.bstate, self.cmds)
             if self.world > 1:      # the planner's one exchange step: all ranks agree on the best controller's plan
                 from paper_2606_01478_b200 import planner
-                self.global_plan = planner.select_global_plan(
-                    planner.pack_local_best(out["info"], out["plan"], wl.notes["n_ctrl"], self.rank))
+                self.global_plan = planner.select_global_plan(sim, self.mpar, out, self.rank)
             return
         if self.grad:
             sim.grad(self.cmds, wl.n_steps, wl.notes["goal"], cmd_hold=wl.cmd_hold, loss=self.loss, grad=self.gout)

@@ -245,6 +245,17 @@ int cf_mppi_iterate_host(cf_sim *sim, const cf_mppi_params *mp, const float *x0_
                          void *plan_host, void *info_host, void *plan_dev, void *info_dev, void *scratch_dev,
                          size_t scratch_bytes);
 
+/* Selection across shards (multi-GPU: every rank runs its own controllers).
+ * cf_mppi_pack_best writes this shard's row  [score S_c of its best controller, c + ctrl_offset (the GLOBAL controller
+ * index, as a float), plan (H float4)]  = 2 + 4 H floats to row_dev, from the info_dev / plan_dev of cf_mppi_update.
+ * cf_mppi_select reads n_rows such rows (rows_dev [n_rows][2 + 4 H], e.g. an all-gather of every rank's row) and copies the
+ * winner to best_row_dev: smallest score compared as a float32 in IEEE total order with NaN last, ties -> smallest global
+ * controller index (reading R31) -- the same row on every rank.  Both enqueue on the bound stream. */
+#define CF_MPPI_ROW_WORDS(horizon) (2 + 4 * (horizon))
+int cf_mppi_pack_best(cf_sim *sim, const cf_mppi_params *mp, const void *info_dev, const void *plan_dev, int ctrl_offset,
+                      float *row_dev);
+int cf_mppi_select(cf_sim *sim, const float *rows_dev, int n_rows, int horizon, float *best_row_dev);
+
 /* ---- Gradient of a goal distance w.r.t. the command sequence (Fig. 3D) -------------------------
  * "Measuring throughput over ten simulation steps by differentiating a goal distance with respect to the control
  *  inputs"; "differentiating through high-fidelity dynamics, the full onboard controller stack".
@@ -252,16 +263,28 @@ int cf_mppi_iterate_host(cf_sim *sim, const cf_mppi_params *mp, const float *x0_
  *   neither the planes nor the step counter), driven by cmds_dev [n_cmds][MN] float4 exactly as cf_step would be;
  *   grad_dev [n_cmds][MN] float4 receives dL_i / d cmds[k][i][0..3]  (commands beyond the last used one: 0);
  *   loss_dev [MN] receives L_i.
- * One hand-written reverse-mode kernel: forward sweep parking each step's state in scratch_dev
- * (cf_grad_scratch_bytes = n_steps * HD * MN floats, HD = 24 first-principles / 16 abstracted, 16-byte aligned), backward
- * sweep through normalisation, RK4 / Euler, Eqs. (1)-(4), (6) or (7)-(10), mixer and attitude controller.  Where a
- * clip of the method is active (rotor thrust / speed limits, controller integral, rotor-interface command limits) the
- * derivative is taken as 0 (reading R33); the controller tick schedule follows the global step counter.
- * Supported: CF_CMD_BUFFER; rotor and attitude interface (first-principles), attitude (abstracted); Euler and RK4; per-world
- * randomised parameters; no disturbances, no fidelity extras (CF_E_UNSUPPORTED otherwise).  goal: 3 floats on the HOST. */
+ * One hand-written reverse-mode kernel: forward sweep parking, per step, only what the backward sweep reads non-linearly
+ * in scratch_dev (cf_grad_scratch_bytes = n_steps * HD * MN floats, 16-byte aligned; HD = 16 / 18 / 32 for the
+ * first-principles model with the rotor / attitude / position interface -- attitude, body rates, rotor speeds, controller
+ * integrals, rotor command; position and velocity only when the position controller reads them -- and 8 / 20 for the
+ * abstracted model with the attitude / position interface), backward sweep through normalisation, RK4 / Euler, Eqs.
+ * (1)-(4), (6) or (7)-(10), mixer, attitude controller and geometric position controller (the full onboard stack of
+ * PAPER.md:L69).  Where a clip of the method is active (rotor thrust / speed limits, controller integrals, thrust and tilt
+ * limits, rotor-interface command limits) the derivative is taken as 0 (reading R33); the controller tick schedules
+ * follow the global step counter.
+ * Supported: CF_CMD_BUFFER; rotor, attitude and position interface (first-principles), attitude and position (abstracted);
+ * Euler and RK4; per-world randomised parameters; no disturbances, no fidelity extras, no torque interface
+ * (CF_E_UNSUPPORTED otherwise).  goal: 3 floats on the HOST.
+ * cf_grad_host: the same from HOST buffers -- cmds_host [n_cmds][MN] float4 in, loss_host [MN] and grad_host
+ * [n_cmds][MN] float4 out, through staging_dev (cf_grad_staging_bytes(), 256-byte aligned, caller-owned device memory);
+ * synchronises the stream. */
 size_t cf_grad_scratch_bytes(const cf_sim *sim, int n_steps);
 int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
             float *loss_dev, void *grad_dev, void *scratch_dev, size_t scratch_bytes);
+size_t cf_grad_staging_bytes(const cf_sim *sim, int n_cmds);
+int cf_grad_host(cf_sim *sim, const void *cmds_host, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
+                 float *loss_host, void *grad_host, void *staging_dev, size_t staging_bytes, void *scratch_dev,
+                 size_t scratch_bytes);
 
 /* ---- Batched depth ray casting -------------------------------------------------------------
  * "parallel rendering of depth images ... 350k frames per second at a 64x64 ray resolution across 1,024 environments".
@@ -284,6 +307,11 @@ typedef struct cf_depth_params {
   float    boxes[CF_DEPTH_MAX_PRIMS][6];        /* cx cy cz hx hy hz (half extents) */
 } cf_depth_params;
 int cf_depth(cf_sim *sim, const cf_depth_params *dp, float *depth_dev /* [MN][height][width] */);
+/* The same from HOST buffers: state_host [D][MN] (poses to render; NULL = the simulator's current state) is copied into the
+ * state planes, the images go through staging_dev (MN * height * width floats, caller-owned device memory) to depth_host;
+ * synchronises the stream. */
+int cf_depth_host(cf_sim *sim, const cf_depth_params *dp, const float *state_host, float *depth_host,
+                  float *staging_dev, size_t staging_bytes);
 
 const char *cf_last_error(void);
 /* Host-side Philox4x32-10 of this library, for the bit-exact check against the oracle's (C9). */

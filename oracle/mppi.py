@@ -101,3 +101,11 @@ def update(cost_f32, nominal, *, seed: int, world_offset: int, worlds_per_ctrl: 
     idx = np.minimum(np.arange(H) + shift, H - 1)
     return dict(elites=elites, mean=mean, score=score, jmin=jmin, wsum=wsum, best=best, plan=mean[best].copy(),
                 nominal_next=mean[:, idx, :].copy())
+
+
+def select_rows(rows) -> int:
+    """R31 across shards: rows [n][2 + 4 H] of (score, global controller index, plan...) -> index of the winning row:
+    smallest score compared as a float32 in IEEE total order with NaN last (the R28 key), ties -> smallest controller index."""
+    rows = np.asarray(rows, dtype=np.float32).reshape(len(rows), -1)
+    key = cost_key(rows[:, 0])
+    return int(np.lexsort((rows[:, 1], key))[0])

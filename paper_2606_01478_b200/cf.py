@@ -113,7 +113,12 @@ def lib():
         "cf_mppi_update": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, sz]),
         "cf_mppi_iterate": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, sz]),
         "cf_mppi_iterate_host": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, vp, sz]),
+        "cf_mppi_pack_best": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, C.c_int, vp]),
+        "cf_mppi_select": (C.c_int, [vp, vp, C.c_int, C.c_int, vp]),
         "cf_grad_scratch_bytes": (sz, [vp, C.c_int]),
+        "cf_grad_staging_bytes": (sz, [vp, C.c_int]),
+        "cf_grad_host": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float * 3), vp, vp, vp, sz, vp, sz]),
+        "cf_depth_host": (C.c_int, [vp, C.POINTER(DepthParams), vp, vp, vp, sz]),
         "cf_grad": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float * 3), vp, vp, vp, sz]),
         "cf_depth": (C.c_int, [vp, C.POINTER(DepthParams), vp]),
         "cf_last_error": (C.c_char_p, []),
@@ -132,7 +137,8 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_get_state", "cf_get_state_host", "cf_get_aux", "cf_get_aux_host", "cf_step_counter", "cf_sync_counters",
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
            "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host", "cf_grad_scratch_bytes",
-           "cf_grad", "cf_depth", "cf_reset_masked"]
+           "cf_grad", "cf_depth", "cf_reset_masked", "cf_grad_staging_bytes", "cf_grad_host", "cf_depth_host",
+           "cf_mppi_pack_best", "cf_mppi_select"]
 
 
 def _check(rc: int):
@@ -384,6 +390,16 @@ class Sim:
         _check(lib().cf_depth(self._h, C.byref(dp), _dptr(out)))
         return out
 
+    def depth_host(self, dp: DepthParams, out_host, state_host=None):
+        """End-to-end rendering: state_host [D][MN] (pinned CPU tensor of poses, or None) in, out_host [MN][H][W] (pinned) out."""
+        torch = _torch()
+        n = self.MN * dp.height * dp.width
+        if getattr(self, "_depth_stage", None) is None or self._depth_stage.numel() < n:
+            self._depth_stage = torch.empty(n, dtype=torch.float32, device=self.device)
+        sp = None if state_host is None else C.c_void_p(state_host.data_ptr())
+        _check(lib().cf_depth_host(self._h, C.byref(dp), sp, C.c_void_p(out_host.data_ptr()), _dptr(self._depth_stage), 4 * n))
+        return out_host
+
     # -- gradient of the goal distance w.r.t. the commands (cf_grad) --------------------------------------------------
     def grad(self, cmds, n_steps: int, goal, cmd_hold: int = 1, loss=None, grad=None):
         """cmds: float32 [K][MN][4] (device).  Returns (loss [MN], grad [K][MN][4]) device tensors; the simulator state
@@ -405,7 +421,41 @@ class Sim:
                              C.c_void_p(sp), need))
         return loss, grad
 
+    def grad_host(self, cmds_host, n_steps: int, goal, loss_host, grad_host, cmd_hold: int = 1):
+        """End-to-end gradient: cmds_host [K][MN][4], loss_host [MN], grad_host [K][MN][4] are (pinned) CPU tensors."""
+        torch = _torch()
+        K = cmds_host.numel() // (4 * self.MN)
+        need = lib().cf_grad_scratch_bytes(self._h, int(n_steps))
+        if getattr(self, "_grad_scratch", None) is None or self._grad_scratch.numel() < need + 16:
+            self._grad_scratch = torch.empty(need + 16, dtype=torch.uint8, device=self.device)
+        sp = self._grad_scratch.data_ptr() + (-self._grad_scratch.data_ptr()) % 16
+        st = lib().cf_grad_staging_bytes(self._h, K)
+        if getattr(self, "_grad_stage", None) is None or self._grad_stage.numel() < st + 256:
+            self._grad_stage = torch.empty(st + 256, dtype=torch.uint8, device=self.device)
+        stp = self._grad_stage.data_ptr() + (-self._grad_stage.data_ptr()) % 256
+        g3 = (C.c_float * 3)(*[float(v) for v in goal])
+        _check(lib().cf_grad_host(self._h, C.c_void_p(cmds_host.data_ptr()), K, int(cmd_hold), int(n_steps), C.byref(g3),
+                                  C.c_void_p(loss_host.data_ptr()), C.c_void_p(grad_host.data_ptr()), C.c_void_p(stp), st,
+                                  C.c_void_p(sp), need))
+        return loss_host, grad_host
+
     # -- sampling-based planner (cf_mppi_*) --------------------------------------------------------------------------
+    def mppi_pack_best(self, mp: MppiParams, info, plan, ctrl_offset: int, row=None):
+        """This shard's [score, global controller index, plan] row (device tensor of 2 + 4 H floats)."""
+        if row is None:
+            row = _torch().empty(2 + 4 * mp.horizon, dtype=_torch().float32, device=self.device)
+        _check(lib().cf_mppi_pack_best(self._h, C.byref(mp), _dptr(info), _dptr(plan), int(ctrl_offset), _dptr(row)))
+        return row
+
+    def mppi_select(self, rows, horizon: int, out=None):
+        """rows: device tensor [n_rows][2 + 4 H] -> the winning row (R31), identical whatever the row order."""
+        assert rows.is_cuda and rows.is_contiguous() and rows.dtype == _torch().float32
+        n_rows = rows.numel() // (2 + 4 * horizon)
+        if out is None:
+            out = _torch().empty(2 + 4 * horizon, dtype=_torch().float32, device=self.device)
+        _check(lib().cf_mppi_select(self._h, _dptr(rows), n_rows, int(horizon), _dptr(out)))
+        return out
+
     def mppi_params(self, horizon: int, cmd_hold: int, n_elite: int, lam: float, shift: int = 1) -> MppiParams:
         return MppiParams(C.sizeof(MppiParams), int(horizon), int(cmd_hold), int(n_elite), int(shift), float(lam))
 

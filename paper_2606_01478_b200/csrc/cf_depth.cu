@@ -187,3 +187,27 @@ extern "C" int cf_depth(cf_sim *sim, const cf_depth_params *dp, float *depth_dev
   CF_CUDA(cudaGetLastError());
   return CF_OK;
 }
+
+// The same rendering driven from HOST buffers (the end-to-end path): state_host [D][MN] (the poses; NULL = render the
+// simulator's current state) is copied host->device into the state planes, the images are rendered into staging_dev and
+// copied device->host, and the stream is synchronised.
+extern "C" int cf_depth_host(cf_sim *sim, const cf_depth_params *dp, const float *state_host, float *depth_host,
+                             float *staging_dev, size_t staging_bytes) {
+  if (!sim || !dp || !depth_host || !staging_dev) return fail(CF_E_ARG, "NULL argument");
+  if (dp->struct_size != sizeof(cf_depth_params)) return fail(CF_E_ARG, "cf_depth_params.struct_size mismatch");
+  if (dp->width < 1 || dp->height < 1) return fail(CF_E_ARG, "bad image size");
+  const size_t bytes = sizeof(float) * (size_t)sim->MN * (size_t)dp->width * (size_t)dp->height;
+  if (staging_bytes < bytes) return fail(CF_E_BUFFER, "staging too small: %zu < %zu", staging_bytes, bytes);
+  if (state_host) {
+    if (!sim->have_state) return fail(CF_E_STATE, "cf_depth_host needs a prior cf_reset (world parameters)");
+    int rc = cf_materialise(sim);
+    if (rc != CF_OK) return rc;
+    CF_CUDA(cudaMemcpyAsync(sim->state, state_host, sizeof(float) * sim->D * (size_t)sim->MN, cudaMemcpyHostToDevice, sim->stream));
+    sim->md_valid = false; sim->cost_valid = false; sim->rearmed = false;
+  }
+  int rc = cf_depth(sim, dp, staging_dev);
+  if (rc != CF_OK) return rc;
+  CF_CUDA(cudaMemcpyAsync(depth_host, staging_dev, bytes, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  return CF_OK;
+}

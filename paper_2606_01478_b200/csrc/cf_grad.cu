@@ -290,27 +290,152 @@ __device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MO
   }
 }
 
-// history record of one step: pre-step state, and for the first-principles model the controller integral before the
-// step's tick and the rotor command the step integrated with
+// ---- VJP of the geometric position controller tick (C7, reading R16) ----------------------------------------------------
+// inputs of the tick: p, v (state), zB (body z axis in the world frame), target = (x, y, z, yaw), ip (integral before).
+// cotangents in: g_att[4] of the attitude command (roll, pitch, yaw, F) the tick produced, g_ipn[3] of the integral
+// after the tick.  out: accumulates into g_p[3], g_v[3], g_zB[3], g_tg[4]; g_ip[3] = cotangent of the integral before.
+// Where a clip of the method is active (integral, thrust, tilt, asin argument, norm floors) the derivative is 0 (R33).
+__device__ __forceinline__ void vjp_position_tick(const DevParams &P, const float *pos, const float *vel, const float *zB,
+                                                  const float *target, const float *ip, const float *g_att,
+                                                  const float *g_ipn, float *g_p, float *g_v, float *g_zB, float *g_tg,
+                                                  float *g_ip) {
+  // forward recomputation (same arithmetic as position_tick, accurate trigonometry: this is a linearisation point)
+  float ep[3], pre[3], t[3];
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    ep[j] = target[j] - pos[j];
+    pre[j] = fmaf(ep[j], P.h_pos, ip[j]);
+    float ipn = clipf(pre[j], -P.ip_max[j], P.ip_max[j]);
+    float ad = P.kp[j] * ep[j] - P.kd[j] * vel[j] + P.ki[j] * ipn + (j == 2 ? P.g : 0.0f);
+    t[j] = P.mass * ad;
+  }
+  const float Fraw = t[0] * zB[0] + t[1] * zB[1] + t[2] * zB[2];
+  const float n2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
+  const bool n_live = n2 > 1e-12f;
+  const float inv = rsqrtf(fmaxf(n2, 1e-12f));
+  const float zd[3] = { t[0] * inv, t[1] * inv, t[2] * inv };
+  float sy, cy;
+  sincosf(target[3], &sy, &cy);
+  const float yr[3] = { -zd[2] * sy, zd[2] * cy, zd[0] * sy - zd[1] * cy };
+  const float ny2 = yr[0] * yr[0] + yr[1] * yr[1] + yr[2] * yr[2];
+  const bool y_live = ny2 > 1e-12f;
+  const float invy = rsqrtf(fmaxf(ny2, 1e-12f));
+  const float yd[3] = { yr[0] * invy, yr[1] * invy, yr[2] * invy };
+  const float xd[3] = { yd[1] * zd[2] - yd[2] * zd[1], yd[2] * zd[0] - yd[0] * zd[2], yd[0] * zd[1] - yd[1] * zd[0] };
+  const float roll_raw = atan2f(yd[2], zd[2]);
+  const float sarg = -xd[2];
+  const float pitch_raw = asinf(clipf(sarg, -1.0f, 1.0f));
+  // reverse
+  float g_xd[3] = { 0.f, 0.f, 0.f }, g_yd[3] = { 0.f, 0.f, 0.f }, g_zd[3] = { 0.f, 0.f, 0.f };
+  {                                                   // yaw = atan2(xd_y, xd_x)
+    const float r2 = xd[0] * xd[0] + xd[1] * xd[1];
+    if (r2 > 0.f) { g_xd[1] += g_att[2] * xd[0] / r2; g_xd[0] -= g_att[2] * xd[1] / r2; }
+  }
+  if (fabsf(pitch_raw) < P.tilt_max && fabsf(sarg) < 1.0f)          // pitch = asin(-xd_z)
+    g_xd[2] -= g_att[1] * rsqrtf(fmaxf(1.0f - sarg * sarg, 1e-20f));
+  if (fabsf(roll_raw) < P.tilt_max) {                                 // roll = atan2(yd_z, zd_z)
+    const float r2 = yd[2] * yd[2] + zd[2] * zd[2];
+    if (r2 > 0.f) { g_yd[2] += g_att[0] * zd[2] / r2; g_zd[2] -= g_att[0] * yd[2] / r2; }
+  }
+  // xd = yd x zd:  g_yd += zd x g_xd,  g_zd += g_xd x yd
+  g_yd[0] += zd[1] * g_xd[2] - zd[2] * g_xd[1]; g_yd[1] += zd[2] * g_xd[0] - zd[0] * g_xd[2]; g_yd[2] += zd[0] * g_xd[1] - zd[1] * g_xd[0];
+  g_zd[0] += g_xd[1] * yd[2] - g_xd[2] * yd[1]; g_zd[1] += g_xd[2] * yd[0] - g_xd[0] * yd[2]; g_zd[2] += g_xd[0] * yd[1] - g_xd[1] * yd[0];
+  // yd = yr / |yr|
+  float g_yr[3];
+  {
+    const float dot = yd[0] * g_yd[0] + yd[1] * g_yd[1] + yd[2] * g_yd[2];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) g_yr[j] = y_live ? invy * (g_yd[j] - yd[j] * dot) : invy * g_yd[j];
+  }
+  // yr = (-zd_z sy, zd_z cy, zd_x sy - zd_y cy)
+  g_zd[2] += -sy * g_yr[0] + cy * g_yr[1];
+  g_zd[0] += sy * g_yr[2];
+  g_zd[1] -= cy * g_yr[2];
+  g_tg[3] += g_yr[0] * (-zd[2] * cy) + g_yr[1] * (-zd[2] * sy) + g_yr[2] * (zd[0] * cy + zd[1] * sy);
+  // zd = t / |t|
+  float g_t[3];
+  {
+    const float dot = zd[0] * g_zd[0] + zd[1] * g_zd[1] + zd[2] * g_zd[2];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) g_t[j] = n_live ? inv * (g_zd[j] - zd[j] * dot) : inv * g_zd[j];
+  }
+  // F = clip(t . zB)
+  if (Fraw > P.thrust_min && Fraw < P.thrust_max) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { g_t[j] += g_att[3] * zB[j]; g_zB[j] += g_att[3] * t[j]; }
+  }
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    const float g_ad = P.mass * g_t[j];
+    float g_ep = P.kp[j] * g_ad;
+    g_v[j] -= P.kd[j] * g_ad;
+    const float g_in = g_ipn[j] + P.ki[j] * g_ad;
+    const float g_pre = (pre[j] > -P.ip_max[j] && pre[j] < P.ip_max[j]) ? g_in : 0.0f;
+    g_ip[j] = g_pre;
+    g_ep += P.h_pos * g_pre;
+    g_tg[j] += g_ep;
+    g_p[j] -= g_ep;
+  }
+}
+
+// body z axis in the world frame and the pull-back of its cotangent to the attitude state
+__device__ __forceinline__ void zB_fp(const float *q, float *zB) {
+  zB[0] = 2.0f * (q[0] * q[2] + q[3] * q[1]);
+  zB[1] = 2.0f * (q[1] * q[2] - q[3] * q[0]);
+  zB[2] = 1.0f - 2.0f * (q[0] * q[0] + q[1] * q[1]);
+}
+__device__ __forceinline__ void vjp_zB_fp(const float *q, const float *gz, float *g_q) {
+  g_q[0] += 2.0f * (q[2] * gz[0] - q[3] * gz[1]) - 4.0f * q[0] * gz[2];
+  g_q[1] += 2.0f * (q[3] * gz[0] + q[2] * gz[1]) - 4.0f * q[1] * gz[2];
+  g_q[2] += 2.0f * (q[0] * gz[0] + q[1] * gz[1]);
+  g_q[3] += 2.0f * (q[1] * gz[0] - q[0] * gz[1]);
+}
+__device__ __forceinline__ void zB_ab(const float *psi, float *zB, float *sn, float *cs) {
+  sincos3_step(psi, sn, cs);
+  zB[0] = cs[2] * sn[1] * cs[0] + sn[2] * sn[0]; zB[1] = sn[2] * sn[1] * cs[0] - cs[2] * sn[0]; zB[2] = cs[1] * cs[0];
+}
+__device__ __forceinline__ void vjp_zB_ab(const float *sn, const float *cs, const float *gz, float *g_psi) {
+  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
+  g_psi[0] += (-cy * sp * sr + sy * cr) * gz[0] + (-sy * sp * sr - cy * cr) * gz[1] + (-cp * sr) * gz[2];
+  g_psi[1] += (cy * cp * cr) * gz[0] + (sy * cp * cr) * gz[1] + (-sp * cr) * gz[2];
+  g_psi[2] += (-sy * sp * cr + cy * sr) * gz[0] + (cy * sp * cr + sy * sr) * gz[1];
+}
+
+// History of one step: only what the backward sweep reads NON-linearly.  Position and velocity enter Eqs. (1)-(4) /
+// (7)-(10) linearly (no drag here), so without the position controller they are neither parked nor re-read:
+//   FP rotor     16 floats: q(4) w(3) - Omega(4) rotor command(4)
+//   FP attitude  18 floats: q(4) w(3) iR_0 Omega(4) rotor command(4) | iR_1 iR_2        (4 float4 + 1 float2)
+//   FP position  32 floats: the 17 state floats, iR(3), ip(3), rotor command(4), attitude command after the tick(4), pad
+//   AB attitude   8 floats: Psi(3) dPsi(3) f_Sigma pad
+//   AB position  20 floats: the 13 state floats, ip(3), attitude command after the tick(4)
+// Layout: all float4 planes first, [n_steps][H4][MN] float4, then the float2 planes [n_steps][MN] (FP attitude only), so
+// every plane is aligned whatever MN is; a warp writes 512 (256) contiguous bytes per plane.
 #ifndef GRAD_MIN_BLOCKS
 #define GRAD_MIN_BLOCKS 4
 #endif
-// (float4 planes: a warp writes 512 contiguous bytes per plane with one STG.128 per lane; the abstracted model pads 13 -> 16)
-template <int MODEL> struct Hist { static constexpr int HD = MODEL == MODEL_FP ? 17 + 3 + 4 : 16; };
+template <int MODEL, int IFACE> struct Hist {
+  static constexpr bool POS = IFACE == IF_POSITION;
+  static constexpr int HD = MODEL == MODEL_FP ? (POS ? 32 : (IFACE == IF_ATTITUDE ? 18 : 16)) : (POS ? 20 : 8);
+  static constexpr int H4 = HD / 4, H2 = (HD % 4) / 2;
+};
 
 template <int MODEL, int INTEG, int IFACE>
 __global__ void __launch_bounds__(128, GRAD_MIN_BLOCKS)
 grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParams P, int randp) {
-  constexpr int D = Dim<MODEL>::D, HD = Hist<MODEL>::HD;
+  using H = Hist<MODEL, IFACE>;
+  constexpr int D = Dim<MODEL>::D, HD = H::HD, H4 = H::H4, HP = H4 * 4 + 4;
   constexpr bool FP = MODEL == MODEL_FP;
-  constexpr bool HAS_ATT = FP && IFACE == IF_ATTITUDE;
+  constexpr bool POS = IFACE == IF_POSITION;
+  constexpr bool HAS_ATT = FP && IFACE >= IF_ATTITUDE;
+  constexpr int VEL = FP ? 7 : 6;
   const long long MN = A.MN;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= MN) return;
   Plant<MODEL, 0> pl;
   pl.load(P, A.wparam, A.M, i / A.N, randp != 0);
 
-  float x[D], iR[3] = { 0, 0, 0 }, rpm_cmd[4] = { 0, 0, 0, 0 }, cmd[4] = { 0, 0, 0, 0 };
+  float x[D], iR[3] = { 0, 0, 0 }, ip[3] = { 0, 0, 0 }, rpm_cmd[4] = { 0, 0, 0, 0 }, cmd[4] = { 0, 0, 0, 0 };
+  float att_cmd[4] = { 0, 0, 0, 0 };      // position interface: the attitude command the outer loop holds
 #pragma unroll
   for (int j = 0; j < D; ++j) x[j] = A.state[j * MN + i];
   if (FP) {
@@ -319,13 +444,46 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
 #pragma unroll
     for (int j = 0; j < 4; ++j) rpm_cmd[j] = A.ctrl[(10 + j) * MN + i];
   }
-  // ---- forward sweep -----------------------------------------------------------------------------------------
-  int att_phase = (int)(A.s0 % (uint32_t)P.att_div);
-  for (int t = 0; t < A.n_steps; ++t) {
-    float4 *h = A.hist + (size_t)t * (HD / 4) * MN + i;
-    float rec[HD];                                          // the step's record: x, [iR before the tick, rotor command]
+  if (POS) {
 #pragma unroll
-    for (int j = 0; j < HD; ++j) rec[j] = j < D ? x[j] : 0.f;
+    for (int j = 0; j < 3; ++j) ip[j] = A.ctrl[(3 + j) * MN + i];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) att_cmd[j] = A.ctrl[(6 + j) * MN + i];
+  }
+  float4 *const h4 = A.hist;
+  float2 *const h2 = reinterpret_cast<float2 *>(A.hist + (size_t)A.n_steps * H4 * MN);
+  // pack / unpack of one step's record (see the table above)
+  auto pack = [&](float *rec) {
+#pragma unroll
+    for (int j = 0; j < HP; ++j) rec[j] = 0.f;
+    if constexpr (POS) {
+#pragma unroll
+      for (int j = 0; j < D; ++j) rec[j] = x[j];
+      int o = D;
+      if (FP) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) rec[o + j] = iR[j];
+        o += 3;
+      }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) rec[o + j] = ip[j];
+    } else if constexpr (FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { rec[j] = x[3 + j]; rec[8 + j] = x[13 + j]; }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) rec[4 + j] = x[10 + j];
+      if (HAS_ATT) { rec[7] = iR[0]; rec[16] = iR[1]; rec[17] = iR[2]; }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) { rec[j] = x[3 + j]; rec[3 + j] = x[9 + j]; }
+      rec[6] = x[12];
+    }
+  };
+  // ---- forward sweep -----------------------------------------------------------------------------------------
+  int att_phase = (int)(A.s0 % (uint32_t)P.att_div), pos_phase = (int)(A.s0 % (uint32_t)P.pos_div);
+  for (int t = 0; t < A.n_steps; ++t) {
+    float rec[HP];                                          // pre-step state and controller state of this step
+    pack(rec);
     if (t % A.cmd_hold == 0) {
       float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
       cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
@@ -334,23 +492,40 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
         for (int j = 0; j < 4; ++j) rpm_cmd[j] = clipf(cmd[j], P.rpm_min, P.rpm_max);
       }
     }
+    if (POS) {
+      if (pos_phase == 0) {
+        float zB[3], sn[3], cs[3];
+        if (FP) zB_fp(x + 3, zB); else zB_ab(x + 3, zB, sn, cs);
+        position_tick(P, x, x + VEL, zB, cmd, ip, att_cmd);
+      }
+      pos_phase = pos_phase + 1 == P.pos_div ? 0 : pos_phase + 1;
+    }
+    const float *acmd = POS ? att_cmd : cmd;                // the attitude command in force at this step
     if (HAS_ATT) {
-#pragma unroll
-      for (int j = 0; j < 3; ++j) rec[17 + j] = iR[j];
       if (att_phase == 0) {
         float Rd[3][3];
-        euler_to_R(cmd[0], cmd[1], cmd[2], Rd);
-        attitude_tick<0>(P, x + 3, x + 10, Rd, cmd[3], iR, rpm_cmd);
+        euler_to_R(acmd[0], acmd[1], acmd[2], Rd);
+        attitude_tick<0>(P, x + 3, x + 10, Rd, acmd[3], iR, rpm_cmd);
       }
       att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
     }
-    if (FP) {
+    if constexpr (POS) {
+      constexpr int o = FP ? D + 6 : D + 3;
+      if (FP) {
 #pragma unroll
-      for (int j = 0; j < 4; ++j) rec[20 + j] = rpm_cmd[j];
+        for (int j = 0; j < 4; ++j) rec[o + j] = rpm_cmd[j];
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) rec[o + (FP ? 4 : 0) + j] = att_cmd[j];
+    } else if constexpr (FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) rec[12 + j] = rpm_cmd[j];
     }
 #pragma unroll
-    for (int j = 0; j < HD / 4; ++j) __stcs(h + (size_t)j * MN, make_float4(rec[4 * j], rec[4 * j + 1], rec[4 * j + 2], rec[4 * j + 3]));
-    step_forward<MODEL, INTEG>(P, pl, x, FP ? rpm_cmd : cmd);
+    for (int j = 0; j < H4; ++j)
+      __stcs(h4 + ((size_t)t * H4 + j) * MN + i, make_float4(rec[4 * j], rec[4 * j + 1], rec[4 * j + 2], rec[4 * j + 3]));
+    if constexpr (H::H2) __stcs(h2 + (size_t)t * MN + i, make_float2(rec[4 * H4], rec[4 * H4 + 1]));
+    step_forward<MODEL, INTEG>(P, pl, x, FP ? rpm_cmd : acmd);
   }
   // ---- loss and its cotangent ----------------------------------------------------------------------------------
   float lam[D];
@@ -366,41 +541,90 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   // ---- backward sweep ------------------------------------------------------------------------------------------
   float g_cmd[4] = { 0, 0, 0, 0 };      // cotangent of the held command, until its fetch step is reached
   float g_rpm[4] = { 0, 0, 0, 0 };      // cotangent of the held rotor command, until the tick / fetch that set it
-  float g_iR[3] = { 0, 0, 0 };          // cotangent of the controller integral
+  float g_iR[3] = { 0, 0, 0 };          // cotangent of the attitude controller's integral
+  float g_att[4] = { 0, 0, 0, 0 };      // position interface: cotangent of the held attitude command, until the tick that set it
+  float g_ip[3] = { 0, 0, 0 };          // cotangent of the position controller's integral
   att_phase = (int)((A.s0 + (uint32_t)A.n_steps - 1u) % (uint32_t)P.att_div);
-  for (int t = A.n_steps - 1; t >= 0; --t) {
-    const float4 *h = A.hist + (size_t)t * (HD / 4) * MN + i;
-    float rec[HD];
+  pos_phase = (int)((A.s0 + (uint32_t)A.n_steps - 1u) % (uint32_t)P.pos_div);
 #pragma unroll
-    for (int j = 0; j < HD / 4; ++j) {
-      const float4 v = __ldcs(h + (size_t)j * MN);
-      rec[4 * j] = v.x; rec[4 * j + 1] = v.y; rec[4 * j + 2] = v.z; rec[4 * j + 3] = v.w;
+  for (int j = 0; j < D; ++j) x[j] = 0.f;                   // components that are not parked enter only linearly
+  for (int t = A.n_steps - 1; t >= 0; --t) {
+    float rec[HP];
+    if (t > 0) {            // pull the previous step's record towards L2 while this step's pull-back computes
+#pragma unroll
+      for (int j = 0; j < H4; ++j) asm volatile("prefetch.global.L2 [%0];" :: "l"(h4 + ((size_t)(t - 1) * H4 + j) * MN + i));
+      if constexpr (H::H2) asm volatile("prefetch.global.L2 [%0];" :: "l"(h2 + (size_t)(t - 1) * MN + i));
     }
 #pragma unroll
-    for (int j = 0; j < D; ++j) x[j] = rec[j];
+    for (int j = 0; j < H4; ++j) {
+      const float4 v = __ldcs(h4 + ((size_t)t * H4 + j) * MN + i);
+      rec[4 * j] = v.x; rec[4 * j + 1] = v.y; rec[4 * j + 2] = v.z; rec[4 * j + 3] = v.w;
+    }
+    if constexpr (H::H2) { const float2 v = __ldcs(h2 + (size_t)t * MN + i); rec[4 * H4] = v.x; rec[4 * H4 + 1] = v.y; }
+    if constexpr (POS) {
+#pragma unroll
+      for (int j = 0; j < D; ++j) x[j] = rec[j];
+      int o = D;
+      if (FP) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) iR[j] = rec[o + j];
+        o += 3;
+      }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) ip[j] = rec[o + j];
+      o += 3;
+      if (FP) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) rpm_cmd[j] = rec[o + j];
+        o += 4;
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) att_cmd[j] = rec[o + j];
+    } else if constexpr (FP) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { x[3 + j] = rec[j]; x[13 + j] = rec[8 + j]; rpm_cmd[j] = rec[12 + j]; }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) x[10 + j] = rec[4 + j];
+      if (HAS_ATT) { iR[0] = rec[7]; iR[1] = rec[16]; iR[2] = rec[17]; }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) { x[3 + j] = rec[j]; x[9 + j] = rec[3 + j]; }
+      x[12] = rec[6];
+    }
     if (t % A.cmd_hold == A.cmd_hold - 1 || t == A.n_steps - 1) {             // entering the run of command t / hold
       float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
       cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
     }
-    if (FP) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) rpm_cmd[j] = rec[20 + j];
-      step_backward<MODEL, INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
-    } else {
-      step_backward<MODEL, INTEG>(P, pl, x, cmd, lam, g_cmd);
-    }
+    const float *acmd = POS ? att_cmd : cmd;
+    float *g_acmd = POS ? g_att : g_cmd;
+    // (tried and rejected, measured: the four RK4 stages of this pull-back rolled into run-time loops with the stage
+    //  states in shared memory -- "no instruction" stalls 1.03 -> 0.13 per issue, issue-active 68 -> 79 %, but 27 % more
+    //  instructions because the straight-line form lets the compiler drop dead parts of every stage: 0.80 -> 0.87 ms)
+    if (FP) step_backward<MODEL, INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
+    else step_backward<MODEL, INTEG>(P, pl, x, acmd, lam, g_acmd);
     if (HAS_ATT) {
       if (att_phase == 0) {
-#pragma unroll
-        for (int j = 0; j < 3; ++j) iR[j] = rec[17 + j];
         float g_prev[3];
-        vjp_attitude_tick(P, x + 3, x + 10, cmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_cmd, g_prev);
+        vjp_attitude_tick(P, x + 3, x + 10, acmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_acmd, g_prev);
 #pragma unroll
         for (int j = 0; j < 3; ++j) g_iR[j] = g_prev[j];
 #pragma unroll
         for (int j = 0; j < 4; ++j) g_rpm[j] = 0.f;
       }
       att_phase = att_phase == 0 ? P.att_div - 1 : att_phase - 1;
+    }
+    if (POS) {
+      if (pos_phase == 0) {           // the tick of this step produced att_cmd from (p, v, attitude, target, ip)
+        float zB[3], gz[3] = { 0.f, 0.f, 0.f }, g_prev[3], sn[3], cs[3];
+        if (FP) zB_fp(x + 3, zB); else zB_ab(x + 3, zB, sn, cs);
+        vjp_position_tick(P, x, x + VEL, zB, cmd, ip, g_att, g_ip, lam, lam + VEL, gz, g_cmd, g_prev);
+        if (FP) vjp_zB_fp(x + 3, gz, lam + 3); else vjp_zB_ab(sn, cs, gz, lam + 3);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) g_ip[j] = g_prev[j];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) g_att[j] = 0.f;
+      }
+      pos_phase = pos_phase == 0 ? P.pos_div - 1 : pos_phase - 1;
     }
     if (t % A.cmd_hold == 0) {                                                 // the fetch step of command t / hold
       if (FP && IFACE == IF_ROTOR) {
@@ -420,6 +644,9 @@ const Entry kTable[] = {
   CF_G(MODEL_FP, INTEG_EULER, IF_ATTITUDE), CF_G(MODEL_FP, INTEG_RK4, IF_ATTITUDE),
   CF_G(MODEL_FP, INTEG_EULER, IF_ROTOR),    CF_G(MODEL_FP, INTEG_RK4, IF_ROTOR),
   CF_G(MODEL_AB, INTEG_EULER, IF_ATTITUDE), CF_G(MODEL_AB, INTEG_RK4, IF_ATTITUDE),
+  // the full onboard stack: position controller -> attitude controller -> mixer -> rotors
+  CF_G(MODEL_FP, INTEG_EULER, IF_POSITION), CF_G(MODEL_FP, INTEG_RK4, IF_POSITION),
+  CF_G(MODEL_AB, INTEG_EULER, IF_POSITION), CF_G(MODEL_AB, INTEG_RK4, IF_POSITION),
 };
 
 int check(const cf_sim *sim, int n_cmds, int cmd_hold, int n_steps) {
@@ -433,10 +660,16 @@ int check(const cf_sim *sim, int n_cmds, int cmd_hold, int n_steps) {
 
 }  // namespace
 
+static int hist_floats(int model, int iface) {
+  if (model == CF_MODEL_FIRST_PRINCIPLES)
+    return iface == CF_IF_POSITION ? Hist<MODEL_FP, IF_POSITION>::HD : iface == CF_IF_ATTITUDE ? Hist<MODEL_FP, IF_ATTITUDE>::HD
+                                                                                               : Hist<MODEL_FP, IF_ROTOR>::HD;
+  return iface == CF_IF_POSITION ? Hist<MODEL_AB, IF_POSITION>::HD : Hist<MODEL_AB, IF_ATTITUDE>::HD;
+}
+
 extern "C" size_t cf_grad_scratch_bytes(const cf_sim *sim, int n_steps) {
   if (!sim || n_steps < 1) return 0;
-  size_t hd = sim->model == CF_MODEL_FIRST_PRINCIPLES ? Hist<MODEL_FP>::HD : Hist<MODEL_AB>::HD;
-  return sizeof(float) * hd * (size_t)sim->MN * (size_t)n_steps;
+  return sizeof(float) * (size_t)hist_floats(sim->model, sim->p.iface) * (size_t)sim->MN * (size_t)n_steps;
 }
 
 extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
@@ -451,7 +684,7 @@ extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   const Entry *e = nullptr;
   for (const Entry &c : kTable)
     if (c.model == sim->model && c.integ == sim->p.integrator && c.iface == sim->p.iface) e = &c;
-  if (!e) return fail(CF_E_UNSUPPORTED, "cf_grad: interface not differentiated (rotor / attitude for the first-principles model, attitude for the abstracted one)");
+  if (!e) return fail(CF_E_UNSUPPORTED, "cf_grad: interface not differentiated (the torque interface; the abstracted model has no rotor interface)");
   rc = cf_materialise(sim);      // a pending broadcast cf_set_state must be in the planes: the kernel reads them
   if (rc != CF_OK) return rc;
   GradArgs A;
@@ -467,5 +700,33 @@ extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   int used = (n_steps + cmd_hold - 1) / cmd_hold;
   if (used < n_cmds)
     CF_CUDA(cudaMemsetAsync((float4 *)grad_dev + (size_t)used * sim->MN, 0, sizeof(float4) * (size_t)(n_cmds - used) * sim->MN, sim->stream));
+  return CF_OK;
+}
+
+// The same call driven from HOST buffers (the end-to-end path): commands host->device into staging_dev, the kernel, loss
+// and gradient device->host, stream synchronised.  staging_dev: cf_grad_staging_bytes() bytes, 256-byte aligned.
+static size_t align256g(size_t n) { return (n + 255) & ~(size_t)255; }
+extern "C" size_t cf_grad_staging_bytes(const cf_sim *sim, int n_cmds) {
+  if (!sim || n_cmds < 1) return 0;
+  const size_t cb = align256g(sizeof(float) * 4 * (size_t)sim->MN * (size_t)n_cmds);
+  return 2 * cb + align256g(sizeof(float) * (size_t)sim->MN);
+}
+extern "C" int cf_grad_host(cf_sim *sim, const void *cmds_host, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
+                            float *loss_host, void *grad_host, void *staging_dev, size_t staging_bytes, void *scratch_dev,
+                            size_t scratch_bytes) {
+  if (!sim || !cmds_host || !loss_host || !grad_host || !staging_dev) return fail(CF_E_ARG, "NULL argument");
+  if (n_cmds < 1) return fail(CF_E_ARG, "n_cmds >= 1");
+  if (((uintptr_t)staging_dev & 255) != 0) return fail(CF_E_BUFFER, "staging must be 256-byte aligned");
+  if (staging_bytes < cf_grad_staging_bytes(sim, n_cmds)) return fail(CF_E_BUFFER, "staging too small");
+  const size_t raw = sizeof(float) * 4 * (size_t)sim->MN * (size_t)n_cmds, cb = align256g(raw);
+  char *base = (char *)staging_dev;
+  void *cmds_dev = base, *grad_dev = base + cb;
+  float *loss_dev = (float *)(base + 2 * cb);
+  CF_CUDA(cudaMemcpyAsync(cmds_dev, cmds_host, raw, cudaMemcpyHostToDevice, sim->stream));
+  int rc = cf_grad(sim, cmds_dev, n_cmds, cmd_hold, n_steps, goal, loss_dev, grad_dev, scratch_dev, scratch_bytes);
+  if (rc != CF_OK) return rc;
+  CF_CUDA(cudaMemcpyAsync(grad_host, grad_dev, raw, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaMemcpyAsync(loss_host, loss_dev, sizeof(float) * (size_t)sim->MN, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
   return CF_OK;
 }

@@ -326,6 +326,33 @@ Scratch carve_scratch(int n_ctrl, int n_elite, int H) {
   return s;
 }
 
+// ---- the cross-shard selection (reading R31 across ranks) -----------------------------------------------------------------
+// row = [score of the shard's best controller, its GLOBAL controller index, plan (H float4)]
+__global__ void pack_best_kernel(const float *info, const float4 *plan, int n_ctrl, int H, int ctrl_offset, float *row) {
+  const int best = __float_as_int(info[4 * n_ctrl]);
+  if (threadIdx.x == 0) { row[0] = info[4 * best]; row[1] = (float)(best + ctrl_offset); }
+  for (int t = threadIdx.x; t < 4 * H; t += blockDim.x) row[2 + t] = reinterpret_cast<const float *>(plan)[t];
+}
+// the row with the smallest (score as a float32 in IEEE total order with NaN last -- the cost_key order --, global
+// controller index): identical on every rank whatever the order the rows were gathered in
+__global__ void select_row_kernel(const float *rows, int n_rows, int H, float *best_row) {
+  __shared__ int win;
+  const int W = 2 + 4 * H;
+  if (threadIdx.x == 0) {
+    int w = 0;
+    uint32_t kw = cost_key(rows[0]);
+    float iw = rows[1];
+    for (int r = 1; r < n_rows; ++r) {
+      const uint32_t k = cost_key(rows[(size_t)r * W]);
+      const float idx = rows[(size_t)r * W + 1];
+      if (k < kw || (k == kw && idx < iw)) { w = r; kw = k; iw = idx; }
+    }
+    win = w;
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < W; t += blockDim.x) best_row[t] = rows[(size_t)win * W + t];
+}
+
 int check(const cf_sim *sim, const cf_mppi_params *mp) {
   if (!sim || !mp) return fail(CF_E_ARG, "NULL argument");
   if (mp->struct_size != sizeof(cf_mppi_params)) return fail(CF_E_ARG, "cf_mppi_params.struct_size mismatch");
@@ -410,5 +437,24 @@ extern "C" int cf_mppi_iterate_host(cf_sim *sim, const cf_mppi_params *mp, const
   CF_CUDA(cudaMemcpyAsync(info_host, info_dev, sizeof(float) * CF_MPPI_INFO_WORDS(sim->p.n_ctrl), cudaMemcpyDeviceToHost,
                           sim->stream));
   CF_CUDA(cudaStreamSynchronize(sim->stream));
+  return CF_OK;
+}
+
+extern "C" int cf_mppi_pack_best(cf_sim *sim, const cf_mppi_params *mp, const void *info_dev, const void *plan_dev,
+                                 int ctrl_offset, float *row_dev) {
+  int rc = check(sim, mp);
+  if (rc != CF_OK) return rc;
+  if (!info_dev || !plan_dev || !row_dev || ctrl_offset < 0) return fail(CF_E_ARG, "bad argument");
+  pack_best_kernel<<<1, 128, 0, sim->stream>>>((const float *)info_dev, (const float4 *)plan_dev, sim->p.n_ctrl, mp->horizon,
+                                               ctrl_offset, row_dev);
+  CF_CUDA(cudaGetLastError());
+  return CF_OK;
+}
+
+extern "C" int cf_mppi_select(cf_sim *sim, const float *rows_dev, int n_rows, int horizon, float *best_row_dev) {
+  if (!sim || !rows_dev || !best_row_dev) return fail(CF_E_ARG, "NULL argument");
+  if (n_rows < 1 || horizon < 1) return fail(CF_E_ARG, "n_rows, horizon >= 1");
+  select_row_kernel<<<1, 128, 0, sim->stream>>>(rows_dev, n_rows, horizon, best_row_dev);
+  CF_CUDA(cudaGetLastError());
   return CF_OK;
 }

@@ -126,3 +126,22 @@ def test_full_size_batch_sampled_against_the_oracle(cf, W, od):
     assert img.shape == (1024, 64, 64) and np.isfinite(img).all()
     pick = np.concatenate([[0, 1, 1023], np.random.default_rng(0).integers(0, 1024, 45)])
     check_images(od, state[:, pick], wl.model, sc, img[pick])
+
+
+def test_host_buffer_rendering_equals_device_rendering(cf, W):
+    import torch
+    wl = W.depth(seed=4, M=6, width=40, height=24)
+    g = cf.Sim(wl.M, 1, wl.model, wl.params)
+    g.reset(wl.seed)
+    dp = g.depth_params(**wl.notes["scene"])
+    img = g.depth(dp).cpu().numpy()
+    out = torch.empty((wl.M, 24, 40), dtype=torch.float32, pin_memory=True)
+    g.depth_host(dp, out)                                             # the simulator's current poses
+    assert np.array_equal(out.numpy(), img)
+    st = g.get_state().cpu()
+    st[0] += 0.25                                                     # poses supplied by the host: every camera moved in x
+    g.depth_host(dp, out, state_host=st.pin_memory())
+    g2 = cf.Sim(wl.M, 1, wl.model, wl.params)
+    g2.reset(wl.seed)
+    g2.set_state(st.numpy())
+    assert np.array_equal(out.numpy(), g2.depth(dp).cpu().numpy()) and not np.array_equal(out.numpy(), img)

@@ -112,6 +112,58 @@ def test_abstracted_model_gradient_with_jittered_coefficients(cf, cfo, og, integ
     compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
 
 
+def pos_cmds(K, M, p0, seed, amp=0.3):
+    rng = np.random.default_rng(seed)
+    c = np.zeros((K, M, 4), dtype=np.float32)
+    c[..., :3] = p0.T[None] + rng.uniform(-amp, amp, (K, M, 3))
+    c[..., 3] = rng.uniform(-0.4, 0.4, (K, M))
+    return c
+
+
+@pytest.mark.parametrize("model,integrator,hold,n,pre", [(0, 1, 5, 25, 0), (0, 0, 10, 30, 7), (0, 1, 1, 12, 3),
+                                                         (1, 0, 5, 20, 0), (1, 1, 3, 17, 4)])
+def test_position_interface_gradient_through_the_full_controller_stack(cf, cfo, og, model, integrator, hold, n, pre):
+    """PAPER.md:L69 "differentiating through ... the full onboard controller stack": targets of the geometric position
+    controller (C7) -> attitude command -> attitude controller + mixer (C5, C6, first-principles model) -> dynamics.  The
+    runs start `pre` steps off the tick phases, with non-zero controller integrals, several position ticks inside."""
+    M = 130
+    lo, hi = [1.0] * 12, [1.0] * 12
+    lo[0], hi[0] = 0.93, 1.15                                     # the position controller keeps the nominal mass (R11)
+    params = dict(integrator=integrator, iface=3, f_phys=1000.0 if model == 0 else 500.0, f_att=500.0, f_pos=100.0,
+                  init_mode=1, p0_lo=[-1, -1, 0.5], p0_hi=[1, 1, 2], tilt0_max=0.25, rnd_lo=lo, rnd_hi=hi)
+    g, o = cf.Sim(M, 1, model, params), cfo.OracleSim(M, 1, model, params)
+    g.reset(3), o.reset(3)
+    p0 = o.get_state()[:3]
+    if pre:
+        warm = pos_cmds(1, M, p0, seed=99, amp=0.2)
+        g.step(warm, pre, cmd_hold=pre), o.step(warm, pre, cmd_hold=pre)
+    K = -(-n // hold) + 1
+    cmds = pos_cmds(K, M, p0, seed=model * 10 + hold)
+    before = g.get_state().cpu().numpy().copy()
+    L_gpu, g_gpu = g.grad(cmds, n, GOAL, cmd_hold=hold)
+    L_o, g_o = og.value_and_grad(o, cmds, n, hold, GOAL)
+    worst = compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
+    assert (g_gpu[-1] == 0).all().item()
+    assert np.array_equal(g.get_state().cpu().numpy(), before) and g.step_counter == pre
+    assert np.abs(g_o[..., :3]).max() > 0 and np.abs(g_o[..., 3]).max() > 0          # x, y, z and yaw targets are all live
+    print(f"model {model} position interface: worst relative gradient error {worst:.2e}")
+
+
+def test_host_buffer_gradient_equals_device_gradient(cf):
+    import torch
+    M = 200
+    params = dict(FP_TILT, integrator=1, iface=2)
+    g = cf.Sim(M, 1, 0, params)
+    g.reset(5)
+    cmds = att_cmds(4, M, seed=1)
+    L_d, g_d = g.grad(cmds, 10, GOAL, cmd_hold=3)
+    ch = torch.from_numpy(cmds).pin_memory()
+    L_h = torch.empty(M, dtype=torch.float32, pin_memory=True)
+    g_h = torch.empty((4, M, 4), dtype=torch.float32, pin_memory=True)
+    g.grad_host(ch, 10, GOAL, L_h, g_h, cmd_hold=3)
+    assert np.array_equal(L_h.numpy(), L_d.cpu().numpy()) and np.array_equal(g_h.numpy(), g_d.cpu().numpy())
+
+
 def test_saturated_and_broadcast_start_and_unsupported_configurations(cf, cfo, og):
     params = dict(f_phys=1000.0, f_att=500.0, init_mode=0, integrator=1, iface=2)
     g, o = make_pair(cf, cfo, 64, 0, params)
@@ -123,7 +175,7 @@ def test_saturated_and_broadcast_start_and_unsupported_configurations(cf, cfo, o
     L_o, g_o = og.value_and_grad(o, cmds, 10, 2, GOAL)
     compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
     assert (g_gpu[:, :8, 3] == 0).all().item()
-    for bad in (dict(dist_sigma=0.005), dict(Jp=1e-8), dict(iface=3)):
+    for bad in (dict(dist_sigma=0.005), dict(Jp=1e-8), dict(iface=1)):
         s = cf.Sim(4, 1, 0, dict(params, **bad))
         s.reset(1)
         with pytest.raises(cf.CfError) as e:

@@ -259,9 +259,26 @@ def test_a_shard_of_controllers_reproduces_its_slice_of_the_full_run(cf, W):
         assert np.array_equal(gs.cost().cpu().numpy(), cost_f[sl])
         assert np.array_equal(os_["elites"].cpu().numpy(), el_f[2 * rank:2 * rank + 2])
         assert np.array_equal(nom_s.cpu().numpy(), nom_f.cpu().numpy()[2 * rank:2 * rank + 2])
-        rows.append(planner.pack_local_best(os_["info"], os_["plan"], 2, rank).clone())
-    win = int(torch.argmin(torch.stack(rows)[:, 0]))
-    assert int(rows[win][1]) == best_f and np.array_equal(rows[win][2:].reshape(-1, 4).cpu().numpy(), plan_f)
+        mp_ = gs.mppi_params(5, 3, 10, 0.5, 1)
+        rows.append(gs.mppi_pack_best(mp_, os_["info"], os_["plan"], rank * 2).clone())
+        plan1, score1, gidx1 = planner.select_global_plan(gs, mp_, os_, rank)          # world size 1: the shard's own best
+        assert torch.equal(plan1, os_["plan"]) and int(gidx1) == int(rows[-1][1])
+    from oracle import mppi as omppi
+    for order in ([0, 1], [1, 0]):                                                     # the winner does not depend on the row order
+        stacked = torch.stack([rows[k] for k in order]).contiguous()
+        best = gs.mppi_select(stacked, 5).cpu().numpy()
+        assert np.array_equal(best, stacked.cpu().numpy()[omppi.select_rows(stacked.cpu().numpy())])
+        assert int(best[1]) == best_f and np.array_equal(best[2:].reshape(-1, 4), plan_f)
+    # ties -> lowest global controller index, NaN last, -0 before +0 (R31 / R28 key order), against the oracle's rule
+    W_ = 2 + 4 * 5
+    rng = np.random.default_rng(0)
+    for trial in range(20):
+        n = int(rng.integers(1, 9))
+        r = rng.normal(size=(n, W_)).astype(np.float32)
+        r[:, 0] = rng.choice(np.array([1.0, 1.0, -0.0, 0.0, np.nan, 2.5], dtype=np.float32), n)
+        r[:, 1] = rng.permutation(16)[:n]
+        got = gs.mppi_select(torch.as_tensor(r, device="cuda"), 5).cpu().numpy()
+        assert np.array_equal(got, r[omppi.select_rows(r)], equal_nan=True), (trial, r[:, :2])
 
 
 def test_planner_argument_and_state_errors(cf, W):

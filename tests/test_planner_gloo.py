@@ -42,23 +42,31 @@ def _local_update(rank, n_ctrl, seed=5):
     return info, out["plan"].astype(np.float32), out
 
 
+def _pack(info, plan, n_ctrl, rank):
+    """the row cf_mppi_pack_best writes, restated for the CPU run: [score of the local best, GLOBAL controller index, plan]"""
+    best = int(info[4 * n_ctrl:4 * n_ctrl + 1].view(np.int32)[0])
+    return np.concatenate([[info[4 * best], np.float32(best + rank * n_ctrl)], plan.reshape(-1)]).astype(np.float32)
+
+
 def _worker(rank, world, port, out_path):
     sys.path.insert(0, ROOT)
     import torch
     import torch.distributed as dist
-    from oracle import cfo
+    from oracle import cfo, mppi as omppi
     from paper_2606_01478_b200 import planner
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     cfo.set_num_threads(1)
     info, plan, _ = _local_update(rank, N_LOCAL)
-    row = planner.pack_local_best(torch.from_numpy(info), torch.from_numpy(plan), N_LOCAL, rank)
-    gplan, score, gidx = planner.select_global_plan(row)
+    rows = planner.gather_rows(torch.from_numpy(_pack(info, plan, N_LOCAL, rank))).numpy()    # the product's collective
+    assert rows.shape == (world, 2 + 4 * H) and rows[rank, 1] >= rank * N_LOCAL               # rank order
+    best = rows[omppi.select_rows(rows)]                                                       # R31 by the oracle
+    gplan = torch.from_numpy(best[2:].reshape(-1, 4).copy())
     gathered = [torch.empty_like(gplan) for _ in range(world)]
     dist.all_gather(gathered, gplan)
     assert all(torch.equal(g, gplan) for g in gathered)            # every rank holds the same plan
     if rank == 0:
-        np.savez(out_path, plan=gplan.numpy(), score=float(score), gidx=int(gidx))
+        np.savez(out_path, plan=gplan.numpy(), score=float(best[0]), gidx=int(best[1]))
     dist.destroy_process_group()
 
 
@@ -75,15 +83,21 @@ def test_two_ranks_select_the_plan_of_the_single_process_run(tmp_path):
     assert got["score"] == np.float32(ref["score"][ref["best"]])
 
 
-def test_tie_goes_to_the_lowest_global_controller_and_nan_never_wins():
-    import torch
+def test_row_selection_rule_ties_and_nan():
+    """R31 across shards (oracle side; the library's cf_mppi_select is held to it in tests/test_gpu_mppi.py): lowest score,
+    ties -> lowest global controller index whatever the row order, NaN never wins, -0.0 < +0.0 in the total order."""
     sys.path.insert(0, ROOT)
-    from paper_2606_01478_b200 import planner
+    from oracle import mppi as omppi
+    H_ = 2
+    def row(score, idx):
+        return np.concatenate([[score, idx], np.full(4 * H_, idx)]).astype(np.float32)
+    assert omppi.select_rows([row(3.0, 6), row(3.0, 2), row(5.0, 0)]) == 1
+    assert omppi.select_rows([row(np.nan, 0), row(7.0, 3)]) == 1
+    assert omppi.select_rows([row(0.0, 0), row(-0.0, 1)]) == 1
+    assert omppi.select_rows([row(np.nan, 4), row(np.nan, 1)]) == 1
+    assert omppi.select_rows([row(-1.0, 9)]) == 0
     info = np.zeros(12, dtype=np.float32)
-    info[0:8:4] = [3.0, 3.0]
-    info[8:9] = np.array([0], dtype=np.int32).view(np.float32)
-    plan = torch.arange(8, dtype=torch.float32).reshape(2, 4)
-    row = planner.pack_local_best(torch.from_numpy(info), plan, 2, rank=3)
-    assert row[0] == 3.0 and row[1] == 6.0 and torch.equal(row[2:].reshape(2, 4), plan)
-    p, s, g = planner.select_global_plan(row)                       # world size 1: passes through
-    assert torch.equal(p, plan) and int(g) == 6
+    info[0:8:4] = [4.0, 3.0]
+    info[8:9] = np.array([1], dtype=np.int32).view(np.float32)
+    r = _pack(info, np.arange(8, dtype=np.float32).reshape(2, 4), 2, rank=3)
+    assert r[0] == 3.0 and r[1] == 7.0 and np.array_equal(r[2:], np.arange(8))
