@@ -33,12 +33,16 @@ ALGO_FLOPS = {"depth": 4096 * 555,      # per frame: 64 x 64 rays x (16 spheres 
                "grad": 2120, "mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
 BOUND = {"depth": "alu", "grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
 SM_COUNT, FP32_LANES = 148, 128
-# dram__bytes_read.sum + dram__bytes_write.sum of the rollout kernel, one launch, from the `ncu --set full` captures
-# summarised in profiles/r1_<workload>_rollout.md (static: ncu never runs inside bench.py)
-TRAFFIC_NCU = {"cfg2": 5.9e6, "cfg3": 99.1e6, "cfg4": 2.725e9, "cfg5": 4.415e9, "cfg5e": 4.415e9, "mppi": 30.9e6,
-               "grad": 1.680e9, "depth": 0.05e6}
-# (cfg3 / mppi / depth: below the algorithmic bytes because the written planes were still in the 126 MB L2 when the
-#  kernel ended; the figures are what DRAM saw during the launch)
+
+
+def ncu_static():
+    """Per-workload figures of the dominant kernel from the tracked `ncu --set full` captures (profiles/traffic.json, which
+    names the commit and command each figure was captured at): DRAM bytes per launch, FMA-pipe utilisation, SASS flop
+    fraction, issue-slot utilisation.  STATIC: ncu never runs inside bench.py; they are printed beside the live numbers."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    except Exception:
+        return {"workloads": {}}
 
 
 def peaks():
@@ -69,7 +73,7 @@ def algo_bytes_per_launch(wl) -> int:
         sc = wl.notes["scene"]
         return 4 * MN * sc["width"] * sc["height"] + 7 * 4 * MN
     if wl.name == "grad":     # planes in once, history out and back in, commands in, gradient + loss out
-        return (wl.D + 7) * 4 * MN + 2 * wl.n_steps * 24 * 4 * MN + 2 * wl.n_cmds * 16 * MN + 4 * MN
+        return (wl.D + 7) * 4 * MN + 2 * wl.n_steps * 18 * 4 * MN + 2 * wl.n_cmds * 16 * MN + 4 * MN    # history: 18 floats / step
     return cmd + rec + resident + wparam + plan
 
 
@@ -150,7 +154,6 @@ class Runner:
         self.min_dist = torch.empty(wl.M, dtype=torch.float32, device=device) if self.obst else None
         # broadcast resets are folded into the rollout launch and the N = 1 minimum distance comes from its epilogue
         self.launches_per_step = 1 + (1 if (self.obst and wl.N > 1) else 0)
-        self.kernel, self.grid, self.block = self.sim.describe_launch()
         self.planner = name == "mppi"
         self.grad = name == "grad"
         if self.grad:         # one cf_grad launch per step; nothing else moves
@@ -204,6 +207,12 @@ class Runner:
 
     depth = False
 
+    def describe(self):
+        """Kernel name / geometry of the dominant launch (after at least one step: the record mode is part of the name)."""
+        if not (self.grad or self.depth):
+            self.kernel, self.grid, self.block = self.sim.describe_launch()
+        return self.kernel, self.grid, self.block
+
     def step(self):
         wl, sim = self.wl, self.sim
         if self.depth:
@@ -236,18 +245,11 @@ class Runner:
         """The same step through the C ABI with HOST buffers: H2D of this step's inputs and D2H of its results
         (records, or final state + min distance when nothing is recorded) inside the call."""
         wl, sim = self.wl, self.sim
-        if self.depth:        # poses in (the state planes), images out
-            sim.set_state(self.state_pin.to(self.img.device, non_blocking=True))
-            sim.depth(self.dp, out=self.img)
-            self.img_pin.copy_(self.img, non_blocking=True)
-            self.torch.cuda.synchronize()
+        if self.depth:        # poses in (the state planes), images out: cf_depth_host
+            sim.depth_host(self.dp, self.img_pin, state_host=self.state_pin)
             return
-        if self.grad:         # commands in, loss + gradient out (torch copies around the device call: cf_grad has no
-            self.cmds.copy_(self.cmds_pin, non_blocking=True)         # host-buffer variant)
-            self.step()
-            self.loss_pin.copy_(self.loss, non_blocking=True)
-            self.gout_pin.copy_(self.gout, non_blocking=True)
-            self.torch.cuda.synchronize()
+        if self.grad:         # commands in, loss + gradient out: cf_grad_host
+            sim.grad_host(self.cmds_pin, wl.n_steps, wl.notes["goal"], self.loss_pin, self.gout_pin, cmd_hold=wl.cmd_hold)
             return
         if self.planner:      # measured state in (52 B), plan + controller scores out; the nominal stays on the device
             sim.mppi_iterate_host(self.mpar, self.bstate_pin, self.cmds, self.plan_pin, self.info_pin)
@@ -491,6 +493,9 @@ def main():
     ap.add_argument("--sweep", action="store_true",
                     help="Fig. 3B shape (PAPER.md:L63): single drone x 2^k worlds, 50 executions of 50 steps each, "
                          "first-principles model + attitude controller, RK4; prints one JSON line with the table")
+    ap.add_argument("--sweep-swarm", action="store_true",
+                    help="Fig. 3C shape (PAPER.md:L63, L67): worlds x swarm size with the configs[3] recipe (abstracted model, "
+                         "position controller, per-world mass), 20 executions of 50 steps each; one JSON line with the table")
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
@@ -515,7 +520,8 @@ def main():
         line = dict(metric=METRIC, value=value, unit=UNIT, impl="reference", n_gpus=args.gpus, steps=args.steps,
                     warmup=args.warmup, ms_per_step=1e3 * secs / len(rates), higher_is_better=True, scaling="weak",
                     vs_baseline=None, dtype="f64", data="synthetic",
-                    config=dict(workload=name, M=full.M, N=full.N, sub_steps=full.n_steps, note="bounded sample per step"),
+                    config=dict(workload=name, M=wl.M, N=wl.N, sub_steps=wl.n_steps, full_workload_M=full.M,
+                                note="bounded sample of the workload per step: M is the sample's (the last step's)"),
                     cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
                     e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
         print(json.dumps(line))
@@ -556,7 +562,11 @@ def main():
             ach = ALGO_FLOPS[nm] * wl.drone_steps / (k_ms * 1e-3) / 1e12
             roof = dict(bound="alu", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
                         traffic=None, peak_source=f"148 SM x 128 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz")
-        roof["traffic"] = TRAFFIC_NCU.get(nm)
+        st = ncu_static()
+        sw = st.get("workloads", {}).get(nm, {})
+        roof["traffic"] = sw.get("dram_bytes")                      # static, from the tracked ncu capture (see ncu_static)
+        roof["ncu_static"] = dict(sw, captured_at=st.get("commit"), source="profiles/traffic.json") if sw else None
+        R.describe()
         roof.update(kernel=R.kernel, kernel_ms=k_ms, grid=R.grid, block=R.block,
                     hbm_gbs_algorithmic=algo_bytes_per_launch(wl) / (k_ms * 1e-3) / 1e9,
                     algo_flops_per_drone_step=ALGO_FLOPS[nm], algo_bytes_per_launch=algo_bytes_per_launch(wl))
@@ -596,6 +606,26 @@ def main():
             print(json.dumps(dict(sweep="FP + attitude controller, RK4 1 kHz, 50 executions x 50 steps (PAPER.md:L63 protocol), "
                                         "state resident, no L2 flush (the paper's loop re-runs the same buffers)", rows=rows)))
         return 0
+    if args.sweep_swarm:
+        from paper_2606_01478_b200 import cf, workloads as W
+        import numpy as np
+        rows = []
+        for M in (1, 16, 256, 1000, 4096):
+            for N in (1, 16, 256, 4000):
+                wl = W.cfg4(M=M, N=N, n_steps=50)
+                sim = cf.Sim(wl.M, wl.N, wl.model, wl.params, device=device)
+                sim.reset(wl.seed)
+                cm = torch.from_numpy(np.ascontiguousarray(wl.cmds)).to(device)
+                ms = time_steps(lambda: sim.step(cm, 50, cmd_hold=wl.cmd_hold), torch, 20, 3, None)
+                mean, sd = float(np.mean(ms)), float(np.std(ms))
+                rows.append(dict(worlds=M, drones_per_world=N, drones=M * N, ms_per_50_steps=mean, sigma_ms=sd,
+                                 drone_steps_per_sec=M * N * 50 / (mean * 1e-3), world_steps_per_sec=M * 50 / (mean * 1e-3)))
+                del sim, cm
+                torch.cuda.empty_cache()
+        if rank == 0:
+            print(json.dumps(dict(sweep_swarm="AB model + position controller 100 Hz, Euler 500 Hz, per-world mass (configs[3] recipe), "
+                                              "20 executions x 50 steps, state resident, no record, no L2 flush", rows=rows)))
+        return 0
     main_res = measure(name, args.steps, args.warmup, not args.no_e2e)
     others = {}
     if not args.no_others and world == 1:
@@ -624,6 +654,8 @@ def main():
             line["config"]["world_gradients_per_sec"] = main_res["value"] / main_res["sub_steps"]
         if name == "depth":     # the paper's unit: frames per second; a "drone-step" here is one frame
             line["metric"], line["unit"] = "depth_frames_per_sec", "frames/s"
+            if line.get("e2e"):
+                line["e2e"]["unit"] = "frames/s"
             line["config"]["rays_per_sec"] = main_res["value"] * 4096
         if name == "mppi":      # plans per second (the paper's requirement: 50 Hz)
             line["config"]["plans_per_sec"] = 1e3 / main_res["ms_per_step"]
