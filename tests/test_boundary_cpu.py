@@ -65,6 +65,16 @@ def test_workspace_bytes_and_create_validation(cf):
     assert create(4, 4, 0, p, ws=C.c_void_p(0x10000010)) == cf.E_BUFFER        # misaligned
     assert create(4, 4, 0, cf.default_params(0, dict(f_att=300.0))) == cf.E_SHAPE
     assert create(4, 4, 1, cf.default_params(1, dict(iface=cf.IF_ROTOR))) == cf.E_UNSUPPORTED
+    # values the kernels divide by, or that put NaN into the planes, are refused at create
+    lo_bad = [1.0] * 12; lo_bad[6] = 0.0
+    assert create(4, 4, 0, cf.default_params(0, dict(rnd_lo=lo_bad))) == cf.E_ARG           # motor time-constant factor 0
+    lo_bad = [1.0] * 12; lo_bad[0] = -0.5
+    assert create(4, 4, 1, cf.default_params(1, dict(rnd_lo=lo_bad))) == cf.E_ARG           # negative mass factor
+    lo_bad = [1.0] * 12; lo_bad[9] = 1.2
+    assert create(4, 4, 1, cf.default_params(1, dict(rnd_lo=lo_bad))) == cf.E_ARG           # lo > hi
+    assert create(4, 4, 1, cf.default_params(1, dict(cmd_lo=[0.6, -0.5, -3.0, 0.05]))) == cf.E_ARG     # cmd_lo > cmd_hi
+    assert create(4, 4, 1, cf.default_params(1, dict(noise_sigma=[0.1, -0.1, 0.0, 0.0]))) == cf.E_ARG
+    assert create(4, 4, 0, cf.default_params(0, dict(dist_sigma=-1.0))) == cf.E_ARG
     bad = cf.default_params(0)
     bad.struct_size = 8
     assert create(4, 4, 0, bad) == cf.E_ARG
@@ -74,6 +84,7 @@ def test_workspace_bytes_and_create_validation(cf):
     assert L.cf_step(h, fake, 1, 1, 1, 0, None, 0) == cf.E_STATE
     name = C.create_string_buffer(128)
     g, b = C.c_int(), C.c_int()
+    assert L.cf_set_full(h, None, None, None, None, 1 << 32) == cf.E_SHAPE                    # step counter is 32 bits
     assert L.cf_describe_launch(h, name, 128, C.byref(g), C.byref(b)) == cf.OK
     assert name.value.startswith(b"rollout<FP") and g.value * b.value >= 16
     assert L.cf_destroy(h) == cf.OK
