@@ -159,7 +159,8 @@ class Runner:
         if self.grad:         # one cf_grad launch per step; nothing else moves
             self.loss = torch.empty(wl.MN, dtype=torch.float32, device=device)
             self.gout = torch.empty((wl.n_cmds, wl.MN, 4), dtype=torch.float32, device=device)
-            self.kernel = "grad_kernel<FP,INTEG_RK4,IF_ATTITUDE>"
+            self.kernel = "grad_kernel<FP,INTEG_RK4,IF_ATTITUDE,1|2> (forward + backward launch)"
+            self.launches_per_step = 2
             self.block, self.grid = 128, -(-wl.MN // 128)
         if self.planner:      # planning iteration: broadcast reset + fused rollout + update (2 kernels per step)
             n = wl.notes

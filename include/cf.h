@@ -263,8 +263,8 @@ int cf_mppi_select(cf_sim *sim, const float *rows_dev, int n_rows, int horizon, 
  *   neither the planes nor the step counter), driven by cmds_dev [n_cmds][MN] float4 exactly as cf_step would be;
  *   grad_dev [n_cmds][MN] float4 receives dL_i / d cmds[k][i][0..3]  (commands beyond the last used one: 0);
  *   loss_dev [MN] receives L_i.
- * One hand-written reverse-mode kernel: forward sweep parking, per step, only what the backward sweep reads non-linearly
- * in scratch_dev (cf_grad_scratch_bytes = n_steps * HD * MN floats, 16-byte aligned; HD = 16 / 18 / 32 for the
+ * One hand-written reverse-mode kernel (two launches): forward sweep parking, per step, only what the backward sweep reads
+ * non-linearly in scratch_dev (cf_grad_scratch_bytes = (n_steps * HD + 4) * MN floats + 16 bytes, 16-byte aligned; HD = 16 / 18 / 32 for the
  * first-principles model with the rotor / attitude / position interface -- attitude, body rates, rotor speeds, controller
  * integrals, rotor command; position and velocity only when the position controller reads them -- and 8 / 20 for the
  * abstracted model with the attitude / position interface), backward sweep through normalisation, RK4 / Euler, Eqs.
