@@ -406,7 +406,7 @@ extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf
   s->cost_valid = false; s->rearmed = false; s->last_fresh = false; s->last_s0 = 0; s->last_n_steps = s->last_n_cmds = s->last_cmd_hold = 0;
   s->pending_bcast = false; s->md_valid = false;
   s->counters = (Counters *)(base + c.counters); s->rec_table = (uint32_t *)(base + c.rec_table);
-  s->last_rec_mode = REC_NONE;
+  s->last_rec_mode = REC_NONE; s->last_rec_heavy = false;
   s->stream = 0; s->seed = 0; s->s_host = 0; s->n_rec_host = 0; s->have_state = false;
   s->hover_rpm = (float)hover_rpm_nominal(p);
   fill_dev_params(s);
@@ -578,12 +578,12 @@ static EncodeTiledFn encode_tiled_fn() {
   }();
   return fn;
 }
-static bool encode_record_map(CUtensorMap *map, float *record_dev, long long MN, long long n_rec, int D) {
+static bool encode_record_map(CUtensorMap *map, float *record_dev, long long MN, long long n_rec, int D, int group) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
   const cuuint64_t dims[2] = { (cuuint64_t)MN, (cuuint64_t)(n_rec * D) };
   const cuuint64_t strides[1] = { (cuuint64_t)MN * sizeof(float) };      // bytes, a multiple of 16 (MN % 32 == 0)
-  const cuuint32_t box[2] = { 32u, (cuuint32_t)D }, elem[2] = { 1u, 1u };
+  const cuuint32_t box[2] = { 32u, (cuuint32_t)(D * group) }, elem[2] = { 1u, 1u };
   return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, record_dev, dims, strides, box, elem, CU_TENSOR_MAP_INTERLEAVE_NONE,
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -596,12 +596,29 @@ static int pick_block(long long MN) {
   if (warps <= sms * 32) return 64;
   return kMaxBlock;
 }
+// Record-every-step runs (lean kernels): the largest block (<= 512 threads) that leaves the busiest scheduler with no
+// more warps than one-warp blocks would.  The record tensor is [n_rec * D][MN]: a warp writes 128 bytes of each of D rows
+// that lie MN * 4 bytes apart, and what HBM sustains for that pattern grows with the span one SM writes at a time --
+// measured with a write-only kernel of the same pattern (profiles/r2_record_pattern.md): 4.75 TB/s at 32 threads per
+// block, 5.0 at 128, 5.4 at 256, 6.1 - 6.7 at 512 (a linear fill: 6.9).
+static int pick_block_rec(long long MN) {
+  const long long sms = 148, warps = (MN + 31) / 32;
+  auto busiest = [&](long long b) {            // warps on the busiest scheduler with blocks of b warps
+    const long long blocks = (warps + b - 1) / b, per_sm = (blocks + sms - 1) / sms;
+    return (per_sm * b + 3) / 4;
+  };
+  int best = 1;
+  for (int b = 2; b <= kMaxBlockRec / 32; b *= 2)
+    if (busiest(b) <= busiest(1)) best = b;
+  return 32 * best;
+}
 
 static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name, int *grid, int *block) {
   LaunchCfg L;
   const int rec_mode = A ? A->rec_mode : sim->last_rec_mode;    // a dry run describes the kernel of the last cf_step
   if (A) sim->last_rec_mode = A->rec_mode;
-  L.block = pick_block(sim->MN);
+  if (A) sim->last_rec_heavy = A->rec_mode == REC_TMA && A->record_every <= 4 && !(sim->opt & OPT_EXTRAS);
+  L.block = sim->last_rec_heavy ? pick_block_rec(sim->MN) : pick_block(sim->MN);
   L.grid = grid_for(sim->MN, L.block);
   // the kernel stages the parameter rows whenever ITS compile-time options carry OPT_RANDP and N > 1, and the
   // dispatcher may pick a superset instantiation: size the staging area from the instantiation, not from the request
@@ -611,7 +628,7 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
       : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
   if (!found) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
   size_t smem_wp = ((opt_used & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
-  size_t smem_rec = (A && A->rec_mode == REC_TMA) ? kRecBufs * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
+  size_t smem_rec = (A && A->rec_mode == REC_TMA) ? kRecBufs * A->rec_group * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
   L.smem = smem_wp > smem_rec ? smem_wp : smem_rec;
   L.stream = sim->stream;
   if (grid) *grid = L.grid;
@@ -657,9 +674,29 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.record_every = record_every; A.n_rec_cap = (int)n_rec;
   memset(&A.rec_map, 0, sizeof(A.rec_map));
   A.rec_mode = n_rec > 0 ? REC_SCALAR : REC_NONE;
-  if (n_rec > 0 && sim->MN % 32 == 0 && ((uintptr_t)record_dev & 15) == 0 &&
-      encode_record_map(&A.rec_map, record_dev, sim->MN, n_rec, sim->D))
-    A.rec_mode = REC_TMA;
+  memset(&A.rec_map1, 0, sizeof(A.rec_map1));
+  A.rec_group = 1;
+  if (n_rec > 0 && sim->MN % 32 == 0 && ((uintptr_t)record_dev & 15) == 0) {
+    // snapshots per bulk-tensor store: worth it only when records are frequent; bounded by the shared memory the
+    // resident warps can have (two tiles of rec_group * D * 128 bytes per warp; <= 48 KB per block, <= 200 KB per SM with
+    // at most 20 resident warps, the lean kernels' launch bound) and by the number of records of this call
+    int group = 1;
+    if (record_every <= 4 && !(sim->opt & OPT_EXTRAS)) {
+      const int block = pick_block_rec(sim->MN);
+      const long long warps = (sim->MN + 31) / 32, bw = block / 32, blocks = (warps + bw - 1) / bw;
+      long long resident = ((blocks + 147) / 148) * bw;                      // warps on the busiest SM
+      if (resident > 20) resident = 20;
+      const size_t tile = sizeof(float) * sim->D * 32;
+      for (int g = kRecGroupMax; g > 1 && group == 1; --g)
+        if (g <= n_rec && kRecBufs * g * tile * (size_t)resident <= 200 * 1024) group = g;
+    }
+    if (encode_record_map(&A.rec_map, record_dev, sim->MN, n_rec, sim->D, group) &&
+        (group == 1 || encode_record_map(&A.rec_map1, record_dev, sim->MN, n_rec, sim->D, 1))) {
+      if (group == 1) A.rec_map1 = A.rec_map;
+      A.rec_mode = REC_TMA;
+      A.rec_group = group;
+    }
+  }
   A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);
   for (int r = 0; r < 10; ++r) {      // Philox key schedule: k += (0x9E3779B9, 0xBB67AE85) per round
     A.rk[2 * r] = A.seed_lo + (uint32_t)r * 0x9E3779B9u;

@@ -13,6 +13,7 @@ namespace cf {
 constexpr int kMaxObst = 8;
 constexpr int kCtrlPlanes = 14;
 constexpr int kRecTableCap = 4096;
+constexpr int kRecGroupMax = 4;   // snapshots per bulk-tensor store, at most
 constexpr int kRecBufs = 2;       // record staging tiles per warp (TMA path: one in flight, one being filled; 3 and 4
                                   // measured no faster)
 
@@ -87,7 +88,10 @@ struct StepArgs {
                            // [D][32] shared-memory tile; needs MN % 32 == 0 and a 16-byte aligned record buffer)
   uint32_t seed_lo, seed_hi;
   uint32_t rk[20];         // Philox round keys (k0_r, k1_r), r = 0..9, precomputed on the host from the seed
-  alignas(64) CUtensorMap rec_map;   // REC_TMA: the record buffer as the 2-D tensor [n_rec * D][MN], box = 32 x D
+  int rec_group;           // REC_TMA: snapshots per bulk-tensor store (1..kRecGroupMax), chosen by the host from the
+                           // record period and the shared memory the resident warps can have
+  alignas(64) CUtensorMap rec_map;    // REC_TMA: the record buffer as the 2-D tensor [n_rec * D][MN], box = 32 x rec_group * D
+  alignas(64) CUtensorMap rec_map1;   // the same tensor with box = 32 x D (partial last group)
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -661,8 +665,11 @@ enum : int { REC_NONE = 0, REC_SCALAR = 1, REC_TMA = 2, REC_RUNTIME = -1 };
 // configs[3] and the planner); first-principles lean kernels at >= 4 blocks (<= 128 registers, so that the 2048
 // one-warp blocks of configs[4] are all resident: at > 146 registers they spill into a second wave, +50 % time).
 constexpr int kMaxBlock = 128;
+// The lean kernels' bounds are written as ONE block of 640 / 512 threads: the same register caps (<= 96 / <= 128), and
+// blocks of up to 512 threads may be launched -- used when every step is recorded (see pick_block in cf_api.cu).
+constexpr int kMaxBlockRec = 512;
 template <int MODEL, int INTEG, int IFACE, int OPT, int REC>
-__global__ void __launch_bounds__(kMaxBlock, (OPT & OPT_EXTRAS) ? 1 : (MODEL == MODEL_AB ? 5 : 4))
+__global__ void __launch_bounds__((OPT & OPT_EXTRAS) ? kMaxBlock : (MODEL == MODEL_AB ? 640 : 512), 1)
 rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevParams P) {
   constexpr int D = MODEL == MODEL_FP ? 17 : 13;
   constexpr int NP = MODEL == MODEL_FP ? 14 : 11;
@@ -792,13 +799,13 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     int rec_phase = A.record_every > 0 ? (int)(s0 % (uint32_t)A.record_every) : 0;
     int rec_slot = 0;
     const int lane = threadIdx.x & 31;
-    // record staging (REC_TMA): the warp's snapshot is a [D][32] tile (kRecBufs of them, used in turn); one
-    // cp.async.bulk.tensor.2d of the whole tile by lane 0, box = 32 columns x D rows at (column = first drone of the
-    // warp, row = slot * D) of the [n_rec * D][MN] record tensor
-    float *rec_tile = wp_s + warp_u * (kRecBufs * D * 32);
-    const uint32_t rec_tile_sa = (uint32_t)__cvta_generic_to_shared(wp_s) + (uint32_t)warp_u * (kRecBufs * D * 128);
+    // record staging (REC_TMA): the warp's snapshots go to a [rec_group * D][32] tile (kRecBufs of them, used in turn); one
+    // cp.async.bulk.tensor.2d of the whole tile by lane 0, box = 32 columns x rec_group * D rows at (column = first drone
+    // of the warp, row = first slot of the group * D) of the [n_rec * D][MN] record tensor
+    float *rec_tile = wp_s + warp_u * (kRecBufs * A.rec_group * D * 32);
+    const uint32_t rec_tile_sa = (uint32_t)__cvta_generic_to_shared(wp_s) + (uint32_t)warp_u * (kRecBufs * A.rec_group * D * 128);
     const int rec_col = (int)((long long)blockIdx.x * blockDim.x) + warp_u * 32;
-    int rec_buf = 0;
+    int rec_buf = 0, rec_grp = 0;
     // commands.  Buffer mode: one float4 per drone and command, prefetched one command ahead.  Noise mode: the nominal
     // sequence of this world's controller (R26), the same 16 bytes for (nearly) every lane: a plain indexed read-only
     // load at the top of the step, served by L1, with the Philox rounds between it and its use.
@@ -954,18 +961,27 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           rec_phase = 0;
           if (rec_slot < A.n_rec_cap) {
             if (rec_mode == REC_TMA) {
-              tma_store_wait_read<kRecBufs - 1>();    // the engine has read the tile written kRecBufs records ago
-              __syncwarp();
-              // slot and buffer index as provably warp-uniform values (one shuffle): the TMA instruction takes its
-              // operands from uniform registers; without this the compiler wraps it in a per-lane uniformisation loop
-              const int sb = __shfl_sync(0xffffffffu, kRecBufs * rec_slot + rec_buf, 0);
-              float *t = rec_tile + (sb % kRecBufs) * (D * 32);
+              // Consecutive record slots are consecutive row blocks of the record tensor, so K = A.rec_group snapshots
+              // are parked in one [K * D][32] tile and leave with ONE bulk-tensor store: the fence, the elected-lane
+              // issue and its scoreboard waits are paid once per K records.  Two such tiles alternate.
+              if (rec_grp == 0) {
+                tma_store_wait_read<kRecBufs - 1>();  // the engine has read the tile handed over two groups ago
+                __syncwarp();
+              }
+              float *t = rec_tile + (rec_buf * A.rec_group + rec_grp) * (D * 32);
 #pragma unroll
               for (int j = 0; j < D; ++j) t[j * 32 + lane] = x[j];
-              fence_proxy_async_smem();               // generic-proxy writes -> visible to the async proxy
-              __syncwarp();
-              tma_store_tile_2d(&A.rec_map, rec_tile_sa + (sb % kRecBufs) * (D * 128), rec_col, (sb / kRecBufs) * D, lane == 0);
-              rec_buf = (rec_buf + 1) % kRecBufs;
+              if (++rec_grp == A.rec_group) {
+                fence_proxy_async_smem();             // generic-proxy writes -> visible to the async proxy
+                __syncwarp();
+                // first slot and buffer index as provably warp-uniform values (one shuffle): the TMA instruction takes
+                // its operands from uniform registers; without this the compiler wraps it in a per-lane uniformisation loop
+                const int sb = __shfl_sync(0xffffffffu, kRecBufs * (rec_slot + 1 - rec_grp) + rec_buf, 0);
+                tma_store_tile_2d(&A.rec_map, rec_tile_sa + (sb % kRecBufs) * (A.rec_group * D * 128), rec_col,
+                                  (sb / kRecBufs) * D, lane == 0);
+                rec_buf = (rec_buf + 1) % kRecBufs;
+                rec_grp = 0;
+              }
             } else {                                  // one streaming 4-byte store per component (any MN, any alignment)
               float *r = A.record + (size_t)rec_slot * D * MN + i;
 #pragma unroll
@@ -990,7 +1006,19 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{});
       }
     }
-    if (REC == REC_TMA || (REC == REC_RUNTIME && A.rec_mode == REC_TMA)) { tma_store_wait_read<0>(); __syncwarp(); }   // the tiles must outlive the engine's reads
+    if (REC == REC_TMA || (REC == REC_RUNTIME && A.rec_mode == REC_TMA)) {
+      if (rec_grp > 0) {                              // a partial last group leaves record by record (box = D rows)
+        fence_proxy_async_smem();
+        __syncwarp();
+        const int sb = __shfl_sync(0xffffffffu, kRecBufs * (rec_slot - rec_grp) + rec_buf, 0);
+        const int n_tail = __shfl_sync(0xffffffffu, rec_grp, 0);
+        for (int r = 0; r < n_tail; ++r)
+          tma_store_tile_2d(&A.rec_map1, rec_tile_sa + ((sb % kRecBufs) * A.rec_group + r) * (D * 128), rec_col,
+                            (sb / kRecBufs + r) * D, lane == 0);
+      }
+      tma_store_wait_read<0>();                       // the tiles must outlive the engine's reads
+      __syncwarp();
+    }
     // final store
 #pragma unroll
     for (int j = 0; j < D; ++j) A.state[j * MN + i] = x[j];

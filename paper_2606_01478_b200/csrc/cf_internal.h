@@ -26,6 +26,7 @@ struct cf_sim {
   bool last_fresh; long long last_s0; int last_n_steps, last_n_cmds, last_cmd_hold;
   bool pending_bcast, md_valid;
   int last_rec_mode;          // record mode of the last cf_step launch (cf_describe_launch names that kernel)
+  bool last_rec_heavy;        // ... and whether it took the large blocks of record-every-step runs
   Counters *counters;
   uint32_t *rec_table;
   cudaStream_t stream;

@@ -30,7 +30,10 @@ bool launch_fp(int integ, int iface, int opt, int rec_mode, const StepArgs *A, c
   if (!best) return false;
   if (name) *name = best->name;
   if (opt_used) *opt_used = best->opt;
-  if (!dry) best->fn<<<L->grid, L->block, L->smem, L->stream>>>(*A, *P);
+  if (!dry) {
+    if (L->smem > 48 * 1024) cudaFuncSetAttribute(best->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L->smem);
+    best->fn<<<L->grid, L->block, L->smem, L->stream>>>(*A, *P);
+  }
   return true;
 }
 
