@@ -290,6 +290,168 @@ __device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MO
   }
 }
 
+// ---- lean adjoint of the first-principles step (the exact transpose of integrate_fp_lean) -----------------------------
+// The forward sweep runs the rollout kernel's lean step: stage states exist only for (q, w, Omega) -- position and
+// velocity are carried in closed form, p+ = p + h v + h^2/6 (a1 + a2 + a3), v+ = v + h/6 (a1 + 2 a2 + 2 a3 + a4), and the
+// rotor stages are Omega_i = u + e c_i with e = Omega - u.  Its transpose therefore needs, per stage, only the (dw, dq)
+// part of the rates for the recomputation and ONE 10-cotangent VJP of fp_lean_rates (a(3), dw(3), dq(4) -> q, w, Omega);
+// the cotangents of the accelerations come straight from (lam_p, lam_v) and feed nothing else.  Against the generic
+// 17-component pull-back (4 deriv_fp + 4 vjp_deriv_fp + 17-wide RK4 bookkeeping) this is less than half the instructions.
+__device__ __forceinline__ void fp_lean_dwdq(const Plant<MODEL_FP, 0> &pl, const float *q, const float *w, const float *Om,
+                                             float *dw, float *dq) {
+  float w2[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) w2[k] = Om[k] * Om[k];
+  const float A = w2[0] + w2[1], B = w2[2] + w2[3], C = w2[1] + w2[2], Dd = w2[0] + w2[3];
+  const float E = w2[1] + w2[3], G = w2[0] + w2[2];
+  dw[0] = fmaf(pl.cJ[0], w[1] * w[2], pl.ct[0] * (B - A));
+  dw[1] = fmaf(pl.cJ[1], w[2] * w[0], pl.ct[1] * (C - Dd));
+  dw[2] = fmaf(pl.cJ[2], w[0] * w[1], pl.ct[2] * (E - G));
+  dq[0] = fmaf(q[3], w[0], fmaf(q[1], w[2], -(q[2] * w[1])));
+  dq[1] = fmaf(q[3], w[1], fmaf(q[2], w[0], -(q[0] * w[2])));
+  dq[2] = fmaf(q[3], w[2], fmaf(q[0], w[1], -(q[1] * w[0])));
+  dq[3] = -fmaf(q[0], w[0], fmaf(q[1], w[1], q[2] * w[2]));
+}
+__device__ __forceinline__ void fp_lean_dq(const float *q, const float *w, float *dq) {
+  dq[0] = fmaf(q[3], w[0], fmaf(q[1], w[2], -(q[2] * w[1])));
+  dq[1] = fmaf(q[3], w[1], fmaf(q[2], w[0], -(q[0] * w[2])));
+  dq[2] = fmaf(q[3], w[2], fmaf(q[0], w[1], -(q[1] * w[0])));
+  dq[3] = -fmaf(q[0], w[0], fmaf(q[1], w[1], q[2] * w[2]));
+}
+// cotangents (ga, gdw, gdq) of fp_lean_rates at (q, w, Om) -> cotangents gq, gw, gO of its inputs (assigned)
+__device__ __forceinline__ void vjp_fp_lean_rates(const Plant<MODEL_FP, 0> &pl, const float *q, const float *w,
+                                                  const float *Om, const float *ga, const float *gdw, const float *gdq,
+                                                  float *gq, float *gw, float *gO) {
+  // a = (zx, zy, 1/2 - zh) acc2 + fa,  acc2 = kfm2 sum Om^2,  zx = q0 q2 + q3 q1, zy = q1 q2 - q3 q0, zh = q0^2 + q1^2
+  const float s2 = fmaf(Om[0], Om[0], Om[1] * Om[1]) + fmaf(Om[2], Om[2], Om[3] * Om[3]);
+  const float acc2 = pl.kfm2 * s2;
+  const float zx = fmaf(q[0], q[2], q[3] * q[1]), zy = fmaf(q[1], q[2], -(q[3] * q[0])), zh = fmaf(q[0], q[0], q[1] * q[1]);
+  const float g_acc2 = fmaf(zx, ga[0], fmaf(zy, ga[1], (0.5f - zh) * ga[2]));
+  const float gzx = acc2 * ga[0], gzy = acc2 * ga[1], gzh2 = -2.0f * acc2 * ga[2];
+  // dw_j = cJ_j w_a w_b + ct_j (signed sum of Om^2): signs (B - A), (C - Dd), (E - G)
+  const float t0 = pl.ct[0] * gdw[0], t1 = pl.ct[1] * gdw[1], t2 = pl.ct[2] * gdw[2];
+  const float s = pl.kfm2 * g_acc2, sm = s - t0, sp = s + t0, u = t1 + t2, v = t1 - t2;
+  gO[0] = 2.0f * Om[0] * (sm - u);
+  gO[1] = 2.0f * Om[1] * (sm + u);
+  gO[2] = 2.0f * Om[2] * (sp + v);
+  gO[3] = 2.0f * Om[3] * (sp - v);
+  const float c0 = pl.cJ[0] * gdw[0], c1 = pl.cJ[1] * gdw[1], c2 = pl.cJ[2] * gdw[2];
+  // dq = 2 q-dot:  dq0 = q3 w0 + q1 w2 - q2 w1, dq1 = q3 w1 + q2 w0 - q0 w2, dq2 = q3 w2 + q0 w1 - q1 w0, dq3 = -(q . w)
+  gw[0] = fmaf(w[2], c1, fmaf(w[1], c2, fmaf(q[3], gdq[0], fmaf(q[2], gdq[1], -fmaf(q[1], gdq[2], q[0] * gdq[3])))));
+  gw[1] = fmaf(w[2], c0, fmaf(w[0], c2, fmaf(q[3], gdq[1], fmaf(q[0], gdq[2], -fmaf(q[2], gdq[0], q[1] * gdq[3])))));
+  gw[2] = fmaf(w[1], c0, fmaf(w[0], c1, fmaf(q[3], gdq[2], fmaf(q[1], gdq[0], -fmaf(q[0], gdq[1], q[2] * gdq[3])))));
+  gq[0] = fmaf(q[2], gzx, fmaf(q[0], gzh2, fmaf(w[1], gdq[2], -fmaf(q[3], gzy, fmaf(w[2], gdq[1], w[0] * gdq[3])))));
+  gq[1] = fmaf(q[3], gzx, fmaf(q[2], gzy, fmaf(q[1], gzh2, fmaf(w[2], gdq[0], -fmaf(w[0], gdq[2], w[1] * gdq[3])))));
+  gq[2] = fmaf(q[0], gzx, fmaf(q[1], gzy, fmaf(w[0], gdq[1], -fmaf(w[1], gdq[0], w[2] * gdq[3]))));
+  gq[3] = fmaf(q[1], gzx, fmaf(w[0], gdq[0], fmaf(w[1], gdq[1], fmaf(w[2], gdq[2], -(q[0] * gzy)))));
+}
+
+// lam (cotangent of the post-step state, 17 components) -> cotangent of the pre-step state; gu accumulates the
+// cotangent of the held rotor command u.  x: pre-step state, only q (3..6), w (10..12), Omega (13..16) are read.
+template <int INTEG>
+__device__ __forceinline__ void step_backward_fp_lean(const DevParams &P, const Plant<MODEL_FP, 0> &pl, const float *x,
+                                                      const float *u, float *lam, float *gu) {
+  const float *q = x + 3, *w = x + 10, *Om = x + 13;
+  float *lp = lam, *lq = lam + 3, *lv = lam + 7, *lw = lam + 10, *lO = lam + 13;
+  float e[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) e[k] = Om[k] - u[k];
+  const float hq = 0.5f * P.h;
+  if constexpr (INTEG == INTEG_EULER) {
+    float dq1[4], qt[4];
+    fp_lean_dq(q, w, dq1);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) qt[j] = fmaf(hq, dq1[j], q[j]);
+    const float inv = rsqrtf(fmaf(qt[0], qt[0], fmaf(qt[1], qt[1], fmaf(qt[2], qt[2], qt[3] * qt[3]))));
+    float dot = 0.f;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qt[j] *= inv; dot = fmaf(qt[j], lq[j], dot); }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) lq[j] = (lq[j] - qt[j] * dot) * inv;
+    float ga[3], gdw[3], gdq[4], gq[4], gw[3], gO[4];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { ga[j] = P.h * lv[j]; gdw[j] = P.h * lw[j]; }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) gdq[j] = hq * lq[j];
+    vjp_fp_lean_rates(pl, q, w, Om, ga, gdw, gdq, gq, gw, gO);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { lv[j] = fmaf(P.h, lp[j], lv[j]); lw[j] += gw[j]; }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      lq[j] += gq[j];
+      const float ge = fmaf(pl.rho1, lO[j], gO[j]);
+      gu[j] += (gO[j] + lO[j]) - ge;
+      lO[j] = ge;
+    }
+  } else {
+    float q2[4], q3[4], q4[4], w2[3], w3[3], w4[3], O2[4], O3[4], O4[4], dw[3], dq[4], qt[4];
+    fp_lean_dwdq(pl, q, w, Om, dw, dq);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qt[j] = dq[j]; q2[j] = fmaf(0.5f * hq, dq[j], q[j]); O2[j] = fmaf(e[j], pl.rc2, u[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) w2[j] = fmaf(P.half_h, dw[j], w[j]);
+    fp_lean_dwdq(pl, q2, w2, O2, dw, dq);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qt[j] = fmaf(2.0f, dq[j], qt[j]); q3[j] = fmaf(0.5f * hq, dq[j], q[j]); O3[j] = fmaf(e[j], pl.rc3, u[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) w3[j] = fmaf(P.half_h, dw[j], w[j]);
+    fp_lean_dwdq(pl, q3, w3, O3, dw, dq);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qt[j] = fmaf(2.0f, dq[j], qt[j]); q4[j] = fmaf(hq, dq[j], q[j]); O4[j] = fmaf(e[j], pl.rc4, u[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) w4[j] = fmaf(P.h, dw[j], w[j]);
+    fp_lean_dq(q4, w4, dq);
+    const float hq6 = 0.5f * P.h_sixth, h2_6 = P.h * P.h_sixth;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) qt[j] = fmaf(hq6, qt[j] + dq[j], q[j]);
+    // q+ = qt / |qt|:  g_qt = (g - q+ (q+ . g)) / |qt|
+    const float inv = rsqrtf(fmaf(qt[0], qt[0], fmaf(qt[1], qt[1], fmaf(qt[2], qt[2], qt[3] * qt[3]))));
+    float dot = 0.f;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { qt[j] *= inv; dot = fmaf(qt[j], lq[j], dot); }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) lq[j] = (lq[j] - qt[j] * dot) * inv;
+    // stage cotangents, last stage first
+    float gaA[3], gaB[3], gaC[3], lw6[3], lq6[4];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      gaC[j] = P.h_sixth * lv[j];
+      const float hp = h2_6 * lp[j];
+      gaA[j] = hp + gaC[j];
+      gaB[j] = fmaf(2.0f, gaC[j], hp);
+      lw6[j] = P.h_sixth * lw[j];
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) lq6[j] = hq6 * lq[j];
+    float gdw[3], gdq[4], gq[4], gw[3], gO[4], ge[4], gus[4];
+    vjp_fp_lean_rates(pl, q4, w4, O4, gaC, lw6, lq6, gq, gw, gO);                     // k4
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { ge[j] = pl.rc4 * gO[j]; gus[j] = gO[j]; lq[j] += gq[j]; gdq[j] = fmaf(hq, gq[j], 2.0f * lq6[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { lw[j] += gw[j]; gdw[j] = fmaf(P.h, gw[j], 2.0f * lw6[j]); }
+    vjp_fp_lean_rates(pl, q3, w3, O3, gaB, gdw, gdq, gq, gw, gO);                     // k3
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { ge[j] = fmaf(pl.rc3, gO[j], ge[j]); gus[j] += gO[j]; lq[j] += gq[j]; gdq[j] = fmaf(0.5f * hq, gq[j], 2.0f * lq6[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { lw[j] += gw[j]; gdw[j] = fmaf(P.half_h, gw[j], 2.0f * lw6[j]); }
+    vjp_fp_lean_rates(pl, q2, w2, O2, gaB, gdw, gdq, gq, gw, gO);                     // k2
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { ge[j] = fmaf(pl.rc2, gO[j], ge[j]); gus[j] += gO[j]; lq[j] += gq[j]; gdq[j] = fmaf(0.5f * hq, gq[j], lq6[j]); }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { lw[j] += gw[j]; gdw[j] = fmaf(P.half_h, gw[j], lw6[j]); }
+    vjp_fp_lean_rates(pl, q, w, Om, gaA, gdw, gdq, gq, gw, gO);                       // k1
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { lw[j] += gw[j]; lv[j] = fmaf(P.h, lp[j], lv[j]); }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      lq[j] += gq[j];
+      const float g_e = fmaf(pl.rho4, lO[j], ge[j] + gO[j]);
+      gu[j] += (gus[j] + gO[j] + lO[j]) - g_e;
+      lO[j] = g_e;
+    }
+  }
+}
+
 // ---- VJP of the geometric position controller tick (C7, reading R16) ----------------------------------------------------
 // inputs of the tick: p, v (state), zB (body z axis in the world frame), target = (x, y, z, yaw), ip (integral before).
 // cotangents in: g_att[4] of the attitude command (roll, pitch, yaw, F) the tick produced, g_ipn[3] of the integral
@@ -488,17 +650,18 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   int att_phase = (int)(A.s0 % (uint32_t)P.att_div), pos_phase = (int)(A.s0 % (uint32_t)P.pos_div);
   float4 *const lam0 = A.hist + ((size_t)A.n_steps * HD * MN + 3) / 4;       // [MN] float4 after the history (split launches)
   if constexpr (PHASE != 2)
-  for (int t = 0; t < A.n_steps; ++t) {
+  for (int t = 0, hold_phase = 0, k_cmd = 0; t < A.n_steps; ++t) {      // t = k_cmd * cmd_hold + hold_phase, no division
     float rec[HP];                                          // pre-step state and controller state of this step
     pack(rec);
-    if (t % A.cmd_hold == 0) {
-      float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
+    if (hold_phase == 0) {
+      float4 c4 = __ldg(A.cmds + (size_t)k_cmd * MN + i);
       cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
       if (FP && IFACE == IF_ROTOR) {
 #pragma unroll
         for (int j = 0; j < 4; ++j) rpm_cmd[j] = clipf(cmd[j], P.rpm_min, P.rpm_max);
       }
     }
+    if (++hold_phase == A.cmd_hold) { hold_phase = 0; ++k_cmd; }
     if (POS) {
       if (pos_phase == 0) {
         float zB[3], sn[3], cs[3];
@@ -559,6 +722,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   pos_phase = (int)((A.s0 + (uint32_t)A.n_steps - 1u) % (uint32_t)P.pos_div);
 #pragma unroll
   for (int j = 0; j < D; ++j) x[j] = 0.f;                   // components that are not parked enter only linearly
+  int hold_phase = (A.n_steps - 1) % A.cmd_hold, k_cmd = (A.n_steps - 1) / A.cmd_hold;    // of step t, kept by counting
   for (int t = A.n_steps - 1; t >= 0; --t) {
     float rec[HP];
     if (t > 0) {            // pull the previous step's record towards L2 while this step's pull-back computes
@@ -602,8 +766,8 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
       for (int j = 0; j < 3; ++j) { x[3 + j] = rec[j]; x[9 + j] = rec[3 + j]; }
       x[12] = rec[6];
     }
-    if (t % A.cmd_hold == A.cmd_hold - 1 || t == A.n_steps - 1) {             // entering the run of command t / hold
-      float4 c4 = __ldg(A.cmds + (size_t)(t / A.cmd_hold) * MN + i);
+    if (hold_phase == A.cmd_hold - 1 || t == A.n_steps - 1) {                 // entering the run of command k_cmd
+      float4 c4 = __ldg(A.cmds + (size_t)k_cmd * MN + i);
       cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
     }
     const float *acmd = POS ? att_cmd : cmd;
@@ -611,7 +775,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     // (tried and rejected, measured: the four RK4 stages of this pull-back rolled into run-time loops with the stage
     //  states in shared memory -- "no instruction" stalls 1.03 -> 0.13 per issue, issue-active 68 -> 79 %, but 27 % more
     //  instructions because the straight-line form lets the compiler drop dead parts of every stage: 0.80 -> 0.87 ms)
-    if (FP) step_backward<MODEL, INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
+    if constexpr (FP) step_backward_fp_lean<INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
     else step_backward<MODEL, INTEG>(P, pl, x, acmd, lam, g_acmd);
     if (HAS_ATT) {
       if (att_phase == 0) {
@@ -637,14 +801,17 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
       }
       pos_phase = pos_phase == 0 ? P.pos_div - 1 : pos_phase - 1;
     }
-    if (t % A.cmd_hold == 0) {                                                 // the fetch step of command t / hold
+    if (hold_phase == 0) {                                                     // the fetch step of command k_cmd
       if (FP && IFACE == IF_ROTOR) {
 #pragma unroll
         for (int j = 0; j < 4; ++j) { g_cmd[j] = (cmd[j] > P.rpm_min && cmd[j] < P.rpm_max) ? g_rpm[j] : 0.f; g_rpm[j] = 0.f; }
       }
-      A.grad[(size_t)(t / A.cmd_hold) * MN + i] = make_float4(g_cmd[0], g_cmd[1], g_cmd[2], g_cmd[3]);
+      A.grad[(size_t)k_cmd * MN + i] = make_float4(g_cmd[0], g_cmd[1], g_cmd[2], g_cmd[3]);
 #pragma unroll
       for (int j = 0; j < 4; ++j) g_cmd[j] = 0.f;
+      hold_phase = A.cmd_hold - 1; --k_cmd;
+    } else {
+      --hold_phase;
     }
   }
 }
