@@ -272,9 +272,15 @@ int cf_mppi_select(cf_sim *sim, const float *rows_dev, int n_rows, int horizon, 
  * PAPER.md:L69).  Where a clip of the method is active (rotor thrust / speed limits, controller integrals, thrust and tilt
  * limits, rotor-interface command limits) the derivative is taken as 0 (reading R33); the controller tick schedules
  * follow the global step counter.
- * Supported: CF_CMD_BUFFER; rotor, attitude and position interface (first-principles), attitude and position (abstracted);
- * Euler and RK4; per-world randomised parameters; no disturbances, no fidelity extras, no torque interface
- * (CF_E_UNSUPPORTED otherwise).  goal: 3 floats on the HOST.
+ * Supported: CF_CMD_BUFFER; every interface of the first-principles model (rotor, torque, attitude, position), attitude
+ * and position of the abstracted model; Euler and RK4; per-world randomised parameters.  Configurations with force
+ * disturbances (the differentiated rollout draws the same Philox forces as cf_step would from the current
+ * step counter), any fidelity extra (full Eq. (6), thrust / torque polynomials incl. the mixer's inverse, Eq. (5), body
+ * drag, the simplified abstracted model of PAPER.md:L354) or the torque interface run the GENERAL adjoint kernels: the
+ * generic 17 / 13-component pull-back and a full record per step, HD = 32 (first-principles) / 20 (abstracted).  Full
+ * Eq. (6) is only piecewise smooth (its coefficients switch with the sign of a rotor's speed error): the gradient is
+ * that of the branch taken.  CF_E_UNSUPPORTED: CF_CMD_NOMINAL_PLUS_NOISE (no command buffer to differentiate with respect
+ * to).  goal: 3 floats on the HOST.
  * cf_grad_host: the same from HOST buffers -- cmds_host [n_cmds][MN] float4 in, loss_host [MN] and grad_host
  * [n_cmds][MN] float4 out, through staging_dev (cf_grad_staging_bytes(), 256-byte aligned, caller-owned device memory);
  * synchronises the stream. */

@@ -11,7 +11,9 @@
 // (6) and (7)-(10)), the motor mixer (sqrt and clips: derivative 0 where a clip is active, reading R33) and the attitude
 // controller (rotation-matrix error, clipped integral, desired rotation from the commanded Euler angles).  The adjoint
 // of a held command accumulates over the steps / ticks that used it and is written when its fetch step is reached.
-// The simulator state is not modified.
+// The simulator state is not modified.  Configurations with fidelity extras, force disturbances or the torque interface run
+// the GENERAL instantiations (OPT = GOPT): generic integrator and 17 / 13-wide pull-back, VJPs of full Eq. (6), the thrust
+// / torque polynomials, Eq. (5), body drag and the simplified abstracted model, the disturbance re-drawn from Philox.
 #include "cf_internal.h"
 
 using namespace cf;
@@ -28,6 +30,8 @@ struct GradArgs {
   int n_steps, cmd_hold, n_cmds;
   uint32_t s0;
   float goal[3];
+  long long world_offset;
+  uint32_t rk[20];         // Philox round keys of the simulator's seed (general kernels: the DIST stream)
 };
 
 template <int MODEL> struct Dim { static constexpr int D = MODEL == MODEL_FP ? 17 : 13; };
@@ -104,17 +108,218 @@ __device__ __forceinline__ void vjp_deriv_ab(const DevParams &P, const Plant<MOD
   gu[3] += pl.ctau * a_f;
 }
 
-template <int MODEL>
-__device__ __forceinline__ void vjp_deriv(const DevParams &P, const Plant<MODEL, 0> &pl, const float *x, const float *a,
-                                          float *gx, float *gu) {
-  if constexpr (MODEL == MODEL_FP) vjp_deriv_fp(P, pl, x, a, gx, gu);
-  else vjp_deriv_ab(P, pl, x, a, gx, gu);
+// ---- shared pieces of the controller VJPs -----------------------------------------------------------------------------
+// R = quat_to_R(q): cotangent GR[i][j] = dL/dR_ij -> g_q (accumulated)
+__device__ __forceinline__ void vjp_quat_to_R(const float *q, const float GR[3][3], float *g_q) {
+  const float x = q[0], y = q[1], z = q[2], ww = q[3];
+  g_q[0] += 2.0f * (y * (GR[0][1] + GR[1][0]) + z * (GR[0][2] + GR[2][0]) + ww * (GR[2][1] - GR[1][2])) - 4.0f * x * (GR[1][1] + GR[2][2]);
+  g_q[1] += 2.0f * (x * (GR[0][1] + GR[1][0]) + z * (GR[1][2] + GR[2][1]) + ww * (GR[0][2] - GR[2][0])) - 4.0f * y * (GR[0][0] + GR[2][2]);
+  g_q[2] += 2.0f * (x * (GR[0][2] + GR[2][0]) + y * (GR[1][2] + GR[2][1]) + ww * (GR[1][0] - GR[0][1])) - 4.0f * z * (GR[0][0] + GR[1][1]);
+  g_q[3] += 2.0f * (x * (GR[2][1] - GR[1][2]) + y * (GR[0][2] - GR[2][0]) + z * (GR[1][0] - GR[0][1]));
+}
+// Rd = Rz(yaw) Ry(pitch) Rx(roll) (reading R13) from its sines / cosines
+__device__ __forceinline__ void euler_R_from_sc(const float *sn, const float *cs, float Rd[3][3]) {
+  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
+  Rd[0][0] = cy * cp; Rd[0][1] = cy * sp * sr - sy * cr; Rd[0][2] = cy * sp * cr + sy * sr;
+  Rd[1][0] = sy * cp; Rd[1][1] = sy * sp * sr + cy * cr; Rd[1][2] = sy * sp * cr - cy * sr;
+  Rd[2][0] = -sp;     Rd[2][1] = cp * sr;                Rd[2][2] = cp * cr;
+}
+// cotangent GD[i][j] = dL/dRd_ij -> (roll, pitch, yaw) (accumulated): d/droll rotates columns 1, 2; d/dyaw rotates rows
+// 0, 1; d/dpitch written out
+__device__ __forceinline__ void vjp_euler_R(const float Rd[3][3], const float *sn, const float *cs, const float GD[3][3],
+                                            float *g_ang) {
+  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
+  g_ang[0] += GD[0][1] * Rd[0][2] - GD[0][2] * Rd[0][1] + GD[1][1] * Rd[1][2] - GD[1][2] * Rd[1][1] + GD[2][1] * Rd[2][2] - GD[2][2] * Rd[2][1];
+  g_ang[1] += GD[0][0] * (-cy * sp) + GD[0][1] * (cy * cp * sr) + GD[0][2] * (cy * cp * cr)
+            + GD[1][0] * (-sy * sp) + GD[1][1] * (sy * cp * sr) + GD[1][2] * (sy * cp * cr)
+            + GD[2][0] * (-cp) + GD[2][1] * (-sp * sr) + GD[2][2] * (-sp * cr);
+  g_ang[2] += -GD[0][0] * Rd[1][0] - GD[0][1] * Rd[1][1] - GD[0][2] * Rd[1][2]
+            + GD[1][0] * Rd[0][0] + GD[1][1] * Rd[0][1] + GD[1][2] * Rd[0][2];
+}
+// ---- the general kernels (fidelity extras, disturbances, torque interface): option set of their device functions ------
+constexpr int GOPT = OPT_EXTRAS | OPT_DIST;
+
+// body drag  d = R (Ca . (R^T v)) / m  (Eq. (3) / Eq. (8) with C_a != 0): cotangent gd of d -> g_v (accumulated) and the
+// cotangent GR of the rotation matrix (assigned)
+__device__ __forceinline__ void vjp_drag(const DevParams &P, float inv_m, const float R[3][3], const float *v, const float *gd,
+                                         float *g_v, float GR[3][3]) {
+  float b[3], gc[3], gb[3];
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    b[j] = R[0][j] * v[0] + R[1][j] * v[1] + R[2][j] * v[2];                         // body-frame velocity
+    gc[j] = (R[0][j] * gd[0] + R[1][j] * gd[1] + R[2][j] * gd[2]) * inv_m;           // cotangent of c = Ca . b
+    gb[j] = P.Ca[j] * gc[j];
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    g_v[i] += R[i][0] * gb[0] + R[i][1] * gb[1] + R[i][2] * gb[2];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) GR[i][j] = gd[i] * inv_m * (P.Ca[j] * b[j]) + v[i] * gb[j];
+  }
+}
+
+// ---- VJP of the first-principles derivative with the fidelity extras (deriv_fp<OPT_EXTRAS>): asymmetric + quadratic
+// rotor dynamics (full Eq. (6)), thrust / torque polynomials, Eq. (5) gyroscopic and reaction torque (reading R2), body
+// drag.  The disturbance force is additive and has no derivative.  u = held rotor command.
+__device__ __forceinline__ void vjp_deriv_fp_ex(const DevParams &P, const Plant<MODEL_FP, GOPT> &pl, const float *x,
+                                                const float *u, const float *a, float *gx, float *gu) {
+  const float *q = x + 3, *v = x + 7, *w = x + 10, *Om = x + 13;
+  const float *a_p = a, *a_q = a + 3, *a_v = a + 7, *a_w = a + 10, *a_Om = a + 13;
+  float *g_q = gx + 3, *g_v = gx + 7, *g_w = gx + 10, *g_Om = gx + 13;
+#pragma unroll
+  for (int j = 0; j < 3; ++j) g_v[j] += a_p[j];                                       // Eq. (1)
+  float f[4], dOm[4], cvk[4], cdk[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    float e = u[k] - Om[k];
+    bool up = e >= 0.0f;
+    cvk[k] = up ? pl.cv : pl.cv_dn; cdk[k] = up ? pl.cd_up : pl.cd_dn;
+    dOm[k] = cvk[k] * e + cdk[k] * (u[k] * u[k] - Om[k] * Om[k]);
+    f[k] = pl.kf0 + Om[k] * (pl.kf1 + pl.kf2 * Om[k]);
+  }
+  const float F = (f[0] + f[1]) + (f[2] + f[3]);
+  // Eq. (3): dv = zB F/m + f_dist/m - g e_z (+ drag)
+  float acc = F * pl.inv_m;
+  float zx = 2.0f * (q[0] * q[2] + q[3] * q[1]), zy = 2.0f * (q[1] * q[2] - q[3] * q[0]);
+  float zz = 1.0f - 2.0f * (q[0] * q[0] + q[1] * q[1]);
+  float gF = (zx * a_v[0] + zy * a_v[1] + zz * a_v[2]) * pl.inv_m;
+  float gzx = a_v[0] * acc, gzy = a_v[1] * acc, gzz = a_v[2] * acc;
+  g_q[0] += 2.0f * (q[2] * gzx - q[3] * gzy) - 4.0f * q[0] * gzz;
+  g_q[1] += 2.0f * (q[3] * gzx + q[2] * gzy) - 4.0f * q[1] * gzz;
+  g_q[2] += 2.0f * (q[0] * gzx + q[1] * gzy);
+  g_q[3] += 2.0f * (q[1] * gzx - q[0] * gzy);
+  if (P.has_drag) {
+    float R[3][3], GR[3][3];
+    quat_to_R(q, R);
+    vjp_drag(P, pl.inv_m, R, v, a_v, g_v, GR);
+    vjp_quat_to_R(q, GR, g_q);
+  }
+  // Eq. (4): dw = tau/J + cJ (w x w terms); tau from the mixing matrix C1 (+ Eq. (5))
+  float gt[3] = { a_w[0] * pl.inv_J[0], a_w[1] * pl.inv_J[1], a_w[2] * pl.inv_J[2] };
+  float gS = 0.0f, gdS = 0.0f;
+  if (P.has_gyro) {     // tau += Jp (-w_y S, +w_x S, -dS), S = W1 - W2 + W3 - W4 (rad/s)
+    const float S = (Om[0] - Om[1]) + (Om[2] - Om[3]);
+    g_w[1] -= P.Jp_rad * S * gt[0];
+    g_w[0] += P.Jp_rad * S * gt[1];
+    gS = P.Jp_rad * (w[0] * gt[1] - w[1] * gt[0]);
+    gdS = -P.Jp_rad * gt[2];
+  }
+  const float sx[4] = { -1, -1, 1, 1 }, sy[4] = { -1, 1, 1, -1 }, sz[4] = { -1, 1, -1, 1 }, sd[4] = { 1, -1, 1, -1 };
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const float gfk = gF + P.lever * (sx[k] * gt[0] + sy[k] * gt[1]);                 // cotangent of the rotor thrust f_k
+    const float gmk = sz[k] * gt[2];                                                  // ... of the rotor drag torque m_k
+    const float aO = a_Om[k] + sd[k] * gdS;                                           // ... of dOm_k
+    g_Om[k] += gfk * (pl.kf1 + 2.0f * pl.kf2 * Om[k]) + gmk * (pl.km1 + 2.0f * pl.km2 * Om[k]) + sd[k] * gS
+             - aO * (cvk[k] + 2.0f * cdk[k] * Om[k]);                                 // Eq. (6)
+    gu[k] += aO * (cvk[k] + 2.0f * cdk[k] * u[k]);
+  }
+  g_w[1] += pl.cJ[0] * w[2] * a_w[0]; g_w[2] += pl.cJ[0] * w[1] * a_w[0];
+  g_w[2] += pl.cJ[1] * w[0] * a_w[1]; g_w[0] += pl.cJ[1] * w[2] * a_w[1];
+  g_w[0] += pl.cJ[2] * w[1] * a_w[2]; g_w[1] += pl.cJ[2] * w[0] * a_w[2];
+  // Eq. (2): dq = 1/2 q (x) (w, 0)
+  float bx = 0.5f * a_q[0], by = 0.5f * a_q[1], bz = 0.5f * a_q[2], bw = 0.5f * a_q[3];
+  g_q[3] += w[0] * bx + w[1] * by + w[2] * bz;
+  g_q[0] += -w[2] * by + w[1] * bz - w[0] * bw;
+  g_q[1] += w[2] * bx - w[0] * bz - w[1] * bw;
+  g_q[2] += -w[1] * bx + w[0] * by - w[2] * bw;
+  g_w[0] += q[3] * bx + q[2] * by - q[1] * bz - q[0] * bw;
+  g_w[1] += -q[2] * bx + q[3] * by + q[0] * bz - q[1] * bw;
+  g_w[2] += q[1] * bx - q[0] * by + q[3] * bz - q[2] * bw;
+}
+
+// ---- VJP of the abstracted derivative with the extras (deriv_ab<OPT_EXTRAS>): body drag, simplified model of
+// PAPER.md:L354 (ab_thrust_dyn = 0: the thrust command acts directly, f_Sigma has no dynamics)
+__device__ __forceinline__ void vjp_deriv_ab_ex(const DevParams &P, const Plant<MODEL_AB, GOPT> &pl, const float *x,
+                                                const float *u, const float *a, float *gx, float *gu) {
+  float sn[3], cs[3];
+  sincos3_step(x + 3, sn, cs);
+  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
+  const float *a_p = a, *a_ps = a + 3, *a_v = a + 6, *a_dps = a + 9;
+  const float a_f = a[12];
+  const bool simple = !P.ab_thrust_dyn;
+  float zx = cy * sp * cr + sy * sr, zy = sy * sp * cr - cy * sr, zz = cp * cr;
+  float acc = (P.ab_cf * (simple ? u[3] : x[12])) * pl.inv_m;
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    gx[6 + j] += a_p[j];
+    gx[9 + j] += a_ps[j] + pl.b[j] * a_dps[j];
+    gx[3 + j] += pl.a[j] * a_dps[j];
+    gu[j] += pl.c[j] * a_dps[j];
+  }
+  float dzr[3] = { -cy * sp * sr + sy * cr, -sy * sp * sr - cy * cr, -cp * sr };
+  float dzp[3] = { cy * cp * cr, sy * cp * cr, -sp * cr };
+  float dzy[3] = { -sy * sp * cr + cy * sr, cy * sp * cr + sy * sr, 0.0f };
+  gx[3] += (dzr[0] * a_v[0] + dzr[1] * a_v[1] + dzr[2] * a_v[2]) * acc;
+  gx[4] += (dzp[0] * a_v[0] + dzp[1] * a_v[1] + dzp[2] * a_v[2]) * acc;
+  gx[5] += (dzy[0] * a_v[0] + dzy[1] * a_v[1]) * acc;
+  const float g_fS = (zx * a_v[0] + zy * a_v[1] + zz * a_v[2]) * (P.ab_cf * pl.inv_m);
+  if (simple) {
+    gu[3] += g_fS;
+  } else {
+    gx[12] += g_fS - pl.ctau * a_f;                                                   // Eq. (9)
+    gu[3] += pl.ctau * a_f;
+  }
+  if (P.has_drag) {
+    float R[3][3], GR[3][3];
+    euler_R_from_sc(sn, cs, R);
+    vjp_drag(P, pl.inv_m, R, x + 6, a_v, gx + 6, GR);
+    vjp_euler_R(R, sn, cs, GR, gx + 3);
+  }
+}
+
+template <int MODEL, int OPT>
+__device__ __forceinline__ void vjp_deriv(const DevParams &P, const Plant<MODEL, OPT> &pl, const float *x, const float *u,
+                                          const float *a, float *gx, float *gu) {
+  if constexpr (OPT != 0) {
+    if constexpr (MODEL == MODEL_FP) vjp_deriv_fp_ex(P, pl, x, u, a, gx, gu);
+    else vjp_deriv_ab_ex(P, pl, x, u, a, gx, gu);
+  } else {
+    if constexpr (MODEL == MODEL_FP) vjp_deriv_fp(P, pl, x, a, gx, gu);
+    else vjp_deriv_ab(P, pl, x, a, gx, gu);
+  }
+}
+
+// C6 motor mixer: (F_c, tau) -> rotor command.  Cotangent g_rpm[4] -> g_Fc (accumulated), g_tau[3] (assigned).  The
+// forward pass is recomputed to know which clips are active (R33: derivative 0 there).  With a thrust polynomial
+// (OPT_EXTRAS) r = (sqrt(kf1^2 - 4 kf2 (kf0 - f)) - kf1) / (2 kf2), so dr/df = 1 / sqrt(disc).
+template <int OPT>
+__device__ __forceinline__ void vjp_mixer(const DevParams &P, float Fc, const float *tau, const float *g_rpm, float *g_Fc,
+                                          float *g_tau) {
+  float a = 0.25f * Fc, bx = tau[0] * P.inv_4lever, by = tau[1] * P.inv_4lever, bz = tau[2] * P.inv_4kappa;
+  float f[4] = { a - bx - by - bz, a - bx + by + bz, a + bx + by - bz, a + bx - by + bz };
+  float gf[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    float fk = clipf(f[k], 0.0f, P.f_rotor_max);
+    float r, drdf;
+    bool ok = true;
+    if ((OPT & OPT_EXTRAS) && P.thrust_poly) {
+      float disc = P.kf[1] * P.kf[1] - 4.0f * P.kf[2] * (P.kf[0] - fk);
+      ok = disc > 0.0f;
+      float sd = sqrtf(fmaxf(disc, 0.0f));
+      r = (sd - P.kf[1]) * (0.5f * P.inv_kf2);
+      drdf = 1.0f / sd;
+    } else {
+      r = sqrtf(fk * P.inv_kf2);
+      drdf = 0.5f * P.inv_kf2 / r;                                                          // d sqrt(f/kf)/df = 1/(2 kf r)
+    }
+    bool live = ok && f[k] > 0.0f && f[k] < P.f_rotor_max && r > P.rpm_min && r < P.rpm_max;   // R33: 0 where a clip is active
+    gf[k] = live ? g_rpm[k] * drdf : 0.0f;
+  }
+  float g_a = (gf[0] + gf[1]) + (gf[2] + gf[3]);
+  float g_bx = (gf[2] + gf[3]) - (gf[0] + gf[1]);
+  float g_by = (gf[1] + gf[2]) - (gf[0] + gf[3]);
+  float g_bz = (gf[1] + gf[3]) - (gf[0] + gf[2]);
+  *g_Fc += 0.25f * g_a;
+  g_tau[0] = g_bx * P.inv_4lever; g_tau[1] = g_by * P.inv_4lever; g_tau[2] = g_bz * P.inv_4kappa;
 }
 
 // ---- VJP of the attitude controller tick + mixer (C5, C6) -----------------------------------------------------------
 // inputs of the tick: q, w (state), cmd = (roll, pitch, yaw, F), iR (integral before the tick).
 // cotangents in: g_rpm[4] (of the rotor command), g_iRn[3] (of the integral after the tick).
 // out: accumulates into g_q[4], g_w[3], g_cmd[4]; g_iR[3] = cotangent of the integral before the tick.
+template <int OPT>
 __device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const float *q, const float *w, const float *cmd,
                                                   const float *iR, const float *g_rpm, const float *g_iRn,
                                                   float *g_q, float *g_w, float *g_cmd, float *g_iR) {
@@ -122,10 +327,7 @@ __device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const floa
   quat_to_R(q, R);
   float sn[3], cs[3];                                             // one evaluation serves Rd and its angle derivatives;
   sincos3_step(cmd, sn, cs);                                      // MUFU (abs err 5e-7): a linearisation point, not the forward value
-  const float sr = sn[0], cr = cs[0], sp = sn[1], cp = cs[1], sy = sn[2], cy = cs[2];
-  Rd[0][0] = cy * cp; Rd[0][1] = cy * sp * sr - sy * cr; Rd[0][2] = cy * sp * cr + sy * sr;      // reading R13, as euler_to_R
-  Rd[1][0] = sy * cp; Rd[1][1] = sy * sp * sr + cy * cr; Rd[1][2] = sy * sp * cr - cy * sr;
-  Rd[2][0] = -sp;     Rd[2][1] = cp * sr;                Rd[2][2] = cp * cr;
+  euler_R_from_sc(sn, cs, Rd);
   auto Mij = [&](int i, int j) { return Rd[0][i] * R[0][j] + Rd[1][i] * R[1][j] + Rd[2][i] * R[2][j]; };
   float eR[3] = { 0.5f * (Mij(2, 1) - Mij(1, 2)), 0.5f * (Mij(0, 2) - Mij(2, 0)), 0.5f * (Mij(1, 0) - Mij(0, 1)) };
   float pre[3], iRn[3], tau[3];
@@ -135,23 +337,8 @@ __device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const floa
     iRn[j] = clipf(pre[j], -P.iR_max, P.iR_max);
     tau[j] = P.Jnom[j] * (-P.kR[j] * eR[j] - P.kW[j] * w[j] - P.kI[j] * iRn[j]);
   }
-  // mixer forward (to know which clips are active), then its reverse
-  float a = 0.25f * cmd[3], bx = tau[0] * P.inv_4lever, by = tau[1] * P.inv_4lever, bz = tau[2] * P.inv_4kappa;
-  float f[4] = { a - bx - by - bz, a - bx + by + bz, a + bx + by - bz, a + bx - by + bz };
-  float gf[4];
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    float fk = clipf(f[k], 0.0f, P.f_rotor_max);
-    float r = sqrtf(fk * P.inv_kf2);
-    bool live = f[k] > 0.0f && f[k] < P.f_rotor_max && r > P.rpm_min && r < P.rpm_max;     // R33: 0 where a clip is active
-    gf[k] = live ? g_rpm[k] * (0.5f * P.inv_kf2 / r) : 0.0f;                               // d sqrt(f/kf)/df = 1/(2 kf r)
-  }
-  float g_a = (gf[0] + gf[1]) + (gf[2] + gf[3]);
-  float g_bx = (gf[2] + gf[3]) - (gf[0] + gf[1]);
-  float g_by = (gf[1] + gf[2]) - (gf[0] + gf[3]);
-  float g_bz = (gf[1] + gf[3]) - (gf[0] + gf[2]);
-  g_cmd[3] += 0.25f * g_a;
-  float g_tau[3] = { g_bx * P.inv_4lever, g_by * P.inv_4lever, g_bz * P.inv_4kappa };
+  float g_tau[3];
+  vjp_mixer<OPT>(P, cmd[3], tau, g_rpm, &g_cmd[3], g_tau);
   float g_eR[3];
 #pragma unroll
   for (int j = 0; j < 3; ++j) {
@@ -175,73 +362,61 @@ __device__ __forceinline__ void vjp_attitude_tick(const DevParams &P, const floa
       GR[k][j] = Rd[k][0] * G[0][j] + Rd[k][1] * G[1][j] + Rd[k][2] * G[2][j];     // dL/dR_kj
       GD[k][j] = R[k][0] * G[j][0] + R[k][1] * G[j][1] + R[k][2] * G[j][2];        // dL/dRd_kj
     }
-  const float x = q[0], y = q[1], z = q[2], ww = q[3];
-  g_q[0] += 2.0f * (y * (GR[0][1] + GR[1][0]) + z * (GR[0][2] + GR[2][0]) + ww * (GR[2][1] - GR[1][2])) - 4.0f * x * (GR[1][1] + GR[2][2]);
-  g_q[1] += 2.0f * (x * (GR[0][1] + GR[1][0]) + z * (GR[1][2] + GR[2][1]) + ww * (GR[0][2] - GR[2][0])) - 4.0f * y * (GR[0][0] + GR[2][2]);
-  g_q[2] += 2.0f * (x * (GR[0][2] + GR[2][0]) + y * (GR[1][2] + GR[2][1]) + ww * (GR[1][0] - GR[0][1])) - 4.0f * z * (GR[0][0] + GR[1][1]);
-  g_q[3] += 2.0f * (x * (GR[2][1] - GR[1][2]) + y * (GR[0][2] - GR[2][0]) + z * (GR[1][0] - GR[0][1]));
-  // Rd = Rz(yaw) Ry(pitch) Rx(roll): d/droll rotates columns 1, 2; d/dyaw rotates rows 0, 1; d/dpitch written out
-  g_cmd[0] += GD[0][1] * Rd[0][2] - GD[0][2] * Rd[0][1] + GD[1][1] * Rd[1][2] - GD[1][2] * Rd[1][1] + GD[2][1] * Rd[2][2] - GD[2][2] * Rd[2][1];
-  g_cmd[1] += GD[0][0] * (-cy * sp) + GD[0][1] * (cy * cp * sr) + GD[0][2] * (cy * cp * cr)
-            + GD[1][0] * (-sy * sp) + GD[1][1] * (sy * cp * sr) + GD[1][2] * (sy * cp * cr)
-            + GD[2][0] * (-cp) + GD[2][1] * (-sp * sr) + GD[2][2] * (-sp * cr);
-  g_cmd[2] += -GD[0][0] * Rd[1][0] - GD[0][1] * Rd[1][1] - GD[0][2] * Rd[1][2]
-            + GD[1][0] * Rd[0][0] + GD[1][1] * Rd[0][1] + GD[1][2] * Rd[0][2];
+  vjp_quat_to_R(q, GR, g_q);
+  vjp_euler_R(Rd, sn, cs, GD, g_cmd);
 }
 
-// ---- one step forward (C4) from x with the inputs held; returns the un-normalised quaternion norm for the FP model ----
-template <int MODEL, int INTEG>
-__device__ __forceinline__ void step_forward(const DevParams &P, const Plant<MODEL, 0> &pl, float *x, const float *u) {
+// ---- one step forward (C4) from x with the inputs held: the rollout kernel's own integrator (lean first-principles
+// step / generic Euler and RK4; quaternion renormalised; simplified abstracted model: f_Sigma <- f_cmd) ----------------
+template <int MODEL, int INTEG, int OPT>
+__device__ __forceinline__ void step_forward(const DevParams &P, const Plant<MODEL, OPT> &pl, float *x, const float *u,
+                                             const float *fd) {
   constexpr int D = Dim<MODEL>::D;
-  const float fd[3] = { 0.f, 0.f, 0.f };
-  if constexpr (MODEL == MODEL_FP) {          // the rollout kernel's own lean step (closed-form rotor lag, factored rates)
-    integrate<MODEL_FP, INTEG, 0>(P, pl, x, u, fd);
+  if constexpr (MODEL == MODEL_FP || OPT != 0) {
+    integrate<MODEL, INTEG, OPT>(P, pl, x, u, fd);
     return;
   }
   float k[D];
   if constexpr (INTEG == INTEG_EULER) {
-    deriv<MODEL, 0>(P, pl, x, u, fd, k);
+    deriv<MODEL, OPT>(P, pl, x, u, fd, k);
 #pragma unroll
     for (int j = 0; j < D; ++j) x[j] = fmaf(P.h, k[j], x[j]);
   } else {
     float xs[D], acc[D];
-    deriv<MODEL, 0>(P, pl, x, u, fd, k);
+    deriv<MODEL, OPT>(P, pl, x, u, fd, k);
 #pragma unroll
     for (int j = 0; j < D; ++j) { acc[j] = k[j]; xs[j] = fmaf(P.half_h, k[j], x[j]); }
-    deriv<MODEL, 0>(P, pl, xs, u, fd, k);
+    deriv<MODEL, OPT>(P, pl, xs, u, fd, k);
 #pragma unroll
     for (int j = 0; j < D; ++j) { acc[j] = fmaf(2.0f, k[j], acc[j]); xs[j] = fmaf(P.half_h, k[j], x[j]); }
-    deriv<MODEL, 0>(P, pl, xs, u, fd, k);
+    deriv<MODEL, OPT>(P, pl, xs, u, fd, k);
 #pragma unroll
     for (int j = 0; j < D; ++j) { acc[j] = fmaf(2.0f, k[j], acc[j]); xs[j] = fmaf(P.h, k[j], x[j]); }
-    deriv<MODEL, 0>(P, pl, xs, u, fd, k);
+    deriv<MODEL, OPT>(P, pl, xs, u, fd, k);
 #pragma unroll
     for (int j = 0; j < D; ++j) x[j] = fmaf(P.h_sixth, acc[j] + k[j], x[j]);
-  }
-  if constexpr (MODEL == MODEL_FP) {
-    float *q = x + 3;
-    float inv = rsqrtf(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
-#pragma unroll
-    for (int j = 0; j < 4; ++j) q[j] *= inv;
   }
 }
 
 // ---- pull the cotangent lam (of the post-step state) back through one step that started at x with held inputs u -----
-// on return lam = cotangent of x, gu accumulates the cotangent of u
-template <int MODEL, int INTEG>
-__device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MODEL, 0> &pl, const float *x,
-                                              const float *u, float *lam, float *gu) {
+// on return lam = cotangent of x, gu accumulates the cotangent of u.  fd: the step's disturbance force (held over the
+// stages; it shifts the stage velocities, which the drag term reads)
+template <int MODEL, int INTEG, int OPT>
+__device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MODEL, OPT> &pl, const float *x,
+                                              const float *u, const float *fd, float *lam, float *gu) {
   constexpr int D = Dim<MODEL>::D;
-  const float fd[3] = { 0.f, 0.f, 0.f };
+  if constexpr (MODEL == MODEL_AB && OPT != 0) {
+    if (!P.ab_thrust_dyn) { gu[3] += lam[12]; lam[12] = 0.0f; }                // simplified model: f_Sigma+ = f_cmd
+  }
   float k1[D], x2[D], x3[D], x4[D], kk[D];
-  deriv<MODEL, 0>(P, pl, x, u, fd, k1);
+  deriv<MODEL, OPT>(P, pl, x, u, fd, k1);
   if constexpr (INTEG == INTEG_RK4) {
 #pragma unroll
     for (int j = 0; j < D; ++j) x2[j] = fmaf(P.half_h, k1[j], x[j]);
-    deriv<MODEL, 0>(P, pl, x2, u, fd, kk);
+    deriv<MODEL, OPT>(P, pl, x2, u, fd, kk);
 #pragma unroll
     for (int j = 0; j < D; ++j) { k1[j] = fmaf(2.0f, kk[j], k1[j]); x3[j] = fmaf(P.half_h, kk[j], x[j]); }
-    deriv<MODEL, 0>(P, pl, x3, u, fd, kk);
+    deriv<MODEL, OPT>(P, pl, x3, u, fd, kk);
 #pragma unroll
     for (int j = 0; j < D; ++j) { k1[j] = fmaf(2.0f, kk[j], k1[j]); x4[j] = fmaf(P.h, kk[j], x[j]); }
   }
@@ -249,7 +424,7 @@ __device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MO
     // q+ = qt / |qt| with qt the integrator's un-normalised quaternion: g_qt = (g - q+ (q+ . g)) / |qt|
     float qt[4];
     if constexpr (INTEG == INTEG_RK4) {
-      deriv<MODEL, 0>(P, pl, x4, u, fd, kk);
+      deriv<MODEL, OPT>(P, pl, x4, u, fd, kk);
 #pragma unroll
       for (int j = 0; j < 4; ++j) qt[j] = fmaf(P.h_sixth, k1[3 + j] + kk[3 + j], x[3 + j]);
     } else {
@@ -267,7 +442,7 @@ __device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MO
   if constexpr (INTEG == INTEG_EULER) {
 #pragma unroll
     for (int j = 0; j < D; ++j) { a[j] = P.h * lam[j]; gx[j] = 0.f; }
-    vjp_deriv<MODEL>(P, pl, x, a, gx, gu);
+    vjp_deriv<MODEL, OPT>(P, pl, x, u, a, gx, gu);
 #pragma unroll
     for (int j = 0; j < D; ++j) lam[j] += gx[j];
   } else {
@@ -275,16 +450,16 @@ __device__ __forceinline__ void step_backward(const DevParams &P, const Plant<MO
     float tot[D];
 #pragma unroll
     for (int j = 0; j < D; ++j) { a[j] = P.h_sixth * lam[j]; gx[j] = 0.f; tot[j] = 0.f; }
-    vjp_deriv<MODEL>(P, pl, x4, a, gx, gu);                                   // k4
+    vjp_deriv<MODEL, OPT>(P, pl, x4, u, a, gx, gu);                           // k4
 #pragma unroll
     for (int j = 0; j < D; ++j) { tot[j] += gx[j]; a[j] = fmaf(P.h, gx[j], 2.0f * P.h_sixth * lam[j]); gx[j] = 0.f; }
-    vjp_deriv<MODEL>(P, pl, x3, a, gx, gu);                                   // k3
+    vjp_deriv<MODEL, OPT>(P, pl, x3, u, a, gx, gu);                           // k3
 #pragma unroll
     for (int j = 0; j < D; ++j) { tot[j] += gx[j]; a[j] = fmaf(P.half_h, gx[j], 2.0f * P.h_sixth * lam[j]); gx[j] = 0.f; }
-    vjp_deriv<MODEL>(P, pl, x2, a, gx, gu);                                   // k2
+    vjp_deriv<MODEL, OPT>(P, pl, x2, u, a, gx, gu);                           // k2
 #pragma unroll
     for (int j = 0; j < D; ++j) { tot[j] += gx[j]; a[j] = fmaf(P.half_h, gx[j], P.h_sixth * lam[j]); gx[j] = 0.f; }
-    vjp_deriv<MODEL>(P, pl, x, a, gx, gu);                                    // k1
+    vjp_deriv<MODEL, OPT>(P, pl, x, u, a, gx, gu);                            // k1
 #pragma unroll
     for (int j = 0; j < D; ++j) lam[j] += tot[j] + gx[j];
   }
@@ -575,8 +750,8 @@ __device__ __forceinline__ void vjp_zB_ab(const float *sn, const float *cs, cons
 #ifndef GRAD_MIN_BLOCKS
 #define GRAD_MIN_BLOCKS 4
 #endif
-template <int MODEL, int IFACE> struct Hist {
-  static constexpr bool POS = IFACE == IF_POSITION;
+template <int MODEL, int IFACE, int OPT = 0> struct Hist {
+  static constexpr bool POS = IFACE == IF_POSITION || OPT != 0;     // general kernels park the full record
   static constexpr int HD = MODEL == MODEL_FP ? (POS ? 32 : (IFACE == IF_ATTITUDE ? 18 : 16)) : (POS ? 20 : 8);
   static constexpr int H4 = HD / 4, H2 = (HD % 4) / 2;
 };
@@ -586,10 +761,14 @@ template <int MODEL, int IFACE> struct Hist {
 // blocks of different waves are in different sweeps -- and "no instruction" was the largest stall; split, each launch's
 // loop fits the instruction cache on its own: 0.793 -> 0.761 ms for 2^20 worlds x 10 RK4 steps (same GPU).  Launch bounds
 // 3 / 5 / 6 / 8 blocks for either phase measured no better than 4.
-template <int MODEL, int INTEG, int IFACE, int PHASE>
-__global__ void __launch_bounds__(128, GRAD_MIN_BLOCKS)
+// General kernels (OPT = GOPT: fidelity extras gated at run time by the DevParams flags, disturbances, torque interface):
+// the generic integrator and 17 / 13-wide pull-back, full record per step, 2 blocks per SM (<= 255 registers).
+template <int MODEL, int INTEG, int IFACE, int PHASE, int OPT = 0>
+__global__ void __launch_bounds__(128, OPT != 0 ? 2 : GRAD_MIN_BLOCKS)
 grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParams P, int randp) {
-  using H = Hist<MODEL, IFACE>;
+  using H = Hist<MODEL, IFACE, OPT>;
+  constexpr bool GEN = OPT != 0;
+  constexpr bool FULL = H::POS;
   constexpr int D = Dim<MODEL>::D, HD = H::HD, H4 = H::H4, HP = H4 * 4 + 4;
   constexpr bool FP = MODEL == MODEL_FP;
   constexpr bool POS = IFACE == IF_POSITION;
@@ -598,8 +777,24 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   const long long MN = A.MN;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= MN) return;
-  Plant<MODEL, 0> pl;
-  pl.load(P, A.wparam, A.M, i / A.N, randp != 0);
+  Plant<MODEL, OPT> pl;
+  const long long w_loc = i / A.N;
+  pl.load(P, A.wparam, A.M, w_loc, randp != 0);
+  // C8 step 4: the disturbance of step s is sigma (z0, z1, z2) from Philox(seed; global world, drone, s, DIST)
+  const uint32_t wg = (uint32_t)(w_loc + A.world_offset), nn = (uint32_t)(i - w_loc * A.N);
+  auto disturbance = [&](uint32_t step, float *fd) {
+    fd[0] = fd[1] = fd[2] = 0.0f;
+    if constexpr (GEN) {
+      if (P.dist_sigma > 0.0f) {
+        uint32_t r[4]; float z[4];
+        philox4x32_10_rk(A.rk, wg, nn, step, STREAM_DIST, r);
+        normal_pair(r[0], r[1], z[0], z[1]);
+        normal_pair(r[2], r[3], z[2], z[3]);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) fd[j] = P.dist_sigma * z[j];
+      }
+    }
+  };
 
   float x[D], iR[3] = { 0, 0, 0 }, ip[3] = { 0, 0, 0 }, rpm_cmd[4] = { 0, 0, 0, 0 }, cmd[4] = { 0, 0, 0, 0 };
   float att_cmd[4] = { 0, 0, 0, 0 };      // position interface: the attitude command the outer loop holds
@@ -611,7 +806,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
 #pragma unroll
     for (int j = 0; j < 4; ++j) rpm_cmd[j] = A.ctrl[(10 + j) * MN + i];
   }
-  if (POS) {
+  if (FULL) {
 #pragma unroll
     for (int j = 0; j < 3; ++j) ip[j] = A.ctrl[(3 + j) * MN + i];
 #pragma unroll
@@ -623,7 +818,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   auto pack = [&](float *rec) {
 #pragma unroll
     for (int j = 0; j < HP; ++j) rec[j] = 0.f;
-    if constexpr (POS) {
+    if constexpr (FULL) {
 #pragma unroll
       for (int j = 0; j < D; ++j) rec[j] = x[j];
       int o = D;
@@ -660,6 +855,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
 #pragma unroll
         for (int j = 0; j < 4; ++j) rpm_cmd[j] = clipf(cmd[j], P.rpm_min, P.rpm_max);
       }
+      if (FP && IFACE == IF_TORQUE) mixer<OPT>(P, cmd[3], cmd, rpm_cmd);      // (tau_x, tau_y, tau_z, F) straight into the mixer
     }
     if (++hold_phase == A.cmd_hold) { hold_phase = 0; ++k_cmd; }
     if (POS) {
@@ -675,11 +871,11 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
       if (att_phase == 0) {
         float Rd[3][3];
         euler_to_R(acmd[0], acmd[1], acmd[2], Rd);
-        attitude_tick<0>(P, x + 3, x + 10, Rd, acmd[3], iR, rpm_cmd);
+        attitude_tick<OPT>(P, x + 3, x + 10, Rd, acmd[3], iR, rpm_cmd);
       }
       att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
     }
-    if constexpr (POS) {
+    if constexpr (FULL) {
       constexpr int o = FP ? D + 6 : D + 3;
       if (FP) {
 #pragma unroll
@@ -695,7 +891,9 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     for (int j = 0; j < H4; ++j)
       __stcs(h4 + ((size_t)t * H4 + j) * MN + i, make_float4(rec[4 * j], rec[4 * j + 1], rec[4 * j + 2], rec[4 * j + 3]));
     if constexpr (H::H2) __stcs(h2 + (size_t)t * MN + i, make_float2(rec[4 * H4], rec[4 * H4 + 1]));
-    step_forward<MODEL, INTEG>(P, pl, x, FP ? rpm_cmd : acmd);
+    float fd[3];
+    disturbance(A.s0 + (uint32_t)t, fd);
+    step_forward<MODEL, INTEG, OPT>(P, pl, x, FP ? rpm_cmd : acmd, fd);
   }
   // ---- loss and its cotangent ----------------------------------------------------------------------------------
   float lam[D];
@@ -736,7 +934,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
       rec[4 * j] = v.x; rec[4 * j + 1] = v.y; rec[4 * j + 2] = v.z; rec[4 * j + 3] = v.w;
     }
     if constexpr (H::H2) { const float2 v = __ldcs(h2 + (size_t)t * MN + i); rec[4 * H4] = v.x; rec[4 * H4 + 1] = v.y; }
-    if constexpr (POS) {
+    if constexpr (FULL) {
 #pragma unroll
       for (int j = 0; j < D; ++j) x[j] = rec[j];
       int o = D;
@@ -775,12 +973,17 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     // (tried and rejected, measured: the four RK4 stages of this pull-back rolled into run-time loops with the stage
     //  states in shared memory -- "no instruction" stalls 1.03 -> 0.13 per issue, issue-active 68 -> 79 %, but 27 % more
     //  instructions because the straight-line form lets the compiler drop dead parts of every stage: 0.80 -> 0.87 ms)
-    if constexpr (FP) step_backward_fp_lean<INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
-    else step_backward<MODEL, INTEG>(P, pl, x, acmd, lam, g_acmd);
+    if constexpr (FP && !GEN) {
+      step_backward_fp_lean<INTEG>(P, pl, x, rpm_cmd, lam, g_rpm);
+    } else {
+      float fd[3];
+      disturbance(A.s0 + (uint32_t)t, fd);
+      step_backward<MODEL, INTEG, OPT>(P, pl, x, FP ? rpm_cmd : acmd, fd, lam, FP ? g_rpm : g_acmd);
+    }
     if (HAS_ATT) {
       if (att_phase == 0) {
         float g_prev[3];
-        vjp_attitude_tick(P, x + 3, x + 10, acmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_acmd, g_prev);
+        vjp_attitude_tick<OPT>(P, x + 3, x + 10, acmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_acmd, g_prev);
 #pragma unroll
         for (int j = 0; j < 3; ++j) g_iR[j] = g_prev[j];
 #pragma unroll
@@ -806,6 +1009,14 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
 #pragma unroll
         for (int j = 0; j < 4; ++j) { g_cmd[j] = (cmd[j] > P.rpm_min && cmd[j] < P.rpm_max) ? g_rpm[j] : 0.f; g_rpm[j] = 0.f; }
       }
+      if (FP && IFACE == IF_TORQUE) {                                          // the fetch ran the mixer on the command
+        float g_tau[3];
+        vjp_mixer<OPT>(P, cmd[3], cmd, g_rpm, &g_cmd[3], g_tau);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) g_cmd[j] += g_tau[j];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) g_rpm[j] = 0.f;
+      }
       A.grad[(size_t)k_cmd * MN + i] = make_float4(g_cmd[0], g_cmd[1], g_cmd[2], g_cmd[3]);
 #pragma unroll
       for (int j = 0; j < 4; ++j) g_cmd[j] = 0.f;
@@ -826,19 +1037,33 @@ const Entry kTable[] = {
   CF_G(MODEL_FP, INTEG_EULER, IF_POSITION), CF_G(MODEL_FP, INTEG_RK4, IF_POSITION),
   CF_G(MODEL_AB, INTEG_EULER, IF_POSITION), CF_G(MODEL_AB, INTEG_RK4, IF_POSITION),
 };
+// the general kernels: fidelity extras, force disturbances (L280), torque interface (L330)
+#define CF_GG(M_, I_, F_) { M_, I_, F_, grad_kernel<M_, I_, F_, 1, GOPT>, grad_kernel<M_, I_, F_, 2, GOPT> }
+const Entry kTableGen[] = {
+  CF_GG(MODEL_FP, INTEG_EULER, IF_ROTOR),    CF_GG(MODEL_FP, INTEG_RK4, IF_ROTOR),
+  CF_GG(MODEL_FP, INTEG_EULER, IF_TORQUE),   CF_GG(MODEL_FP, INTEG_RK4, IF_TORQUE),
+  CF_GG(MODEL_FP, INTEG_EULER, IF_ATTITUDE), CF_GG(MODEL_FP, INTEG_RK4, IF_ATTITUDE),
+  CF_GG(MODEL_FP, INTEG_EULER, IF_POSITION), CF_GG(MODEL_FP, INTEG_RK4, IF_POSITION),
+  CF_GG(MODEL_AB, INTEG_EULER, IF_ATTITUDE), CF_GG(MODEL_AB, INTEG_RK4, IF_ATTITUDE),
+  CF_GG(MODEL_AB, INTEG_EULER, IF_POSITION), CF_GG(MODEL_AB, INTEG_RK4, IF_POSITION),
+};
+bool wants_general(const cf_sim *sim) {
+  return (sim->opt & (OPT_DIST | OPT_EXTRAS)) != 0 || sim->p.iface == CF_IF_TORQUE;
+}
 
 int check(const cf_sim *sim, int n_cmds, int cmd_hold, int n_steps) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
   if (n_steps < 1 || cmd_hold < 1 || n_cmds < 1) return fail(CF_E_ARG, "n_steps, cmd_hold, n_cmds >= 1");
   if ((long long)n_cmds * cmd_hold < n_steps) return fail(CF_E_SHAPE, "n_cmds * cmd_hold < n_steps");
-  if (sim->p.cmd_source != CF_CMD_BUFFER || (sim->opt & (OPT_DIST | OPT_NOISE | OPT_EXTRAS)) != 0)
-    return fail(CF_E_UNSUPPORTED, "cf_grad differentiates the command-buffer rollout without disturbances / fidelity extras");
+  if (sim->p.cmd_source != CF_CMD_BUFFER || (sim->opt & OPT_NOISE) != 0)
+    return fail(CF_E_UNSUPPORTED, "cf_grad differentiates the command-buffer rollout (the commands are its variables)");
   return CF_OK;
 }
 
 }  // namespace
 
-static int hist_floats(int model, int iface) {
+static int hist_floats(int model, int iface, bool general) {
+  if (general) return model == CF_MODEL_FIRST_PRINCIPLES ? Hist<MODEL_FP, IF_ATTITUDE, GOPT>::HD : Hist<MODEL_AB, IF_ATTITUDE, GOPT>::HD;
   if (model == CF_MODEL_FIRST_PRINCIPLES)
     return iface == CF_IF_POSITION ? Hist<MODEL_FP, IF_POSITION>::HD : iface == CF_IF_ATTITUDE ? Hist<MODEL_FP, IF_ATTITUDE>::HD
                                                                                                : Hist<MODEL_FP, IF_ROTOR>::HD;
@@ -847,7 +1072,7 @@ static int hist_floats(int model, int iface) {
 
 extern "C" size_t cf_grad_scratch_bytes(const cf_sim *sim, int n_steps) {
   if (!sim || n_steps < 1) return 0;
-  return sizeof(float) * ((size_t)hist_floats(sim->model, sim->p.iface) * (size_t)sim->MN * (size_t)n_steps + 4 + 4 * (size_t)sim->MN);
+  return sizeof(float) * ((size_t)hist_floats(sim->model, sim->p.iface, wants_general(sim)) * (size_t)sim->MN * (size_t)n_steps + 4 + 4 * (size_t)sim->MN);
 }
 
 extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, const float goal[3],
@@ -860,9 +1085,14 @@ extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
     return fail(CF_E_BUFFER, "cmds, grad and scratch must be 16-byte aligned");
   if (scratch_bytes < cf_grad_scratch_bytes(sim, n_steps)) return fail(CF_E_BUFFER, "scratch too small");
   const Entry *e = nullptr;
-  for (const Entry &c : kTable)
-    if (c.model == sim->model && c.integ == sim->p.integrator && c.iface == sim->p.iface) e = &c;
-  if (!e) return fail(CF_E_UNSUPPORTED, "cf_grad: interface not differentiated (the torque interface; the abstracted model has no rotor interface)");
+  if (wants_general(sim)) {
+    for (const Entry &c : kTableGen)
+      if (c.model == sim->model && c.integ == sim->p.integrator && c.iface == sim->p.iface) e = &c;
+  } else {
+    for (const Entry &c : kTable)
+      if (c.model == sim->model && c.integ == sim->p.integrator && c.iface == sim->p.iface) e = &c;
+  }
+  if (!e) return fail(CF_E_UNSUPPORTED, "cf_grad: the abstracted model has no rotor / torque interface");
   rc = cf_materialise(sim);      // a pending broadcast cf_set_state must be in the planes: the kernel reads them
   if (rc != CF_OK) return rc;
   GradArgs A;
@@ -871,6 +1101,9 @@ extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   A.MN = sim->MN; A.M = sim->M; A.N = sim->N; A.n_steps = n_steps; A.cmd_hold = cmd_hold; A.n_cmds = n_cmds;
   A.s0 = (uint32_t)sim->s_host;
   for (int j = 0; j < 3; ++j) A.goal[j] = goal[j];
+  A.world_offset = sim->p.world_offset;
+  const uint32_t lo = (uint32_t)sim->seed, hi = (uint32_t)(sim->seed >> 32);
+  for (int r = 0; r < 10; ++r) { A.rk[2 * r] = lo + (uint32_t)r * 0x9E3779B9u; A.rk[2 * r + 1] = hi + (uint32_t)r * 0xBB67AE85u; }
   const int block = 128;
   const unsigned grid = (unsigned)((sim->MN + block - 1) / block);
   e->fwd<<<grid, block, 0, sim->stream>>>(A, sim->dp, (sim->opt & OPT_RANDP) ? 1 : 0);
