@@ -168,6 +168,7 @@ class Runner:
             self.launches_per_step = 2
         # host side buffers for the end-to-end path (pinned)
         self.e2e_ok = e2e and self.cmds_host is not None
+        self.sequential_e2e = False
         if self.e2e_ok:
             self.cmds_pin = self.cmds_host.pin_memory()
             self.rec_pin = torch.empty((n_rec, wl.D, wl.MN), dtype=torch.float32, pin_memory=True) if n_rec else None
@@ -254,6 +255,12 @@ class Runner:
             return
         if self.planner:      # measured state in (52 B), plan + controller scores out; the nominal stays on the device
             sim.mppi_iterate_host(self.mpar, self.bstate_pin, self.cmds, self.plan_pin, self.info_pin)
+            return
+        if self.rec_pin is None and not self.sequential_e2e and wl.N == 1:
+            # fused rollout: ONE C-ABI call, start state + commands in, final state + minimum distance out, the result
+            # copies overlapped with the kernel slice by slice (cf_rollout_host)
+            sim.rollout_host(self.cmds_pin, wl.n_steps, self.state_pin, cmd_hold=wl.cmd_hold, x0_host=self.bstate_pin,
+                             min_dist_host=self.md_pin, n_slices=8)
             return
         if self.bstate_pin is not None:
             self.bstate.copy_(self.bstate_pin, non_blocking=True)
@@ -575,12 +582,20 @@ def main():
                    gpu_launches=R.launches_per_step * steps, M=wl.M, N=wl.N, sub_steps=wl.n_steps,
                    record_every=wl.record_every, drone_steps_per_step=wl.drone_steps)
         if want_e2e and R.e2e_ok:
-            ems = time_host_steps(R.step_e2e, torch, max(2, min(steps, 5)), 1)
+            ems = time_host_steps(R.step_e2e, torch, max(3, min(steps, 10)), 2)
             et = torch.tensor([sum(ems) / len(ems)], dtype=torch.float64, device=device)
             if world > 1:
                 dist.all_reduce(et, op=dist.ReduceOp.MAX)
             out["e2e"] = dict(value=world * wl.drone_steps / (float(et.item()) * 1e-3), unit=UNIT,
                               h2d_bytes_per_step=R.h2d, d2h_bytes_per_step=R.d2h, ms_per_step=float(et.item()))
+            if not (R.grad or R.depth or R.planner) and R.rec_pin is None and wl.N == 1:
+                R.sequential_e2e = True          # the same through cf_step_host + cf_get_state_host + cf_get_aux_host
+                sms = time_host_steps(R.step_e2e, torch, max(3, min(steps, 10)), 2)
+                R.sequential_e2e = False
+                out["e2e"]["sequential_calls"] = dict(value=wl.drone_steps / (sum(sms) / len(sms) * 1e-3),
+                                                      ms_per_step=sum(sms) / len(sms),
+                                                      note="cf_step_host, cf_get_state_host, cf_get_aux_host one after the "
+                                                           "other (no overlap); value above is cf_rollout_host")
             if world == 1 and nm in ("cfg3", "mppi", "depth"):      # double-buffered host loop (two calls in flight)
                 pms = time_host_steps_pipelined(lambda: Runner(nm, device, rank=rank, e2e=True), torch, 10, 2)
                 out["e2e"]["pipelined"] = dict(value=wl.drone_steps / (pms * 1e-3), ms_per_step=pms,

@@ -183,6 +183,20 @@ int cf_step_host(cf_sim *sim, const void *cmds_host, int n_cmds, int cmd_hold,
                  int n_steps, int record_every, float *record_host, size_t record_bytes,
                  void *staging_dev, size_t staging_bytes);
 
+/* One fused rollout from HOST buffers with the result copies overlapped -- the planning shape of BASELINE.json configs[2]
+ * (every rollout starts from the measured state, only the final state and the minimum distance come
+ * back).  Equivalent to  cf_set_state(x0, broadcast) [if x0_host != NULL];  cf_step(cmds, n_cmds, cmd_hold, n_steps,
+ * record_every = 0);  cf_get_state_host(state_host);  cf_get_aux_host(CF_AUX_MIN_DIST, min_dist_host)  -- bit-identical
+ * results and counters -- but the drones are advanced in n_slices (1..16) consecutive kernel launches over contiguous
+ * slices of the batch, and a second stream (owned by the handle, created on first use) copies slice k's rows of the state
+ * planes and minimum distances to the host while slice k + 1 computes.
+ *   x0_host [D] floats or NULL (keep the current state); cmds_host as cf_step_host; state_host [D][MN] floats;
+ *   min_dist_host [MN] floats or NULL (needs obstacles and N = 1: the per-drone read-out of the rollout epilogue, else
+ *   CF_E_UNSUPPORTED); staging_dev: cf_staging_bytes(sim, n_cmds, n_steps, 0) + 256 bytes, 256-byte aligned, caller-owned.
+ * Host buffers should be pinned (pageable memory serialises the copies).  Synchronises both streams before returning. */
+int cf_rollout_host(cf_sim *sim, const float *x0_host, const void *cmds_host, int n_cmds, int cmd_hold, int n_steps,
+                    float *state_host, float *min_dist_host, void *staging_dev, size_t staging_bytes, int n_slices);
+
 /* Copy the state planes [D][MN] to out_dev (device, on the stream) / out_host (host, synchronises). */
 int cf_get_state(cf_sim *sim, float *out_dev);
 int cf_get_state_host(cf_sim *sim, float *out_host);

@@ -101,6 +101,7 @@ def lib():
         "cf_step": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, sz]),
         "cf_staging_bytes": (sz, [vp, C.c_int, C.c_int, C.c_int]),
         "cf_step_host": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, sz, vp, sz]),
+        "cf_rollout_host": (C.c_int, [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, sz, C.c_int]),
         "cf_get_state": (C.c_int, [vp, vp]),
         "cf_get_state_host": (C.c_int, [vp, vp]),
         "cf_get_aux": (C.c_int, [vp, C.c_int, vp]),
@@ -138,7 +139,7 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
            "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host", "cf_grad_scratch_bytes",
            "cf_grad", "cf_depth", "cf_reset_masked", "cf_grad_staging_bytes", "cf_grad_host", "cf_depth_host",
-           "cf_mppi_pack_best", "cf_mppi_select"]
+           "cf_mppi_pack_best", "cf_mppi_select", "cf_rollout_host"]
 
 
 def _check(rc: int):
@@ -303,6 +304,25 @@ class Sim:
                                   int(record_every), C.c_void_p(record_host.data_ptr()) if n_rec else None,
                                   record_host.numel() * 4 if n_rec else 0, C.c_void_p(sp), need))
         return record_host[:n_rec] if n_rec else None
+
+    def rollout_host(self, cmds_host, n_steps: int, state_host, cmd_hold: int = 1, x0_host=None, min_dist_host=None,
+                     n_slices: int = 8):
+        """cf_rollout_host: broadcast start (x0_host [D] or None), fused rollout, final state [D][MN] and minimum distance
+        [MN] back in (pinned) CPU tensors, the copies overlapped with the kernel slice by slice.  Synchronous."""
+        torch = _torch()
+        per = 4 * self.MN if self.params.cmd_source == CMD_BUFFER else 4 * self.params.n_ctrl
+        assert cmds_host.dtype == torch.float32 and cmds_host.is_contiguous() and not cmds_host.is_cuda
+        n_cmds = cmds_host.numel() // per
+        need = lib().cf_staging_bytes(self._h, n_cmds, int(n_steps), 0) + 256
+        if self._staging is None or self._staging.numel() < need + 256:
+            self._staging = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+        sp = self._staging.data_ptr() + (-self._staging.data_ptr()) % 256
+        _check(lib().cf_rollout_host(self._h, C.c_void_p(x0_host.data_ptr()) if x0_host is not None else None,
+                                     C.c_void_p(cmds_host.data_ptr()), n_cmds, int(cmd_hold), int(n_steps),
+                                     C.c_void_p(state_host.data_ptr()),
+                                     C.c_void_p(min_dist_host.data_ptr()) if min_dist_host is not None else None,
+                                     C.c_void_p(sp), need, int(n_slices)))
+        return state_host, min_dist_host
 
     def get_state_host(self, out=None):
         torch = _torch()

@@ -422,6 +422,8 @@ extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf
 
 extern "C" int cf_destroy(cf_sim *sim) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  for (cudaEvent_t e : sim->slice_ev) if (e) cudaEventDestroy(e);
+  if (sim->copy_stream) cudaStreamDestroy(sim->copy_stream);
   delete sim;
   return CF_OK;
 }
@@ -619,7 +621,7 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
   if (A) sim->last_rec_mode = A->rec_mode;
   if (A) sim->last_rec_heavy = A->rec_mode == REC_TMA && A->record_every <= 4 && !(sim->opt & OPT_EXTRAS);
   L.block = sim->last_rec_heavy ? pick_block_rec(sim->MN) : pick_block(sim->MN);
-  L.grid = grid_for(sim->MN, L.block);
+  L.grid = grid_for(A ? A->i_end - A->i_begin : sim->MN, L.block);
   // the kernel stages the parameter rows whenever ITS compile-time options carry OPT_RANDP and N > 1, and the
   // dispatcher may pick a superset instantiation: size the staging area from the instantiation, not from the request
   int opt_used = 0;
@@ -649,8 +651,12 @@ extern "C" int cf_describe_launch(const cf_sim *sim, char *buf, size_t buf_len, 
   return CF_OK;
 }
 
-extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, int record_every,
-                       float *record_dev, size_t record_bytes) {
+// One cf_step call.  n_slices == 1: one launch over all drones.  n_slices > 1 (cf_rollout_host): consecutive launches over
+// slices of `slice` drones on the simulator's stream -- every slice reads the same counters, the last one advances them --
+// with after_slice(k, i0, i1) called after each launch (the caller queues that slice's result copy on another stream).
+typedef int (*SliceFn)(void *ctx, int k, long long i0, long long i1);
+static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, int record_every,
+                       float *record_dev, size_t record_bytes, long long slice, SliceFn after_slice, void *ctx) {
   if (!sim || !cmds_dev) return fail(CF_E_ARG, "NULL argument");
   if (n_steps < 1 || cmd_hold < 1 || n_cmds < 1 || record_every < 0) return fail(CF_E_ARG, "n_steps, cmd_hold, n_cmds >= 1; record_every >= 0");
   if (!sim->have_state) return fail(CF_E_STATE, "cf_step before cf_reset");
@@ -702,9 +708,16 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
     A.rk[2 * r] = A.seed_lo + (uint32_t)r * 0x9E3779B9u;
     A.rk[2 * r + 1] = A.seed_hi + (uint32_t)r * 0xBB67AE85u;
   }
-  int rc = do_launch(sim, &A, false, nullptr, nullptr, nullptr);
-  if (rc != CF_OK) return rc;
-  CF_CUDA(cudaGetLastError());
+  if (slice <= 0 || slice >= sim->MN) slice = sim->MN;
+  for (long long i0 = 0, k = 0; i0 < sim->MN; i0 += slice, ++k) {
+    A.i_begin = (int)i0;
+    A.i_end = (int)(i0 + slice < sim->MN ? i0 + slice : sim->MN);
+    A.advance = A.i_end == sim->MN;
+    int rc = do_launch(sim, &A, false, nullptr, nullptr, nullptr);
+    if (rc != CF_OK) return rc;
+    CF_CUDA(cudaGetLastError());
+    if (after_slice) { rc = after_slice(ctx, (int)k, A.i_begin, A.i_end); if (rc != CF_OK) return rc; }
+  }
   sim->s_host = s0 + n_steps;
   sim->n_rec_host += n_rec;
   sim->pending_bcast = false;
@@ -713,6 +726,11 @@ extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   sim->last_fresh = sim->rearmed; sim->last_s0 = s0; sim->last_n_steps = n_steps; sim->last_n_cmds = n_cmds;
   sim->last_cmd_hold = cmd_hold; sim->rearmed = false;
   return CF_OK;
+}
+
+extern "C" int cf_step(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_hold, int n_steps, int record_every,
+                       float *record_dev, size_t record_bytes) {
+  return step_launch(sim, cmds_dev, n_cmds, cmd_hold, n_steps, record_every, record_dev, record_bytes, 0, nullptr, nullptr);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -747,6 +765,57 @@ extern "C" int cf_step_host(cf_sim *sim, const void *cmds_host, int n_cmds, int 
   int rc = cf_step(sim, staging_dev, n_cmds, cmd_hold, n_steps, record_every, rec_dev, rb);
   if (rc != CF_OK) return rc;
   if (rb > 0) CF_CUDA(cudaMemcpyAsync(record_host, rec_dev, rb, cudaMemcpyDeviceToHost, sim->stream));
+  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  return CF_OK;
+}
+
+// One fused rollout driven from HOST buffers with the result copies overlapped (the planning shape of configs[2]):
+// the drones are advanced in n_slices consecutive launches on the simulator's stream; after each launch an event is
+// recorded and a second stream copies that slice of the final state planes (a 2-D copy: D rows of `slice` floats, pitch
+// MN floats) and of the per-drone minimum distance to the host while the next slice computes.
+struct RolloutCopy { cf_sim *sim; float *state_host, *md_host; };
+static int rollout_copy_slice(void *ctx, int k, long long i0, long long i1) {
+  RolloutCopy *c = (RolloutCopy *)ctx;
+  cf_sim *sim = c->sim;
+  cudaEvent_t ev = sim->slice_ev[k];
+  CF_CUDA(cudaEventRecord(ev, sim->stream));
+  CF_CUDA(cudaStreamWaitEvent(sim->copy_stream, ev, 0));
+  const size_t pitch = sizeof(float) * (size_t)sim->MN, width = sizeof(float) * (size_t)(i1 - i0);
+  CF_CUDA(cudaMemcpy2DAsync(c->state_host + i0, pitch, sim->state + i0, pitch, width, (size_t)sim->D, cudaMemcpyDeviceToHost,
+                            sim->copy_stream));
+  if (c->md_host)
+    CF_CUDA(cudaMemcpyAsync(c->md_host + i0, sim->md_drone + i0, width, cudaMemcpyDeviceToHost, sim->copy_stream));
+  return CF_OK;
+}
+extern "C" int cf_rollout_host(cf_sim *sim, const float *x0_host, const void *cmds_host, int n_cmds, int cmd_hold,
+                               int n_steps, float *state_host, float *min_dist_host, void *staging_dev,
+                               size_t staging_bytes, int n_slices) {
+  if (!sim || !cmds_host || !state_host || !staging_dev) return fail(CF_E_ARG, "NULL argument");
+  if (n_cmds < 1 || n_steps < 1) return fail(CF_E_ARG, "n_cmds, n_steps >= 1");
+  if (n_slices < 1 || n_slices > 16) return fail(CF_E_ARG, "n_slices in 1..16");
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_rollout_host before cf_reset");
+  if (min_dist_host && (!sim->min_d2 || sim->N != 1))
+    return fail(CF_E_UNSUPPORTED, "min_dist_host needs obstacles and one drone per world (the rollout epilogue's per-drone read-out)");
+  if (((uintptr_t)staging_dev & 255) != 0) return fail(CF_E_BUFFER, "staging must be 256-byte aligned");
+  const size_t cb = cmd_bytes(sim, n_cmds), xb = align256(sizeof(float) * sim->D);
+  if (staging_bytes < cb + xb) return fail(CF_E_BUFFER, "staging too small: %zu < %zu", staging_bytes, cb + xb);
+  if (!sim->copy_stream) CF_CUDA(cudaStreamCreateWithFlags(&sim->copy_stream, cudaStreamNonBlocking));
+  for (int k = 0; k < n_slices; ++k)
+    if (!sim->slice_ev[k]) CF_CUDA(cudaEventCreateWithFlags(&sim->slice_ev[k], cudaEventDisableTiming));
+  const size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? (size_t)sim->p.n_ctrl : (size_t)sim->MN;
+  CF_CUDA(cudaMemcpyAsync(staging_dev, cmds_host, sizeof(float) * 4 * per * (size_t)n_cmds, cudaMemcpyHostToDevice, sim->stream));
+  if (x0_host) {                         // every drone starts from this state (lazy broadcast, folded into the launches)
+    float *x0_dev = (float *)((char *)staging_dev + cb);
+    CF_CUDA(cudaMemcpyAsync(x0_dev, x0_host, sizeof(float) * sim->D, cudaMemcpyHostToDevice, sim->stream));
+    int rc = cf_set_state(sim, x0_dev, 1);
+    if (rc != CF_OK) return rc;
+  }
+  // slices of whole blocks (1024 drones is a multiple of every block size the launcher picks)
+  long long slice = ((sim->MN + n_slices - 1) / n_slices + 1023) / 1024 * 1024;
+  RolloutCopy ctx = { sim, state_host, min_dist_host };
+  int rc = step_launch(sim, staging_dev, n_cmds, cmd_hold, n_steps, 0, nullptr, 0, slice, rollout_copy_slice, &ctx);
+  if (rc != CF_OK) return rc;
+  CF_CUDA(cudaStreamSynchronize(sim->copy_stream));
   CF_CUDA(cudaStreamSynchronize(sim->stream));
   return CF_OK;
 }

@@ -92,6 +92,9 @@ struct StepArgs {
                            // record period and the shared memory the resident warps can have
   alignas(64) CUtensorMap rec_map;    // REC_TMA: the record buffer as the 2-D tensor [n_rec * D][MN], box = 32 x rec_group * D
   alignas(64) CUtensorMap rec_map1;   // the same tensor with box = 32 x D (partial last group)
+  // (appended: the offsets of everything above -- the Philox keys are read with 8 / 16-byte constant loads -- stay put)
+  int i_begin, i_end;         // (M N < 2^31) this launch advances the drones [i_begin, i_end) (a slice of the batch: cf_rollout_host; else [0, MN))
+  int advance;                // this launch advances the device-side counters (the last slice of a call)
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -689,8 +692,13 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   if (OPT & OPT_OBST) __syncthreads();
 
   const long long MN = A.MN;
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const bool active = i < MN;
+  // slices of the batch (cf_rollout_host) exist only for launches that record nothing: the recording lean kernels keep
+  // the whole-batch geometry as a compile-time fact
+  constexpr bool SLICED = REC == REC_NONE || REC == REC_RUNTIME;
+  const int blk0 = (SLICED ? A.i_begin : 0) + (int)(blockIdx.x * blockDim.x);      // first drone of this block
+  const int i_end = SLICED ? A.i_end : (int)MN;
+  const long long i = blk0 + (int)threadIdx.x;
+  const bool active = i < i_end;
   // the warp index as a value the compiler can prove warp-uniform (the TMA instruction takes uniform operands)
   const int warp_u = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   // the device-side counters, broadcast from lane 0 so that the compiler can prove them (and every phase counter, loop
@@ -704,8 +712,8 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   if (active) { w = i / A.N; n = i - w * A.N; }
   if ((OPT & OPT_RANDP) && A.N > 1) {
     // stage the parameter rows of the worlds this block touches in shared memory, then read them from there
-    long long first = (long long)blockIdx.x * blockDim.x;
-    long long last = first + blockDim.x - 1 < MN - 1 ? first + blockDim.x - 1 : MN - 1;
+    long long first = blk0;
+    long long last = first + blockDim.x - 1 < i_end - 1 ? first + blockDim.x - 1 : i_end - 1;
     long long w_first = first / A.N;
     int span = (int)(last / A.N - w_first) + 1;
     for (int idx = threadIdx.x; idx < NP * span; idx += blockDim.x) {
@@ -804,7 +812,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // of the warp, row = first slot of the group * D) of the [n_rec * D][MN] record tensor
     float *rec_tile = wp_s + warp_u * (kRecBufs * A.rec_group * D * 32);
     const uint32_t rec_tile_sa = (uint32_t)__cvta_generic_to_shared(wp_s) + (uint32_t)warp_u * (kRecBufs * A.rec_group * D * 128);
-    const int rec_col = (int)((long long)blockIdx.x * blockDim.x) + warp_u * 32;
+    const int rec_col = (int)blk0 + warp_u * 32;
     int rec_buf = 0, rec_grp = 0;
     // commands.  Buffer mode: one float4 per drone and command, prefetched one command ahead.  Noise mode: the nominal
     // sequence of this world's controller (R26), the same 16 bytes for (nearly) every lane: a plain indexed read-only
@@ -1069,7 +1077,8 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   if (threadIdx.x == 0) {
     __threadfence();
     uint32_t done = atomicAdd(&A.counters->blocks_done, 1u);
-    if (done == gridDim.x - 1) {
+    if (SLICED && done == gridDim.x - 1 && !A.advance) A.counters->blocks_done = 0;   // a slice that is not the call's last one
+    if (done == gridDim.x - 1 && (!SLICED || A.advance)) {
       const uint32_t s1 = s0 + (uint32_t)A.n_steps;
       uint32_t n_rec = A.record_every > 0 ? s1 / (uint32_t)A.record_every - s0 / (uint32_t)A.record_every : 0u;
       auto ticks = [&](uint32_t div) { return (s1 + div - 1u) / div - (s0 + div - 1u) / div; };

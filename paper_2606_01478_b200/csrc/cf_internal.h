@@ -35,6 +35,9 @@ struct cf_sim {
   long long n_rec_host;
   bool have_state;
   float hover_rpm;
+  // cf_rollout_host: a second stream for the result copies and one event per slice (created on first use)
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t slice_ev[16] = {};
 };
 
 int cf_materialise(cf_sim *sim);         // cf_api.cu: write a pending broadcast cf_set_state into the planes

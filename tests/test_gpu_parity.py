@@ -271,6 +271,32 @@ def test_edge_cases_and_status_codes(cf, W):
         assert np.isfinite(x).all() and np.allclose(np.linalg.norm(x[3:7], axis=0), 1, atol=1e-6)
 
 
+@pytest.mark.parametrize("name,M,n_slices", [("cfg3", 5000, 8), ("cfg3", 300, 4), ("cfg3b", 4097, 3), ("cfg3", 33000, 16),
+                                              ("cfg2", 2500, 2)])
+def test_rollout_host_equals_step_and_copies(cf, W, name, M, n_slices):
+    """cf_rollout_host (sliced launches, result copies on a second stream) returns bit-identical final states, minimum
+    distances and counters to cf_set_state + cf_step + cf_get_state + cf_get_aux; a second call continues correctly."""
+    import torch
+    wl = getattr(W, name)(seed=5, M=M, n_steps=30)
+    a, b = fresh_gpu(cf, wl), fresh_gpu(cf, wl)
+    cm = torch.from_numpy(np.ascontiguousarray(wl.cmds)).pin_memory()
+    x0 = None if wl.broadcast_state is None else torch.from_numpy(wl.broadcast_state.astype(np.float32)).pin_memory()
+    obst = wl.params.get("n_obstacles", 0) > 0
+    st = torch.empty((wl.D, wl.M), dtype=torch.float32).pin_memory()
+    md = torch.empty(wl.M, dtype=torch.float32).pin_memory() if obst else None
+    for rep in range(2):
+        if x0 is not None:
+            a.set_state(x0.cuda(), broadcast=True)
+        a.step(cm.cuda(), wl.n_steps, cmd_hold=wl.cmd_hold)
+        b.rollout_host(cm, wl.n_steps, st, cmd_hold=wl.cmd_hold, x0_host=x0, min_dist_host=md, n_slices=n_slices)
+        assert np.array_equal(st.numpy(), a.get_state().cpu().numpy())
+        assert np.array_equal(b.get_state().cpu().numpy(), a.get_state().cpu().numpy())
+        if obst:
+            assert np.array_equal(md.numpy(), a.min_dist().cpu().numpy())
+            assert np.array_equal(b.min_dist().cpu().numpy(), a.min_dist().cpu().numpy())
+        assert np.array_equal(a.counters(), b.counters()) and a.step_counter == b.step_counter == (rep + 1) * wl.n_steps
+
+
 def test_general_kernel_fidelity_switches(cf, cfo, W):
     """The OPT_ALL instantiations: full Eq. (6), thrust/torque polynomials, Eq. (5) gyro, body drag, all four
     interfaces, RK4 on the abstracted model, simplified AB variant -- teacher-free short runs vs the oracle."""
