@@ -149,6 +149,27 @@ def test_position_interface_gradient_through_the_full_controller_stack(cf, cfo, 
     print(f"model {model} position interface: worst relative gradient error {worst:.2e}")
 
 
+@pytest.mark.parametrize("model", [0, 1])
+def test_swarm_gradient_several_drones_per_world(cf, cfo, og, model):
+    """PAPER.md:L69 "... and supporting swarms": N > 1 drones per world share the world's randomised parameters; every
+    drone has its own command sequence and its own gradient (configs[3] shape in miniature: grid start, position targets)."""
+    M, N = 3, 43
+    lo, hi = [1.0] * 12, [1.0] * 12
+    lo[0], hi[0] = 0.93, 1.18
+    params = dict(integrator=0 if model else 1, iface=3, f_phys=500.0 if model else 1000.0, f_att=500.0, f_pos=100.0,
+                  init_mode=2, grid_dims=[4, 4, 3], grid_spacing=0.3, grid_jitter=0.02, grid_origin=[-0.5, -0.5, 0.8],
+                  rnd_lo=lo, rnd_hi=hi)
+    g, o = cf.Sim(M, N, model, params), cfo.OracleSim(M, N, model, params)
+    g.reset(9), o.reset(9)
+    cmds = pos_cmds(4, M * N, o.get_state()[:3], seed=2)
+    L_gpu, g_gpu = g.grad(cmds, 16, GOAL, cmd_hold=5)
+    L_o, g_o = og.value_and_grad(o, cmds, 16, 5, GOAL)
+    worst = compare(g_gpu.cpu().numpy(), L_gpu.cpu().numpy(), L_o, g_o)
+    wp = o.world_params()
+    assert len(np.unique(wp[0])) == M                                 # the worlds really differ
+    print(f"swarm gradient, model {model}: worst relative gradient error {worst:.2e}")
+
+
 def test_host_buffer_gradient_equals_device_gradient(cf):
     import torch
     M = 200
