@@ -297,6 +297,27 @@ def test_rollout_host_equals_step_and_copies(cf, W, name, M, n_slices):
         assert np.array_equal(a.counters(), b.counters()) and a.step_counter == b.step_counter == (rep + 1) * wl.n_steps
 
 
+def test_rollout_host_status_codes(cf, W):
+    import torch
+    wl = W.cfg2(seed=1, M=64, n_steps=10)                       # no obstacles: there is no minimum distance to return
+    sim = cf.Sim(wl.M, 1, wl.model, wl.params)
+    cm = torch.from_numpy(np.ascontiguousarray(wl.cmds)).pin_memory()
+    st = torch.empty((wl.D, wl.M), dtype=torch.float32).pin_memory()
+    md = torch.empty(wl.M, dtype=torch.float32).pin_memory()
+    with pytest.raises(cf.CfError) as e:
+        sim.rollout_host(cm, 10, st, cmd_hold=wl.cmd_hold)
+    assert e.value.code == cf.E_STATE                           # before cf_reset
+    sim.reset(1)
+    with pytest.raises(cf.CfError) as e:
+        sim.rollout_host(cm, 10, st, cmd_hold=wl.cmd_hold, min_dist_host=md)
+    assert e.value.code == cf.E_UNSUPPORTED
+    for bad in (0, 17):
+        with pytest.raises(cf.CfError) as e:
+            sim.rollout_host(cm, 10, st, cmd_hold=wl.cmd_hold, n_slices=bad)
+        assert e.value.code == cf.E_ARG
+    assert sim.step_counter == 0                                # nothing ran
+
+
 def test_general_kernel_fidelity_switches(cf, cfo, W):
     """The OPT_ALL instantiations: full Eq. (6), thrust/torque polynomials, Eq. (5) gyro, body drag, all four
     interfaces, RK4 on the abstracted model, simplified AB variant -- teacher-free short runs vs the oracle."""
