@@ -272,7 +272,7 @@ def test_edge_cases_and_status_codes(cf, W):
 
 
 @pytest.mark.parametrize("name,M,n_slices", [("cfg3", 5000, 8), ("cfg3", 300, 4), ("cfg3b", 4097, 3), ("cfg3", 33000, 16),
-                                              ("cfg2", 2500, 2)])
+                                              ("cfg2", 2500, 2), ("cfg3", 1 << 20, 8)])   # the last: bench.py's e2e call
 def test_rollout_host_equals_step_and_copies(cf, W, name, M, n_slices):
     """cf_rollout_host (sliced launches, result copies on a second stream) returns bit-identical final states, minimum
     distances and counters to cf_set_state + cf_step + cf_get_state + cf_get_aux; a second call continues correctly."""
