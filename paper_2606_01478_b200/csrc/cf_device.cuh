@@ -671,8 +671,12 @@ constexpr int kMaxBlock = 128;
 // The lean kernels' bounds are written as ONE block of 640 / 512 threads: the same register caps (<= 96 / <= 128), and
 // blocks of up to 512 threads may be launched -- used when every step is recorded (see pick_block in cf_api.cu).
 constexpr int kMaxBlockRec = 512;
+// The position-interface abstracted-model kernels (configs[3]: no obstacle table, no Philox) need fewer registers and
+// gain from a sixth resident block: bound 768 = 6 x 128 threads (<= 80 registers, 24 warps / SM): 5.98 -> 5.82 ms on
+// configs[3]; the same bound costs the planning kernels (configs[2], planner) 10 % (measured sweep of bounds 576 .. 832).
+constexpr int kBoundAbPos = 768;
 template <int MODEL, int INTEG, int IFACE, int OPT, int REC>
-__global__ void __launch_bounds__((OPT & OPT_EXTRAS) ? kMaxBlock : (MODEL == MODEL_AB ? 640 : 512), 1)
+__global__ void __launch_bounds__((OPT & OPT_EXTRAS) ? kMaxBlock : (MODEL == MODEL_AB ? (IFACE == IF_POSITION ? kBoundAbPos : 640) : 512), 1)
 rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevParams P) {
   constexpr int D = MODEL == MODEL_FP ? 17 : 13;
   constexpr int NP = MODEL == MODEL_FP ? 14 : 11;
