@@ -181,6 +181,22 @@ __device__ __forceinline__ void sincos3_step(const float *a, float *s, float *c)
   }
 }
 
+// The same for ANY angle without a branch: r = a - 2 pi k, k = rint(a / 2 pi) by magic-number rounding (exact for
+// |a / 2 pi| < 2^22), 2 pi split in two float32 constants (Cody-Waite: 2 pi = 6.2831855 - 1.7484556e-7), so |r| <= pi
+// whatever a is, then MUFU.  For |a| < pi: k = 0 and r = a exactly.  Four FMA-pipe instructions per angle more than the
+// tested form above -- but a step loop that uses it has no branch diamond left, and the compiler then schedules across
+// the step boundary and keeps loop constants live.  Used by the per-step-command (flat) loop of the lean abstracted-model
+// kernels, where that is worth 7 % (configs[2]: 0.699 -> 0.653 ms); the held-command loops measured no gain (planner
+// rollout -0.5 %, configs[3] -8 %) and keep the tested form.
+__device__ __forceinline__ float reduce_to_pi(float a) {
+  const float k = fmaf(a, 0.15915494309f, 12582912.0f) - 12582912.0f;
+  return fmaf(k, 1.7484556e-7f, fmaf(k, -6.2831855f, a));
+}
+__device__ __forceinline__ void sincos3_any(const float *a, float *s, float *c) {
+#pragma unroll
+  for (int j = 0; j < 3; ++j) { const float r = reduce_to_pi(a[j]); s[j] = mufu_sin(r); c[j] = mufu_cos(r); }
+}
+
 // reading R18: 23-bit midpoint uniform in (0,1), exact in float32:  u = ((x >> 9) + 0.5) 2^-23.
 // Built as the float 1.m (m = x >> 9) minus (1 - 2^-24): both are multiples of 2^-24, the difference is exact.
 __device__ __forceinline__ float u01(uint32_t x) {
@@ -905,7 +921,10 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       // sin / cos of the pre-step Euler angles (abstracted model, lean Euler step): taken first -- its range check is the
       // only data-dependent branch of the step -- and shared by the position tick and the integration
       float sn[3], cs[3];
-      if constexpr (AB_LEAN) sincos3_step(x + 3, sn, cs);
+      if constexpr (AB_LEAN) {
+        if constexpr (decltype(fetch_c)::value) sincos3_any(x + 3, sn, cs);     // flat loop: branch-free
+        else sincos3_step(x + 3, sn, cs);
+      }
       // (1) flat loop: this step's command (formed after the sin / cos so that everything below is one basic block)
       if constexpr (decltype(fetch_c)::value) fetch_command(IntC<1>{});
       // (2) position controller tick

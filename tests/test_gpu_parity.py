@@ -297,6 +297,40 @@ def test_rollout_host_equals_step_and_copies(cf, W, name, M, n_slices):
         assert np.array_equal(a.counters(), b.counters()) and a.step_counter == b.step_counter == (rep + 1) * wl.n_steps
 
 
+@pytest.mark.parametrize("big,n", [(1000.0, 4), (1.0e5, 1)])
+@pytest.mark.parametrize("loop", ["flat_noise", "flat_buffer", "held", "position"])
+def test_euler_angles_far_outside_the_mufu_range(cf, cfo, W, loop, big, n):
+    """The lean abstracted-model step takes sin / cos of the Euler angles from the MUFU unit: behind a range test in the
+    held-command loops (accurate sincosf beyond 2 pi), after a branch-free Cody-Waite reduction in the per-step-command
+    loop.  Both must be right for ANY angle: worlds with roll / pitch / yaw of up to +-1000 rad (4 steps) and +-1e5 rad (one
+    step from exactly representable inputs: an unreduced MUFU argument is off by |a| 2^-23 = 1e-2 rad there, 2.4e-4 m/s
+    in the velocity -- above the 1e-4 bar) against the oracle."""
+    M = 300
+    if loop == "flat_noise":
+        wl = W.cfg3(seed=4, M=M, n_steps=n)
+    elif loop == "flat_buffer":
+        wl = W.cfg3b(seed=4, M=M, n_steps=n)
+    elif loop == "held":
+        wl = W.cfg3b(seed=4, M=M, n_steps=2)
+        wl.cmd_hold, wl.n_steps = 2, n
+    else:
+        wl = W.cfg4(seed=4, M=3, N=100, n_steps=n)
+    g = cf.Sim(wl.M, wl.N, wl.model, wl.params)
+    o = cfo.OracleSim(wl.M, wl.N, wl.model, wl.params)
+    g.reset(wl.seed), o.reset(wl.seed)
+    x = o.get_state().copy()
+    rng = np.random.default_rng(7)
+    MN = wl.M * wl.N
+    scale = np.where(np.arange(MN) % 3 == 0, big, np.where(np.arange(MN) % 3 == 1, 12.0, 0.4))
+    x[3:6] = rng.uniform(-1, 1, (3, MN)) * scale
+    x[3:6, :4] = [[6.2831853, -6.2831855, 3.1415927, -3.1415925]] * 3            # at the edges of the tested range
+    x32 = x.astype(np.float32)
+    g.set_state(x32), o.set_state(x32.astype(np.float64))
+    g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold), o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold)
+    assert_state_close(g.get_state().cpu().numpy(), o.get_state(), wl.model, 1e-4, f"large angles, {loop}")
+    assert np.array_equal(g.counters(), o.counters())
+
+
 def test_rollout_host_status_codes(cf, W):
     import torch
     wl = W.cfg2(seed=1, M=64, n_steps=10)                       # no obstacles: there is no minimum distance to return
