@@ -619,7 +619,7 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
   LaunchCfg L;
   const int rec_mode = A ? A->rec_mode : sim->last_rec_mode;    // a dry run describes the kernel of the last cf_step
   if (A) sim->last_rec_mode = A->rec_mode;
-  if (A) sim->last_rec_heavy = A->rec_mode == REC_TMA && A->record_every <= 4 && !(sim->opt & OPT_EXTRAS);
+  if (A) sim->last_rec_heavy = (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR) && A->record_every <= 4 && !(sim->opt & OPT_EXTRAS);
   L.block = sim->last_rec_heavy ? pick_block_rec(sim->MN) : pick_block(sim->MN);
   L.grid = grid_for(A ? A->i_end - A->i_begin : sim->MN, L.block);
   // the kernel stages the parameter rows whenever ITS compile-time options carry OPT_RANDP and N > 1, and the
@@ -630,7 +630,7 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
       : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
   if (!found) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
   size_t smem_wp = ((opt_used & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
-  size_t smem_rec = (A && A->rec_mode == REC_TMA) ? kRecBufs * A->rec_group * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
+  size_t smem_rec = (A && (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR)) ? kRecBufs * A->rec_group * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
   L.smem = smem_wp > smem_rec ? smem_wp : smem_rec;
   L.stream = sim->stream;
   if (grid) *grid = L.grid;
@@ -696,11 +696,18 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
       for (int g = kRecGroupMax; g > 1 && group == 1; --g)
         if (g <= n_rec && kRecBufs * g * tile * (size_t)resident <= 200 * 1024) group = g;
     }
+    // the pair schedule as a compile-time fact (REC_PAIR): every step recorded, two snapshots per store, attitude tick
+    // every second step starting with this call's first, an even number of steps in command runs of even length
+    const bool pair = group >= 2 && record_every == 1 && sim->model == CF_MODEL_FIRST_PRINCIPLES &&
+        sim->p.iface == CF_IF_ATTITUDE && sim->p.integrator == CF_RK4 && !(sim->opt & OPT_EXTRAS) && sim->dp.att_div == 2 &&
+        s0 % 2 == 0 && n_steps % 2 == 0 && cmd_hold != 1 && (cmd_hold % 2 == 0 || cmd_hold >= n_steps) && n_rec == n_steps;
+    if (pair) group = 2;
     if (encode_record_map(&A.rec_map, record_dev, sim->MN, n_rec, sim->D, group) &&
         (group == 1 || encode_record_map(&A.rec_map1, record_dev, sim->MN, n_rec, sim->D, 1))) {
       if (group == 1) A.rec_map1 = A.rec_map;
       A.rec_mode = REC_TMA;
       A.rec_group = group;
+      if (pair) A.rec_mode = REC_PAIR;
     }
   }
   A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);

@@ -670,7 +670,12 @@ template <int N> __device__ __forceinline__ void tma_store_wait_read() {
 struct NoSmem { static constexpr bool value = false; };
 struct InSmem { static constexpr bool value = true; };
 template <int V> struct IntC { static constexpr int value = V; };
-enum : int { REC_NONE = 0, REC_SCALAR = 1, REC_TMA = 2, REC_RUNTIME = -1 };
+enum : int { REC_NONE = 0, REC_SCALAR = 1, REC_TMA = 2, REC_PAIR = 3, REC_RUNTIME = -1 };
+// REC_PAIR: REC_TMA for the record-EVERY-step runs of the first-principles attitude-interface kernels (configs[4]), with
+// the step loop written as pairs of steps whose schedule is a compile-time fact -- the attitude tick (period 2) in the
+// first step, one bulk-tensor store of both snapshots after the second -- so the loop body has no branch at all.  The
+// host selects it when record_every == 1, att_div == 2, two snapshots per store, and the call starts on an even step
+// and runs an even number of steps in runs of even length (cf_api.cu); otherwise REC_TMA.
 
 // The rollout kernel.  One thread = one drone; the state, controller state, held commands and plant parameters stay
 // in registers for all n_steps; HBM is touched for command loads, recorded states and the final store only.
@@ -715,6 +720,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
   // slices of the batch (cf_rollout_host) exist only for launches that record nothing: the recording lean kernels keep
   // the whole-batch geometry as a compile-time fact
   constexpr bool SLICED = REC == REC_NONE || REC == REC_RUNTIME;
+  static_assert(REC != REC_PAIR || (MODEL == MODEL_FP && IFACE >= IF_ATTITUDE), "REC_PAIR: first-principles kernels with the attitude controller");
   const int blk0 = (SLICED ? A.i_begin : 0) + (int)(blockIdx.x * blockDim.x);      // first drone of this block
   const int i_end = SLICED ? A.i_end : (int)MN;
   const long long i = blk0 + (int)threadIdx.x;
@@ -830,8 +836,9 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // record staging (REC_TMA): the warp's snapshots go to a [rec_group * D][32] tile (kRecBufs of them, used in turn); one
     // cp.async.bulk.tensor.2d of the whole tile by lane 0, box = 32 columns x rec_group * D rows at (column = first drone
     // of the warp, row = first slot of the group * D) of the [n_rec * D][MN] record tensor
-    float *rec_tile = wp_s + warp_u * (kRecBufs * A.rec_group * D * 32);
-    const uint32_t rec_tile_sa = (uint32_t)__cvta_generic_to_shared(wp_s) + (uint32_t)warp_u * (kRecBufs * A.rec_group * D * 128);
+    const int rec_group = REC == REC_PAIR ? 2 : A.rec_group;
+    float *rec_tile = wp_s + warp_u * (kRecBufs * rec_group * D * 32);
+    const uint32_t rec_tile_sa = (uint32_t)__cvta_generic_to_shared(wp_s) + (uint32_t)warp_u * (kRecBufs * rec_group * D * 128);
     const int rec_col = (int)blk0 + warp_u * 32;
     int rec_buf = 0, rec_grp = 0;
     // commands.  Buffer mode: one float4 per drone and command, prefetched one command ahead.  Noise mode: the nominal
@@ -916,7 +923,8 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       }
     };
     // (2)-(8) of one physics step
-    auto physics_step = [&](auto obst_in_smem, auto fetch_c) {
+    auto physics_step = [&](auto obst_in_smem, auto fetch_c, auto pair_c) {
+      constexpr int PH = decltype(pair_c)::value;        // REC_PAIR: 0 / 1 = first / second step of a pair; else -1
       const int rec_mode = REC == REC_RUNTIME ? A.rec_mode : REC;
       // sin / cos of the pre-step Euler angles (abstracted model, lean Euler step): taken first -- its range check is the
       // only data-dependent branch of the step -- and shared by the position tick and the integration
@@ -949,8 +957,12 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       }
       // (3) attitude controller tick + mixer
       if (HAS_ATT) {
-        if (att_phase == 0) attitude_tick<OPT>(P, x + 3, x + 10, Rd, att_cmd[3], iR, rpm_cmd);
-        att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
+        if constexpr (PH == 0) {
+          attitude_tick<OPT>(P, x + 3, x + 10, Rd, att_cmd[3], iR, rpm_cmd);
+        } else if constexpr (PH < 0) {
+          if (att_phase == 0) attitude_tick<OPT>(P, x + 3, x + 10, Rd, att_cmd[3], iR, rpm_cmd);
+          att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
+        }
       }
       // (4) disturbance of this step (drawn one step ahead, held over the RK4 stages) and the draw for the next step
       float fdist[3] = { 0, 0, 0 };
@@ -987,6 +999,23 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         cost = fmaf(P.cost_hw_pos, e2, fmaf(P.cost_hw_vel, v2, cost));
       }
       // (8) record
+      if constexpr (PH >= 0) {                      // REC_PAIR: every step recorded, two snapshots per store, no test
+        if constexpr (PH == 0) {
+          tma_store_wait_read<kRecBufs - 1>();      // the engine has read the tile handed over two pairs ago
+          __syncwarp();
+        }
+        float *t = rec_tile + (rec_buf * 2 + PH) * (D * 32);
+#pragma unroll
+        for (int j = 0; j < D; ++j) t[j * 32 + lane] = x[j];
+        if constexpr (PH == 1) {
+          fence_proxy_async_smem();
+          __syncwarp();
+          const int sb = __shfl_sync(0xffffffffu, kRecBufs * rec_slot + rec_buf, 0);
+          tma_store_tile_2d(&A.rec_map, rec_tile_sa + (sb % kRecBufs) * (2 * D * 128), rec_col, (sb / kRecBufs) * D, lane == 0);
+          rec_buf ^= 1;
+          rec_slot += 2;
+        }
+      } else
       if (rec_mode != REC_NONE) {
         if (++rec_phase == A.record_every) {
           rec_phase = 0;
@@ -1028,17 +1057,27 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // cfg4 +3 %); with a fresh command every step (cmd_hold == 1, configs[2]) the flat loop is 2 % faster.
     if (flat) {
 #pragma unroll 2
-      for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{});
+      for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{}, IntC<-1>{});
+    } else if constexpr (REC == REC_PAIR) {
+      for (int t = 0; t < A.n_steps;) {
+        fetch_command(IntC<0>{});
+        const int run_len = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;     // even (host)
+        t += run_len;
+        for (int k = 0; k < run_len; k += 2) {
+          physics_step(InSmem{}, IntC<0>{}, IntC<0>{});
+          physics_step(InSmem{}, IntC<0>{}, IntC<1>{});
+        }
+      }
     } else {
       for (int t = 0; t < A.n_steps;) {
         fetch_command(IntC<0>{});
         const int run_len = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;
         t += run_len;
-        for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{});
+        for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{});
       }
     }
-    if (REC == REC_TMA || (REC == REC_RUNTIME && A.rec_mode == REC_TMA)) {
-      if (rec_grp > 0) {                              // a partial last group leaves record by record (box = D rows)
+    if (REC == REC_TMA || REC == REC_PAIR || (REC == REC_RUNTIME && A.rec_mode == REC_TMA)) {
+      if (REC != REC_PAIR && rec_grp > 0) {                              // a partial last group leaves record by record (box = D rows)
         fence_proxy_async_smem();
         __syncwarp();
         const int sb = __shfl_sync(0xffffffffu, kRecBufs * (rec_slot - rec_grp) + rec_buf, 0);

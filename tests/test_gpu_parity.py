@@ -608,7 +608,8 @@ def test_tma_record_path_small_sizes(cf, cfo, W, name, kw, rec_every):
     g, o = fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
     assert "REC_NONE" in g.describe_launch()[0]
     rg = g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every).cpu().numpy()
-    assert "REC_TMA" in g.describe_launch()[0]
+    # configs[4] proper (RK4, every step recorded, an even run from an even step) takes the pair-scheduled kernel
+    assert ("REC_PAIR" if name == "cfg5" else "REC_TMA") in g.describe_launch()[0]
     ro = o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold, record_every=rec_every)
     assert rg.shape == ro.shape and rg.shape[0] == wl.n_steps // rec_every
     for k in range(ro.shape[0]):
@@ -618,6 +619,7 @@ def test_tma_record_path_small_sizes(cf, cfo, W, name, kw, rec_every):
     recs = []
     for cm, n, hold in split_calls(wl, [1, 2, 5, 3, 11]):
         r = b.step(cm, n, cmd_hold=hold, record_every=rec_every)
+        assert "REC_PAIR" not in b.describe_launch()[0] or (n % 2 == 0 and (b.step_counter - n) % 2 == 0)
         if r is not None:
             recs.append(r.cpu().numpy())
     rb = np.concatenate(recs)
