@@ -896,6 +896,14 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           for (int j = 0; j < 4; ++j) c[j] = clipf(fmaf(P.noise_sigma[j], z[j], c[j]), P.cmd_lo[j], P.cmd_hi[j]);
         } else {
           const float4 c4 = next_cmd;
+          if constexpr (decltype(piped_c)::value) {
+            // flat loop (a command every step): no branch -- the pointer stays on the last command (a harmless re-load)
+            // and the L2 prefetch on a line that has been read
+            --cmds_left;
+            cp += cmds_left > 0 ? MN : 0;
+            next_cmd = __ldg(cp);
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(cp + (cmds_left > 4 ? 4 * MN : 0)));
+          } else
           if (--cmds_left > 0) {
             cp += MN;
             next_cmd = __ldg(cp);
