@@ -148,6 +148,15 @@ static void fill_dev_params(cf_sim *s) {
   d.Jp_rad = (float)((double)p.Jp * 2.0 * 3.14159265358979323846 / 60.0);
   d.ab_ctau = p.ab_ctau; d.ab_cf = p.ab_cf; d.ab_thrust_dyn = p.ab_thrust_dyn;
   d.thrust_poly = (p.kf[0] != 0.f || p.kf[1] != 0.f);
+  {   // bound constants of the abstracted model's angle recursion over every world this simulator can hold (slot map of
+      // reset_params_kernel: a_j <- fac[1 + j], b_j <- fac[4 + j]), rounded up by 1e-6 relative
+    double ha = 0, hb1 = 0;
+    for (int j = 0; j < 3; ++j) {
+      ha = std::max(ha, h * std::fabs((double)p.ab_a[j]) * std::max(std::fabs((double)p.rnd_lo[1 + j]), std::fabs((double)p.rnd_hi[1 + j])));
+      hb1 = std::max(hb1, std::max(std::fabs(1.0 + h * p.ab_b[j] * p.rnd_lo[4 + j]), std::fabs(1.0 + h * p.ab_b[j] * p.rnd_hi[4 + j])));
+    }
+    d.bnd_ha = (float)(ha * (1.0 + 1e-6)); d.bnd_hb1 = (float)(hb1 * (1.0 + 1e-6));
+  }
   d.has_drag = (p.Ca[0] != 0.f || p.Ca[1] != 0.f || p.Ca[2] != 0.f);
   d.has_gyro = p.Jp != 0.f;
   d.inv_4lever = (float)(1.0 / (4.0 * lever));
@@ -469,7 +478,7 @@ extern "C" int cf_reset(cf_sim *sim, uint64_t seed) {
   set_counters_kernel<<<1, 1, 0, sim->stream>>>(sim->counters, 0u, 1);
   CF_CUDA(cudaMemsetAsync(sim->rec_table, 0, sizeof(uint32_t) * kRecTableCap, sim->stream));
   CF_CUDA(cudaGetLastError());
-  sim->seed = seed; sim->s_host = 0; sim->n_rec_host = 0; sim->have_state = true;
+  sim->seed = seed; sim->s_host = 0; sim->n_rec_host = 0; sim->have_state = true; sim->wparam_foreign = false;
   sim->pending_bcast = false; sim->md_valid = false; sim->cost_valid = false; sim->rearmed = true;
   return CF_OK;
 }
@@ -546,6 +555,7 @@ extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctr
   if (wparam_dev) {
     CF_CUDA(cudaMemcpyAsync(sim->wparam, wparam_dev, sizeof(float) * sim->P * (size_t)sim->M, cudaMemcpyDeviceToDevice, sim->stream));
     sim->opt |= OPT_RANDP;     // the planes are now authoritative
+    sim->wparam_foreign = true; // ... and the create-time bounds on the coefficients no longer hold
   }
   if (min_d2_dev) {
     if (!sim->min_d2) return fail(CF_E_ARG, "no obstacles configured");
@@ -720,6 +730,7 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
     A.i_begin = (int)i0;
     A.i_end = (int)(i0 + slice < sim->MN ? i0 + slice : sim->MN);
     A.advance = A.i_end == sim->MN;
+    A.ang_bound_ok = sim->wparam_foreign ? 0 : 1;
     int rc = do_launch(sim, &A, false, nullptr, nullptr, nullptr);
     if (rc != CF_OK) return rc;
     CF_CUDA(cudaGetLastError());

@@ -64,6 +64,9 @@ struct DevParams {
   int   cost_on;
   int   att_div, pos_div;
   float hover_thrust, hover_rpm;   // reading R20: held commands after a reset / set_state
+  // abstracted model, bound on the growth of the Euler angles (lean Euler step): over ALL worlds of this simulator
+  // max_j |h a_j| and max_j |1 + h b_j| (nominal coefficients x randomisation ranges); see run_angles_bounded
+  float bnd_ha, bnd_hb1;
 };
 
 struct StepArgs {
@@ -95,6 +98,7 @@ struct StepArgs {
   // (appended: the offsets of everything above -- the Philox keys are read with 8 / 16-byte constant loads -- stay put)
   int i_begin, i_end;         // (M N < 2^31) this launch advances the drones [i_begin, i_end) (a slice of the batch: cf_rollout_host; else [0, MN))
   int advance;                // this launch advances the device-side counters (the last slice of a call)
+  int ang_bound_ok;           // DevParams.bnd_* hold for every world (false after cf_set_full replaced the parameter planes)
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -931,14 +935,17 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       }
     };
     // (2)-(8) of one physics step
-    auto physics_step = [&](auto obst_in_smem, auto fetch_c, auto pair_c) {
+    auto physics_step = [&](auto obst_in_smem, auto fetch_c, auto pair_c, auto trig_c) {
       constexpr int PH = decltype(pair_c)::value;        // REC_PAIR: 0 / 1 = first / second step of a pair; else -1
       const int rec_mode = REC == REC_RUNTIME ? A.rec_mode : REC;
       // sin / cos of the pre-step Euler angles (abstracted model, lean Euler step): taken first -- its range check is the
       // only data-dependent branch of the step -- and shared by the position tick and the integration
       float sn[3], cs[3];
       if constexpr (AB_LEAN) {
-        if constexpr (decltype(fetch_c)::value) sincos3_any(x + 3, sn, cs);     // flat loop: branch-free
+        if constexpr (decltype(trig_c)::value) {                                // the caller has bounded the run's angles
+#pragma unroll
+          for (int j = 0; j < 3; ++j) { sn[j] = mufu_sin(x[3 + j]); cs[j] = mufu_cos(x[3 + j]); }
+        } else if constexpr (decltype(fetch_c)::value) sincos3_any(x + 3, sn, cs);     // flat loop: branch-free
         else sincos3_step(x + 3, sn, cs);
       }
       // (1) flat loop: this step's command (formed after the sin / cos so that everything below is one basic block)
@@ -1065,15 +1072,15 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // cfg4 +3 %); with a fresh command every step (cmd_hold == 1, configs[2]) the flat loop is 2 % faster.
     if (flat) {
 #pragma unroll 2
-      for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{}, IntC<-1>{});
+      for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{}, IntC<-1>{}, IntC<0>{});
     } else if constexpr (REC == REC_PAIR) {
       for (int t = 0; t < A.n_steps;) {
         fetch_command(IntC<0>{});
         const int run_len = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;     // even (host)
         t += run_len;
         for (int k = 0; k < run_len; k += 2) {
-          physics_step(InSmem{}, IntC<0>{}, IntC<0>{});
-          physics_step(InSmem{}, IntC<0>{}, IntC<1>{});
+          physics_step(InSmem{}, IntC<0>{}, IntC<0>{}, IntC<0>{});
+          physics_step(InSmem{}, IntC<0>{}, IntC<1>{}, IntC<0>{});
         }
       }
     } else {
@@ -1081,7 +1088,31 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         fetch_command(IntC<0>{});
         const int run_len = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;
         t += run_len;
-        for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{});
+        if constexpr (AB_LEAN && IFACE == IF_ATTITUDE) {
+          // Held command (abstracted model, attitude interface): the sin / cos range test is taken for the whole run
+          // from a bound on how far the angles can move while this command is held: with P = max_j |Psi_j|,
+          // Q = max_j |dPsi_j|, C = max_j |h c_j u_j| the Euler step of Eq. (10) gives P+ <= P + h Q,
+          // Q+ <= max|1 + h b| Q + max|h a| P + C (2 FFMA per step of the run).  Within 6.28 (the margin covers the
+          // rounding of the recursion) the run takes the test-free loop body.
+          bool bounded = A.ang_bound_ok != 0 && run_len <= 32;
+          if (bounded) {
+            float Pm = fmaxf(fmaxf(fabsf(x[3]), fabsf(x[4])), fabsf(x[5])), Qm = fmaxf(fmaxf(fabsf(x[9]), fabsf(x[10])), fabsf(x[11]));
+            const float C = fmaxf(fmaxf(fabsf(held[0]), fabsf(held[1])), fabsf(held[2]));
+            for (int k = 0; k < run_len; ++k) {
+              const float Pn = fmaf(P.h, Qm, Pm);
+              Qm = fmaf(P.bnd_hb1, Qm, fmaf(P.bnd_ha, Pm, C));
+              Pm = Pn;
+            }
+            bounded = Pm <= 6.28f;                  // NaN -> false
+          }
+          if (bounded) {
+            for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<1>{});
+          } else {
+            for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{});
+          }
+        } else {
+          for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{});
+        }
       }
     }
     if (REC == REC_TMA || REC == REC_PAIR || (REC == REC_RUNTIME && A.rec_mode == REC_TMA)) {

@@ -36,6 +36,7 @@ struct cf_sim {
   bool have_state;
   float hover_rpm;
   // cf_rollout_host: a second stream for the result copies and one event per slice (created on first use)
+  bool wparam_foreign = false;   // cf_set_full replaced the parameter planes (cf_reset re-draws them and clears this)
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t slice_ev[16] = {};
 };

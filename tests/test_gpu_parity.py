@@ -331,6 +331,40 @@ def test_euler_angles_far_outside_the_mufu_range(cf, cfo, W, loop, big, n):
     assert np.array_equal(g.counters(), o.counters())
 
 
+@pytest.mark.parametrize("case", ["near_the_bound", "foreign_parameters", "nan_state"])
+def test_held_command_runs_choose_the_right_loop_body(cf, cfo, W, case):
+    """Held-command runs of the abstracted model take the sin / cos test once per run from a bound on the angle growth
+    (create-time bounds on the coefficients).  Worlds that start just inside / outside the range with rates that carry
+    them across it within the run, parameter planes replaced through cf_set_full (the create-time bounds no longer hold:
+    coefficients three times larger), and a NaN state all have to come out as the oracle says."""
+    M = 257
+    wl = W.cfg3b(seed=6, M=M, n_steps=3)
+    wl.cmd_hold, wl.n_steps = 10, 30
+    g = cf.Sim(wl.M, 1, wl.model, wl.params)
+    o = cfo.OracleSim(wl.M, 1, wl.model, wl.params)
+    g.reset(wl.seed), o.reset(wl.seed)
+    x = o.get_state().copy()
+    rng = np.random.default_rng(3)
+    if case == "foreign_parameters":
+        wp = o.world_params().copy()
+        wp[1:10] *= 3.0                                              # a, b, c of Eq. (10)
+        g.set_full(wparam=wp.astype(np.float32)), o.set_full(wparam=wp.astype(np.float32).astype(np.float64))
+        x[3:6] = rng.uniform(-3.0, 3.0, (3, M))
+        x[9:12] = rng.uniform(-40.0, 40.0, (3, M))
+    else:
+        x[3:6] = rng.uniform(5.9, 6.6, (3, M)) * rng.choice([-1.0, 1.0], (3, M))
+        x[9:12] = rng.uniform(-60.0, 60.0, (3, M))
+    if case == "nan_state":
+        x[4, ::7] = np.nan
+    x32 = x.astype(np.float32)
+    g.set_state(x32), o.set_state(x32.astype(np.float64))
+    g.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold), o.step(wl.cmds, wl.n_steps, cmd_hold=wl.cmd_hold)
+    xg, xo = g.get_state().cpu().numpy(), o.get_state()
+    ok = np.isfinite(xo).all(axis=0)
+    assert np.array_equal(ok, np.isfinite(xg).all(axis=0)) and (case != "nan_state" or (~ok).sum() >= M // 7)
+    assert_state_close(xg[:, ok], xo[:, ok], wl.model, 2e-4, case)
+
+
 def test_rollout_host_status_codes(cf, W):
     import torch
     wl = W.cfg2(seed=1, M=64, n_steps=10)                       # no obstacles: there is no minimum distance to return
