@@ -934,8 +934,43 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         }
       }
     };
+    // (8) record the current state (the caller has decided that a record is due)
+    auto record_now = [&]() {
+      const int rec_mode = REC == REC_RUNTIME ? A.rec_mode : REC;
+      if (rec_slot < A.n_rec_cap) {
+        if (rec_mode == REC_TMA) {
+          // Consecutive record slots are consecutive row blocks of the record tensor, so K = A.rec_group snapshots
+          // are parked in one [K * D][32] tile and leave with ONE bulk-tensor store: the fence, the elected-lane
+          // issue and its scoreboard waits are paid once per K records.  Two such tiles alternate.
+          if (rec_grp == 0) {
+            tma_store_wait_read<kRecBufs - 1>();  // the engine has read the tile handed over two groups ago
+            __syncwarp();
+          }
+          float *t = rec_tile + (rec_buf * A.rec_group + rec_grp) * (D * 32);
+#pragma unroll
+          for (int j = 0; j < D; ++j) t[j * 32 + lane] = x[j];
+          if (++rec_grp == A.rec_group) {
+            fence_proxy_async_smem();             // generic-proxy writes -> visible to the async proxy
+            __syncwarp();
+            // first slot and buffer index as provably warp-uniform values (one shuffle): the TMA instruction takes
+            // its operands from uniform registers; without this the compiler wraps it in a per-lane uniformisation loop
+            const int sb = __shfl_sync(0xffffffffu, kRecBufs * (rec_slot + 1 - rec_grp) + rec_buf, 0);
+            tma_store_tile_2d(&A.rec_map, rec_tile_sa + (sb % kRecBufs) * (A.rec_group * D * 128), rec_col,
+                              (sb / kRecBufs) * D, lane == 0);
+            rec_buf = (rec_buf + 1) % kRecBufs;
+            rec_grp = 0;
+          }
+        } else {                                  // one streaming 4-byte store per component (any MN, any alignment)
+          float *r = A.record + (size_t)rec_slot * D * MN + i;
+#pragma unroll
+          for (int j = 0; j < D; ++j) __stcs(r + j * MN, x[j]);
+        }
+      }
+      ++rec_slot;
+    };
     // (2)-(8) of one physics step
-    auto physics_step = [&](auto obst_in_smem, auto fetch_c, auto pair_c, auto trig_c) {
+    // hoist_c: the caller runs the position tick and the record test outside the step (position-interface loop below)
+    auto physics_step = [&](auto obst_in_smem, auto fetch_c, auto pair_c, auto trig_c, auto hoist_c) {
       constexpr int PH = decltype(pair_c)::value;        // REC_PAIR: 0 / 1 = first / second step of a pair; else -1
       const int rec_mode = REC == REC_RUNTIME ? A.rec_mode : REC;
       // sin / cos of the pre-step Euler angles (abstracted model, lean Euler step): taken first -- its range check is the
@@ -951,7 +986,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       // (1) flat loop: this step's command (formed after the sin / cos so that everything below is one basic block)
       if constexpr (decltype(fetch_c)::value) fetch_command(IntC<1>{});
       // (2) position controller tick
-      if (HAS_POS) {
+      if (HAS_POS && !decltype(hoist_c)::value) {
         if (pos_phase == 0) {
           float zB[3];
           if (FP) {
@@ -1031,39 +1066,12 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           rec_slot += 2;
         }
       } else
-      if (rec_mode != REC_NONE) {
-        if (++rec_phase == A.record_every) {
-          rec_phase = 0;
-          if (rec_slot < A.n_rec_cap) {
-            if (rec_mode == REC_TMA) {
-              // Consecutive record slots are consecutive row blocks of the record tensor, so K = A.rec_group snapshots
-              // are parked in one [K * D][32] tile and leave with ONE bulk-tensor store: the fence, the elected-lane
-              // issue and its scoreboard waits are paid once per K records.  Two such tiles alternate.
-              if (rec_grp == 0) {
-                tma_store_wait_read<kRecBufs - 1>();  // the engine has read the tile handed over two groups ago
-                __syncwarp();
-              }
-              float *t = rec_tile + (rec_buf * A.rec_group + rec_grp) * (D * 32);
-#pragma unroll
-              for (int j = 0; j < D; ++j) t[j * 32 + lane] = x[j];
-              if (++rec_grp == A.rec_group) {
-                fence_proxy_async_smem();             // generic-proxy writes -> visible to the async proxy
-                __syncwarp();
-                // first slot and buffer index as provably warp-uniform values (one shuffle): the TMA instruction takes
-                // its operands from uniform registers; without this the compiler wraps it in a per-lane uniformisation loop
-                const int sb = __shfl_sync(0xffffffffu, kRecBufs * (rec_slot + 1 - rec_grp) + rec_buf, 0);
-                tma_store_tile_2d(&A.rec_map, rec_tile_sa + (sb % kRecBufs) * (A.rec_group * D * 128), rec_col,
-                                  (sb / kRecBufs) * D, lane == 0);
-                rec_buf = (rec_buf + 1) % kRecBufs;
-                rec_grp = 0;
-              }
-            } else {                                  // one streaming 4-byte store per component (any MN, any alignment)
-              float *r = A.record + (size_t)rec_slot * D * MN + i;
-#pragma unroll
-              for (int j = 0; j < D; ++j) __stcs(r + j * MN, x[j]);
-            }
+      if constexpr (!decltype(hoist_c)::value) {
+        if (rec_mode != REC_NONE) {
+          if (++rec_phase == A.record_every) {
+            rec_phase = 0;
+            record_now();
           }
-          ++rec_slot;
         }
       }
     };
@@ -1072,15 +1080,15 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
     // cfg4 +3 %); with a fresh command every step (cmd_hold == 1, configs[2]) the flat loop is 2 % faster.
     if (flat) {
 #pragma unroll 2
-      for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{}, IntC<-1>{}, IntC<0>{});
+      for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{}, IntC<-1>{}, IntC<0>{}, IntC<0>{});
     } else if constexpr (REC == REC_PAIR) {
       for (int t = 0; t < A.n_steps;) {
         fetch_command(IntC<0>{});
         const int run_len = A.n_steps - t < A.cmd_hold ? A.n_steps - t : A.cmd_hold;     // even (host)
         t += run_len;
         for (int k = 0; k < run_len; k += 2) {
-          physics_step(InSmem{}, IntC<0>{}, IntC<0>{}, IntC<0>{});
-          physics_step(InSmem{}, IntC<0>{}, IntC<1>{}, IntC<0>{});
+          physics_step(InSmem{}, IntC<0>{}, IntC<0>{}, IntC<0>{}, IntC<0>{});
+          physics_step(InSmem{}, IntC<0>{}, IntC<1>{}, IntC<0>{}, IntC<0>{});
         }
       }
     } else {
@@ -1106,12 +1114,53 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
             bounded = Pm <= 6.28f;                  // NaN -> false
           }
           if (bounded) {
-            for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<1>{});
+            for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<1>{}, IntC<0>{});
           } else {
-            for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{});
+            for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{}, IntC<0>{});
+          }
+        } else if constexpr (AB_LEAN && IFACE == IF_POSITION) {
+          // Position interface (configs[3]): the run is cut into sub-runs that end at the next position tick or the next
+          // record, whichever comes first, so that the tick (which sets the attitude command the sub-run holds), the
+          // record test and the angle bound sit BETWEEN sub-runs and the inner loop body has no branch left.
+          const int rec_mode = REC == REC_RUNTIME ? A.rec_mode : REC;
+          for (int k = 0; k < run_len;) {
+            if (pos_phase == 0) {                                     // (2) position tick on this step's pre-step state
+              float sn[3], cs[3], zB[3];
+              sincos3_step(x + 3, sn, cs);
+              zB[0] = cs[2] * sn[1] * cs[0] + sn[2] * sn[0]; zB[1] = sn[2] * sn[1] * cs[0] - cs[2] * sn[0];
+              zB[2] = cs[1] * cs[0];
+              position_tick(P, x, x + 6, zB, target, ip, att_cmd);
+              fold_command();
+            }
+            int sub = run_len - k;
+            if (P.pos_div - pos_phase < sub) sub = P.pos_div - pos_phase;
+            if (rec_mode != REC_NONE && A.record_every - rec_phase < sub) sub = A.record_every - rec_phase;
+            bool bounded = A.ang_bound_ok != 0 && sub <= 32;
+            if (bounded) {
+              float Pm = fmaxf(fmaxf(fabsf(x[3]), fabsf(x[4])), fabsf(x[5])), Qm = fmaxf(fmaxf(fabsf(x[9]), fabsf(x[10])), fabsf(x[11]));
+              const float C = fmaxf(fmaxf(fabsf(held[0]), fabsf(held[1])), fabsf(held[2]));
+              for (int j = 0; j < sub; ++j) {
+                const float Pn = fmaf(P.h, Qm, Pm);
+                Qm = fmaf(P.bnd_hb1, Qm, fmaf(P.bnd_ha, Pm, C));
+                Pm = Pn;
+              }
+              bounded = Pm <= 6.28f;
+            }
+            if (bounded) {
+              for (int j = 0; j < sub; ++j) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<1>{}, IntC<1>{});
+            } else {
+              for (int j = 0; j < sub; ++j) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{}, IntC<1>{});
+            }
+            k += sub;
+            pos_phase += sub;
+            if (pos_phase == P.pos_div) pos_phase = 0;
+            if (rec_mode != REC_NONE) {
+              rec_phase += sub;
+              if (rec_phase == A.record_every) { rec_phase = 0; record_now(); }
+            }
           }
         } else {
-          for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{});
+          for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{}, IntC<0>{});
         }
       }
     }
