@@ -629,7 +629,7 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
   LaunchCfg L;
   const int rec_mode = A ? A->rec_mode : sim->last_rec_mode;    // a dry run describes the kernel of the last cf_step
   if (A) sim->last_rec_mode = A->rec_mode;
-  if (A) sim->last_rec_heavy = (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR) && A->record_every <= 4 && !(sim->opt & OPT_EXTRAS);
+  if (A) sim->last_rec_heavy = (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR || A->rec_mode == REC_TMA_P) && A->record_every <= 4 && !(sim->opt & OPT_EXTRAS);
   L.block = sim->last_rec_heavy ? pick_block_rec(sim->MN) : pick_block(sim->MN);
   L.grid = grid_for(A ? A->i_end - A->i_begin : sim->MN, L.block);
   // the kernel stages the parameter rows whenever ITS compile-time options carry OPT_RANDP and N > 1, and the
@@ -640,7 +640,7 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
       : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
   if (!found) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
   size_t smem_wp = ((opt_used & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
-  size_t smem_rec = (A && (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR)) ? kRecBufs * A->rec_group * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
+  size_t smem_rec = (A && (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR || A->rec_mode == REC_TMA_P)) ? kRecBufs * A->rec_group * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
   L.smem = smem_wp > smem_rec ? smem_wp : smem_rec;
   L.stream = sim->stream;
   if (grid) *grid = L.grid;
@@ -720,6 +720,13 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
       if (pair) A.rec_mode = REC_PAIR;
     }
   }
+  // pair-written loops for the other record modes (REC_*_P, cf_device.cuh): nominal-plant first-principles kernels with
+  // the attitude interface, tick period 2, an even number of steps from an even step in command runs of even length,
+  // records never, every step, or with an even period
+  if (A.rec_mode != REC_PAIR && sim->model == CF_MODEL_FIRST_PRINCIPLES && sim->p.iface == CF_IF_ATTITUDE &&
+      (sim->opt & ~OPT_RANDP) == 0 && sim->dp.att_div == 2 && s0 % 2 == 0 && n_steps % 2 == 0 && cmd_hold != 1 &&
+      (cmd_hold % 2 == 0 || cmd_hold >= n_steps) && (record_every <= 1 || record_every % 2 == 0))
+    A.rec_mode += REC_NONE_P;        // REC_NONE / REC_SCALAR / REC_TMA -> their _P forms
   A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);
   for (int r = 0; r < 10; ++r) {      // Philox key schedule: k += (0x9E3779B9, 0xBB67AE85) per round
     A.rk[2 * r] = A.seed_lo + (uint32_t)r * 0x9E3779B9u;

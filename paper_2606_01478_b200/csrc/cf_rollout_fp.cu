@@ -20,6 +20,9 @@ static const RolloutEntry kTableFP[] = {
   // record-every-step runs with the pair schedule as a compile-time fact (REC_PAIR, cf_device.cuh)
   // (RK4 only: configs[4] 1.288 -> 1.253 ms; the Euler kernel of variant 5E measured 2.8 % slower with it)
   CF_FP1(INTEG_RK4, IF_ATTITUDE, 0, REC_PAIR), CF_FP1(INTEG_RK4, IF_ATTITUDE, OPT_RANDP | OPT_DIST, REC_PAIR),
+  // the pair-written loop for the other record modes (REC_*_P): configs[0], configs[1], the world-count sweep
+  CF_FP1(INTEG_RK4, IF_ATTITUDE, 0, REC_NONE_P), CF_FP1(INTEG_RK4, IF_ATTITUDE, 0, REC_SCALAR_P), CF_FP1(INTEG_RK4, IF_ATTITUDE, 0, REC_TMA_P),
+  CF_FP1(INTEG_EULER, IF_ATTITUDE, 0, REC_NONE_P), CF_FP1(INTEG_EULER, IF_ATTITUDE, 0, REC_SCALAR_P), CF_FP1(INTEG_EULER, IF_ATTITUDE, 0, REC_TMA_P),
   // general kernels
   CF_FP_GEN(INTEG_EULER, IF_ROTOR),    CF_FP_GEN(INTEG_RK4, IF_ROTOR),
   CF_FP_GEN(INTEG_EULER, IF_TORQUE),   CF_FP_GEN(INTEG_RK4, IF_TORQUE),

@@ -365,6 +365,32 @@ def test_held_command_runs_choose_the_right_loop_body(cf, cfo, W, case):
     assert_state_close(xg[:, ok], xo[:, ok], wl.model, 2e-4, case)
 
 
+def test_pair_written_loops_are_selected_and_equal_the_plain_ones(cf, cfo, W):
+    """First-principles attitude kernels, tick period 2: calls of an even number of steps from an even step take the
+    pair-written loop (REC_*_P / REC_PAIR), everything else the plain one; both give the same trajectory (the oracle's)."""
+    for name, rec_every, label in (("cfg2", 10, "REC_TMA_P"), ("cfg2", 0, "REC_NONE_P"), ("cfg1", 1, "REC_SCALAR_P"),
+                                   ("cfg2", 1, "REC_PAIR"), ("cfg2", 3, "REC_TMA>")):
+        wl = W.make(name, seed=2, **(dict(M=64, n_steps=100) if name == "cfg2" else dict(n_steps=100)))
+        g, b, o = fresh_gpu(cf, wl), fresh_gpu(cf, wl), fresh_oracle(cfo, wl)
+        rg = g.step(wl.cmds, 100, cmd_hold=wl.cmd_hold, record_every=rec_every)
+        assert label in g.describe_launch()[0], (name, rec_every, g.describe_launch()[0])
+        ro = o.step(wl.cmds, 100, cmd_hold=wl.cmd_hold, record_every=rec_every)
+        recs = []
+        for cm, n, hold in split_calls(wl, [7, 20, 33, 40]):                  # odd starts / lengths: the plain loops
+            r = b.step(cm, n, cmd_hold=hold, record_every=rec_every)
+            assert "_P" not in b.describe_launch()[0] or (n % 2 == 0 and (b.step_counter - n) % 2 == 0)
+            if r is not None:
+                recs.append(r.cpu().numpy())
+        assert_state_close(g.get_state().cpu().numpy(), o.get_state(), wl.model, 2e-4, f"{name} paired")
+        fl = floors(wl.model)[0][:, None]
+        assert (np.abs(b.get_state().cpu().numpy() - g.get_state().cpu().numpy()) / np.maximum(np.abs(o.get_state()), fl)).max() <= 1e-6
+        if rec_every:
+            rb = np.concatenate(recs)
+            assert rb.shape == tuple(rg.shape) == ro.shape
+            assert (np.abs(rb - rg.cpu().numpy()) / np.maximum(np.abs(ro), fl[None])).max() <= 1e-6
+        assert np.array_equal(g.counters(), o.counters()) and np.array_equal(b.counters(), o.counters())
+
+
 def test_rollout_host_status_codes(cf, W):
     import torch
     wl = W.cfg2(seed=1, M=64, n_steps=10)                       # no obstacles: there is no minimum distance to return
