@@ -763,9 +763,7 @@ template <int MODEL, int IFACE, int OPT = 0> struct Hist {
 // 3 / 5 / 6 / 8 blocks for either phase measured no better than 4.
 // General kernels (OPT = GOPT: fidelity extras gated at run time by the DevParams flags, disturbances, torque interface):
 // the generic integrator and 17 / 13-wide pull-back, full record per step, 2 blocks per SM (<= 255 registers).
-// PAIRED: the sweeps are written in pairs of steps with the attitude tick (period 2, call starts on an even step, even
-// number of steps) in the even step as a compile-time fact: no tick test in either loop body.
-template <int MODEL, int INTEG, int IFACE, int PHASE, int OPT = 0, bool PAIRED = false>
+template <int MODEL, int INTEG, int IFACE, int PHASE, int OPT = 0>
 __global__ void __launch_bounds__(128, OPT != 0 ? 2 : GRAD_MIN_BLOCKS)
 grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParams P, int randp) {
   using H = Hist<MODEL, IFACE, OPT>;
@@ -851,13 +849,13 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
   // rollout kernel's command-buffer loop from 0.495 to 0.361 ms)
   float4 c_next = make_float4(0.f, 0.f, 0.f, 0.f);
   if constexpr (PHASE != 2) c_next = __ldg(A.cmds + i);
-  int f_hold = 0, f_k = 0;                                  // t = f_k * cmd_hold + f_hold, no division
-  auto fwd_step = [&](int t, auto par_c) {
+  if constexpr (PHASE != 2)
+  for (int t = 0, hold_phase = 0, k_cmd = 0; t < A.n_steps; ++t) {      // t = k_cmd * cmd_hold + hold_phase, no division
     float rec[HP];                                          // pre-step state and controller state of this step
     pack(rec);
     const float4 c4 = c_next;
-    c_next = __ldg(A.cmds + (size_t)(f_k + 1 < A.n_cmds ? f_k + 1 : f_k) * MN + i);
-    if (f_hold == 0) {
+    c_next = __ldg(A.cmds + (size_t)(k_cmd + 1 < A.n_cmds ? k_cmd + 1 : k_cmd) * MN + i);
+    if (hold_phase == 0) {
       cmd[0] = c4.x; cmd[1] = c4.y; cmd[2] = c4.z; cmd[3] = c4.w;
       if (FP && IFACE == IF_ROTOR) {
 #pragma unroll
@@ -865,7 +863,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
       }
       if (FP && IFACE == IF_TORQUE) mixer<OPT>(P, cmd[3], cmd, rpm_cmd);      // (tau_x, tau_y, tau_z, F) straight into the mixer
     }
-    if (++f_hold == A.cmd_hold) { f_hold = 0; ++f_k; }
+    if (++hold_phase == A.cmd_hold) { hold_phase = 0; ++k_cmd; }
     if (POS) {
       if (pos_phase == 0) {
         float zB[3], sn[3], cs[3];
@@ -876,19 +874,12 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     }
     const float *acmd = POS ? att_cmd : cmd;                // the attitude command in force at this step
     if (HAS_ATT) {
-      constexpr int PAR = decltype(par_c)::value;           // PAIRED: 0 = even step (tick), 1 = odd step; else -1
-      if constexpr (PAR < 0) {
-        if (att_phase == 0) {
-          float Rd[3][3];
-          euler_to_R(acmd[0], acmd[1], acmd[2], Rd);
-          attitude_tick<OPT>(P, x + 3, x + 10, Rd, acmd[3], iR, rpm_cmd);
-        }
-        att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
-      } else if constexpr (PAR == 0) {
+      if (att_phase == 0) {
         float Rd[3][3];
         euler_to_R(acmd[0], acmd[1], acmd[2], Rd);
         attitude_tick<OPT>(P, x + 3, x + 10, Rd, acmd[3], iR, rpm_cmd);
       }
+      att_phase = att_phase + 1 == P.att_div ? 0 : att_phase + 1;
     }
     if constexpr (FULL) {
       constexpr int o = FP ? D + 6 : D + 3;
@@ -909,13 +900,6 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     float fd[3];
     disturbance(A.s0 + (uint32_t)t, fd);
     step_forward<MODEL, INTEG, OPT>(P, pl, x, FP ? rpm_cmd : acmd, fd);
-    };
-  if constexpr (PHASE != 2) {
-    if constexpr (PAIRED) {
-      for (int t = 0; t < A.n_steps; t += 2) { fwd_step(t, IntC<0>{}); fwd_step(t + 1, IntC<1>{}); }
-    } else {
-      for (int t = 0; t < A.n_steps; ++t) fwd_step(t, IntC<-1>{});
-    }
   }
   // ---- loss and its cotangent ----------------------------------------------------------------------------------
   float lam[D];
@@ -943,7 +927,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
 #pragma unroll
   for (int j = 0; j < D; ++j) x[j] = 0.f;                   // components that are not parked enter only linearly
   int hold_phase = (A.n_steps - 1) % A.cmd_hold, k_cmd = (A.n_steps - 1) / A.cmd_hold;    // of step t, kept by counting
-  auto bwd_step = [&](int t, auto par_c) {
+  for (int t = A.n_steps - 1; t >= 0; --t) {
     float rec[HP];
     if (t > 0) {            // pull the previous step's record towards L2 while this step's pull-back computes
 #pragma unroll
@@ -1003,18 +987,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
       step_backward<MODEL, INTEG, OPT>(P, pl, x, FP ? rpm_cmd : acmd, fd, lam, FP ? g_rpm : g_acmd);
     }
     if (HAS_ATT) {
-      constexpr int PAR = decltype(par_c)::value;           // PAIRED: 0 = even step (tick), 1 = odd step; else -1
-      if constexpr (PAR < 0) {
-        if (att_phase == 0) {
-          float g_prev[3];
-          vjp_attitude_tick<OPT>(P, x + 3, x + 10, acmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_acmd, g_prev);
-  #pragma unroll
-          for (int j = 0; j < 3; ++j) g_iR[j] = g_prev[j];
-  #pragma unroll
-          for (int j = 0; j < 4; ++j) g_rpm[j] = 0.f;
-        }
-        att_phase = att_phase == 0 ? P.att_div - 1 : att_phase - 1;
-      } else if constexpr (PAR == 0) {
+      if (att_phase == 0) {
         float g_prev[3];
         vjp_attitude_tick<OPT>(P, x + 3, x + 10, acmd, iR, g_rpm, g_iR, lam + 3, lam + 10, g_acmd, g_prev);
 #pragma unroll
@@ -1022,6 +995,7 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
 #pragma unroll
         for (int j = 0; j < 4; ++j) g_rpm[j] = 0.f;
       }
+      att_phase = att_phase == 0 ? P.att_div - 1 : att_phase - 1;
     }
     if (POS) {
       if (pos_phase == 0) {           // the tick of this step produced att_cmd from (p, v, attitude, target, ip)
@@ -1056,11 +1030,6 @@ grad_kernel(const __grid_constant__ GradArgs A, const __grid_constant__ DevParam
     } else {
       --hold_phase;
     }
-    };
-  if constexpr (PAIRED) {
-    for (int t = A.n_steps - 1; t >= 1; t -= 2) { bwd_step(t, IntC<1>{}); bwd_step(t - 1, IntC<0>{}); }
-  } else {
-    for (int t = A.n_steps - 1; t >= 0; --t) bwd_step(t, IntC<-1>{});
   }
 }
 
@@ -1074,9 +1043,6 @@ const Entry kTable[] = {
   CF_G(MODEL_FP, INTEG_EULER, IF_POSITION), CF_G(MODEL_FP, INTEG_RK4, IF_POSITION),
   CF_G(MODEL_AB, INTEG_EULER, IF_POSITION), CF_G(MODEL_AB, INTEG_RK4, IF_POSITION),
 };
-// pair-written sweeps (PAIRED): first-principles model, attitude interface, tick period 2, even start and length
-#define CF_GP(M_, I_, F_) { M_, I_, F_, grad_kernel<M_, I_, F_, 1, 0, true>, grad_kernel<M_, I_, F_, 2, 0, true> }
-const Entry kTablePair[] = { CF_GP(MODEL_FP, INTEG_EULER, IF_ATTITUDE), CF_GP(MODEL_FP, INTEG_RK4, IF_ATTITUDE) };
 // the general kernels: fidelity extras, force disturbances (L280), torque interface (L330)
 #define CF_GG(M_, I_, F_) { M_, I_, F_, grad_kernel<M_, I_, F_, 1, GOPT>, grad_kernel<M_, I_, F_, 2, GOPT> }
 const Entry kTableGen[] = {
@@ -1131,9 +1097,6 @@ extern "C" int cf_grad(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   } else {
     for (const Entry &c : kTable)
       if (c.model == sim->model && c.integ == sim->p.integrator && c.iface == sim->p.iface) e = &c;
-    if (sim->dp.att_div == 2 && sim->s_host % 2 == 0 && n_steps % 2 == 0)
-      for (const Entry &c : kTablePair)
-        if (c.model == sim->model && c.integ == sim->p.integrator && c.iface == sim->p.iface) e = &c;
   }
   if (!e) return fail(CF_E_UNSUPPORTED, "cf_grad: the abstracted model has no rotor / torque interface");
   rc = cf_materialise(sim);      // a pending broadcast cf_set_state must be in the planes: the kernel reads them
