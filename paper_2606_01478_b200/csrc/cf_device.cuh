@@ -1082,11 +1082,14 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
         }
       }
     };
+    // unroll factors measured on the branch-free loop bodies (1 / 2 / 4 / 5): the per-step-command loop x2 with in-kernel
+    // noise commands, x4 with a command buffer (cfg3b +2 %); the bounded held-command loop x2 (planner rollout +2.3 %)
+    constexpr int kUnrollFlat = (OPT & OPT_NOISE) ? 2 : 4;
     // The call starts at a command boundary (C8), so a run of cmd_hold steps starts with ONE command fetch.  With held
     // commands the loop is two-level and the inner loop carries no command logic (mppi rollout kernel 705 -> 691 us,
     // cfg4 +3 %); with a fresh command every step (cmd_hold == 1, configs[2]) the flat loop is 2 % faster.
     if (flat) {
-#pragma unroll 2
+#pragma unroll kUnrollFlat
       for (int t = 0; t < A.n_steps; ++t) physics_step(NoSmem{}, IntC<1>{}, IntC<-1>{}, IntC<0>{}, IntC<0>{});
     } else if constexpr (PAIRED) {
       const bool rec_each = RECB != REC_NONE && A.record_every == 1;
@@ -1132,6 +1135,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
             bounded = Pm <= 6.28f;                  // NaN -> false
           }
           if (bounded) {
+#pragma unroll 2
             for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<1>{}, IntC<0>{});
           } else {
             for (int k = 0; k < run_len; ++k) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{}, IntC<0>{});
