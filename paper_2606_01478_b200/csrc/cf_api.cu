@@ -839,9 +839,11 @@ extern "C" int cf_rollout_host(cf_sim *sim, const float *x0_host, const void *cm
   long long slice = ((sim->MN + n_slices - 1) / n_slices + 1023) / 1024 * 1024;
   RolloutCopy ctx = { sim, state_host, min_dist_host };
   int rc = step_launch(sim, staging_dev, n_cmds, cmd_hold, n_steps, 0, nullptr, 0, slice, rollout_copy_slice, &ctx);
+  // both streams are drained whatever happened: copies of the slices that did run may still be in flight
+  cudaError_t e1 = cudaStreamSynchronize(sim->copy_stream), e2 = cudaStreamSynchronize(sim->stream);
   if (rc != CF_OK) return rc;
-  CF_CUDA(cudaStreamSynchronize(sim->copy_stream));
-  CF_CUDA(cudaStreamSynchronize(sim->stream));
+  CF_CUDA(e1);
+  CF_CUDA(e2);
   return CF_OK;
 }
 
