@@ -976,6 +976,7 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       ++rec_slot;
     };
     // (2)-(8) of one physics step
+    float sn_t[3] = { 0, 0, 0 }, cs_t[3] = { 1, 1, 1 };     // sin / cos taken by a hoisted position tick, reused by the step that follows
     // hoist_c: the caller runs the position tick and the record test outside the step (position-interface loop below)
     auto physics_step = [&](auto obst_in_smem, auto fetch_c, auto pair_c, auto trig_c, auto hoist_c) {
       constexpr int PH = decltype(pair_c)::value;        // REC_PAIR: 0 / 1 = first / second step of a pair; else -1
@@ -984,7 +985,10 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
       // only data-dependent branch of the step -- and shared by the position tick and the integration
       float sn[3], cs[3];
       if constexpr (AB_LEAN) {
-        if constexpr (decltype(trig_c)::value) {                                // the caller has bounded the run's angles
+        if constexpr (decltype(trig_c)::value == 2) {                           // the position tick just took them (same state)
+#pragma unroll
+          for (int j = 0; j < 3; ++j) { sn[j] = sn_t[j]; cs[j] = cs_t[j]; }
+        } else if constexpr (decltype(trig_c)::value == 1) {                    // the caller has bounded the run's angles
 #pragma unroll
           for (int j = 0; j < 3; ++j) { sn[j] = mufu_sin(x[3 + j]); cs[j] = mufu_cos(x[3 + j]); }
         } else if constexpr (decltype(fetch_c)::value) sincos3_any(x + 3, sn, cs);     // flat loop: branch-free
@@ -1146,11 +1150,12 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
           // record test and the angle bound sit BETWEEN sub-runs and the inner loop body has no branch left.
           const int rec_mode = REC == REC_RUNTIME ? A.rec_mode : RECB;
           for (int k = 0; k < run_len;) {
-            if (pos_phase == 0) {                                     // (2) position tick on this step's pre-step state
-              float sn[3], cs[3], zB[3];
-              sincos3_step(x + 3, sn, cs);
-              zB[0] = cs[2] * sn[1] * cs[0] + sn[2] * sn[0]; zB[1] = sn[2] * sn[1] * cs[0] - cs[2] * sn[0];
-              zB[2] = cs[1] * cs[0];
+            const bool ticked = pos_phase == 0;
+            if (ticked) {                                             // (2) position tick on this step's pre-step state
+              float zB[3];
+              sincos3_step(x + 3, sn_t, cs_t);
+              zB[0] = cs_t[2] * sn_t[1] * cs_t[0] + sn_t[2] * sn_t[0]; zB[1] = sn_t[2] * sn_t[1] * cs_t[0] - cs_t[2] * sn_t[0];
+              zB[2] = cs_t[1] * cs_t[0];
               position_tick(P, x, x + 6, zB, target, ip, att_cmd);
               fold_command();
             }
@@ -1168,10 +1173,12 @@ rollout_kernel(const __grid_constant__ StepArgs A, const __grid_constant__ DevPa
               }
               bounded = Pm <= 6.28f;
             }
+            int j0 = 0;
+            if (ticked) { physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<2>{}, IntC<1>{}); j0 = 1; }   // the tick's sin / cos
             if (bounded) {
-              for (int j = 0; j < sub; ++j) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<1>{}, IntC<1>{});
+              for (int j = j0; j < sub; ++j) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<1>{}, IntC<1>{});
             } else {
-              for (int j = 0; j < sub; ++j) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{}, IntC<1>{});
+              for (int j = j0; j < sub; ++j) physics_step(InSmem{}, IntC<0>{}, IntC<-1>{}, IntC<0>{}, IntC<1>{});
             }
             k += sub;
             pos_phase += sub;
