@@ -247,6 +247,28 @@ size_t cf_mppi_scratch_bytes(const cf_sim *sim, const cf_mppi_params *mp);
  * aligned, caller-owned.  Enqueues on the bound stream. */
 int cf_mppi_update(cf_sim *sim, const cf_mppi_params *mp, void *nominal_dev, void *plan_dev, void *info_dev,
                    int32_t *elite_idx_dev, void *scratch_dev, size_t scratch_bytes);
+/* cf_mppi_update for callers that have no device memory to give as scratch and no way of getting any.
+ * Two kinds of caller are meant.  (1) A planner thread inside a fixed-rate control loop (the 50 Hz loop of
+ * PAPER.md:L465-L471): cudaMalloc / cudaFree take driver locks and may synchronise the whole device, so a loop with a
+ * deadline must not call them after start-up, and it may not know n_elite / horizon (which size the scratch) before then.
+ * (2) A component living inside someone else's process -- a plug-in, or code running under a framework that owns the
+ * device's memory pool and hands out fixed input / output buffers only -- which is simply not allowed to allocate.
+ * Here the scratch (elite index list, weighted command rows, per-controller means, completion counter) is a fixed
+ * CF_MPPI_STATIC_SCRATCH_BYTES array compiled into libcf.so; the caller passes inputs and outputs only, and the call runs
+ * no cudaMalloc, cudaFree or other allocating routine.  Results are those of cf_mppi_update (same kernel, same arithmetic).
+ *   Limit: cf_mppi_scratch_bytes(sim, mp) <= CF_MPPI_STATIC_SCRATCH_BYTES (8 MiB; BASELINE.json's planner -- 5 controllers,
+ *     1000 elites, 25 knots -- needs 2.1 MB), else CF_E_BUFFER with both numbers in cf_last_error(); nothing is launched.
+ *   Cost: every GPU whose context loads libcf.so carries the 8 MiB from then until the process exits, used or not.
+ *   Set-up: the first call on each device looks up the array's address on THAT device (the device that is current, which
+ *     must be the one holding the simulator's workspace: checked, CF_E_ARG otherwise) and keeps it; make that first call
+ *     during start-up, outside any stream capture.  Later calls only enqueue a 4-byte memset and the kernel.
+ *   Sharing: there is ONE array per device for all simulators, streams and host threads.  It still holds the previous
+ *     call's data on entry (the one word that has to start at zero is cleared on the stream by every call), and two calls
+ *     whose kernels can overlap on the GPU -- different streams, or different simulators bound to different streams --
+ *     overwrite each other's scratch: order them on one stream or with events.  Same-stream calls are safe back to back. */
+#define CF_MPPI_STATIC_SCRATCH_BYTES ((size_t)8 << 20)
+int cf_mppi_update_static(cf_sim *sim, const cf_mppi_params *mp, void *nominal_dev, void *plan_dev, void *info_dev,
+                          int32_t *elite_idx_dev);
 /* One planning iteration: cf_set_state(x0_dev [D], broadcast) + cf_step(nominal_dev, H, cmd_hold, H*cmd_hold) +
  * cf_mppi_update(...). */
 int cf_mppi_iterate(cf_sim *sim, const cf_mppi_params *mp, const float *x0_dev, void *nominal_dev, void *plan_dev,

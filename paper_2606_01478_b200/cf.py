@@ -112,6 +112,7 @@ def lib():
         "cf_set_plan_state": (C.c_int, [vp, vp, vp]),
         "cf_mppi_scratch_bytes": (sz, [vp, C.POINTER(MppiParams)]),
         "cf_mppi_update": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, sz]),
+        "cf_mppi_update_static": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp]),
         "cf_mppi_iterate": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, sz]),
         "cf_mppi_iterate_host": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, vp, sz]),
         "cf_mppi_pack_best": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, C.c_int, vp]),
@@ -139,7 +140,7 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
            "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host", "cf_grad_scratch_bytes",
            "cf_grad", "cf_depth", "cf_reset_masked", "cf_grad_staging_bytes", "cf_grad_host", "cf_depth_host",
-           "cf_mppi_pack_best", "cf_mppi_select", "cf_rollout_host"]
+           "cf_mppi_pack_best", "cf_mppi_select", "cf_rollout_host", "cf_mppi_update_static"]
 
 
 def _check(rc: int):
@@ -508,6 +509,16 @@ class Sim:
         _check(lib().cf_mppi_update(self._h, C.byref(mp), _dptr(nominal), _dptr(self._mppi_plan),
                                     _dptr(self._mppi_info), el, sp, need))
         return self._mppi_result(nominal, want_elites)
+
+    def mppi_update_static(self, mp: MppiParams, nominal, plan, info, elites=None):
+        """cf_mppi_update_static: the planner update for callers that may not allocate device memory (a control loop
+        with a deadline, a plug-in under someone else's memory pool).  The scratch is an 8 MiB array inside libcf.so, so
+        this method creates no tensor either: `plan` [H][4] float32, `info` [4 n_ctrl + 4] float32 and, optionally,
+        `elites` [n_ctrl][n_elite] int32 are the caller's CUDA tensors and are written in place, `nominal`
+        [n_ctrl][H][4] is updated in place.  One scratch array per GPU is shared by every simulator: keep calls that
+        could overlap on the device on one stream.  CfError(CF_E_BUFFER) if the update needs more than the array holds."""
+        _check(lib().cf_mppi_update_static(self._h, C.byref(mp), _dptr(nominal), _dptr(plan), _dptr(info),
+                                           _dptr(elites) if elites is not None else None))
 
     def mppi_iterate(self, mp: MppiParams, x0, nominal, want_elites: bool = False):
         """One planning iteration: broadcast reset to x0 [D] + fused rollout + update (cf_mppi_iterate)."""

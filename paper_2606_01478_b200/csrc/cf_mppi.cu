@@ -20,6 +20,7 @@
 
 #include <cmath>
 #include <cooperative_groups.h>
+#include <mutex>
 
 namespace cg = cooperative_groups;
 
@@ -405,6 +406,59 @@ extern "C" int cf_mppi_update(cf_sim *sim, const cf_mppi_params *mp, void *nomin
   mppi_update_kernel<<<A.n_ctrl * kCluster, kThreads, 0, sim->stream>>>(A, sim->dp);     // one 8-CTA cluster per controller
   CF_CUDA(cudaGetLastError());
   return CF_OK;
+}
+
+// ---- cf_mppi_update_static: the same update with the scratch inside the library (include/cf.h says who needs this) --------
+// The array is ordinary global memory of every device that loads this module; it is never freed and never initialised.
+// In HOST code the identifier below is only a handle for the runtime's symbol table -- not a device address: handing
+// `g_static_scratch` itself to a kernel would make the kernel dereference a host pointer.  The device address is what
+// cudaGetSymbolAddress returns, and it differs from device to device, hence the per-device table.
+namespace {
+static __device__ __align__(256) unsigned char g_static_scratch[CF_MPPI_STATIC_SCRATCH_BYTES];
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+void *g_static_addr[kMaxDevices] = {};        // device ordinal -> device address of g_static_scratch, filled on first use
+
+// Address of the scratch array on the CURRENT device (looked up once per device, under a lock: callers may be threads).
+int static_scratch_addr(int dev, void **out) {
+  if (dev < 0 || dev >= kMaxDevices) return fail(CF_E_UNSUPPORTED, "device ordinal %d beyond the %d this table holds", dev, kMaxDevices);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_addr[dev]) {
+    void *addr = nullptr;
+    CF_CUDA(cudaGetSymbolAddress(&addr, g_static_scratch));      // resolves against the current device's copy of the module
+    if (!addr) return fail(CF_E_CUDA, "cudaGetSymbolAddress returned a NULL address for the static scratch");
+    g_static_addr[dev] = addr;
+  }
+  *out = g_static_addr[dev];
+  return CF_OK;
+}
+}  // namespace
+
+extern "C" int cf_mppi_update_static(cf_sim *sim, const cf_mppi_params *mp, void *nominal_dev, void *plan_dev,
+                                     void *info_dev, int32_t *elite_idx_dev) {
+  int rc = check(sim, mp);
+  if (rc != CF_OK) return rc;
+  const size_t need = carve_scratch(sim->p.n_ctrl, mp->n_elite, mp->horizon).total;
+  if (need > CF_MPPI_STATIC_SCRATCH_BYTES)
+    return fail(CF_E_BUFFER, "cf_mppi_update_static: n_ctrl = %d, n_elite = %d, horizon = %d need %zu bytes of scratch, the "
+                "built-in array holds %zu; use cf_mppi_update with caller-owned scratch",
+                sim->p.n_ctrl, mp->n_elite, mp->horizon, need, (size_t)CF_MPPI_STATIC_SCRATCH_BYTES);
+  // the address is per device: the current device must be the one the simulator's planes live on
+  int dev = -1;
+  CF_CUDA(cudaGetDevice(&dev));
+  cudaPointerAttributes attr;
+  CF_CUDA(cudaPointerGetAttributes(&attr, sim->state));
+  if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+    return fail(CF_E_ARG, "cf_mppi_update_static: the simulator's workspace is not device memory");
+  if (attr.type == cudaMemoryTypeDevice && attr.device != dev)
+    return fail(CF_E_ARG, "cf_mppi_update_static: the simulator's workspace is on device %d but device %d is current",
+                attr.device, dev);
+  void *scratch = nullptr;
+  rc = static_scratch_addr(dev, &scratch);
+  if (rc != CF_OK) return rc;
+  // from here on this is cf_mppi_update on that memory: it zeroes the completion counter on the stream (the rest of the
+  // scratch is written before it is read, so the previous call's leftovers do no harm) and launches the same kernel
+  return cf_mppi_update(sim, mp, nominal_dev, plan_dev, info_dev, elite_idx_dev, scratch, CF_MPPI_STATIC_SCRATCH_BYTES);
 }
 
 extern "C" int cf_mppi_iterate(cf_sim *sim, const cf_mppi_params *mp, const float *x0_dev, void *nominal_dev,
