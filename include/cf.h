@@ -193,7 +193,12 @@ int cf_step_host(cf_sim *sim, const void *cmds_host, int n_cmds, int cmd_hold,
  *   x0_host [D] floats or NULL (keep the current state); cmds_host as cf_step_host; state_host [D][MN] floats;
  *   min_dist_host [MN] floats or NULL (needs obstacles and N = 1: the per-drone read-out of the rollout epilogue, else
  *   CF_E_UNSUPPORTED); staging_dev: cf_staging_bytes(sim, n_cmds, n_steps, 0) + 256 bytes, 256-byte aligned, caller-owned.
- * Host buffers should be pinned (pageable memory serialises the copies).  Synchronises both streams before returning. */
+ * Host buffers should be pinned (pageable memory serialises the copies).  Synchronises both streams before returning.
+ * The copy stream and up to 16 events are created on the first call and owned by the handle (cf_destroy releases them): this
+ * is the one place where the library holds CUDA objects of its own; they are internal to the call, which has drained both
+ * streams when it returns.  If a slice's launch or copy fails after an earlier slice has run, the planes hold a mixture of
+ * advanced and not-advanced drones: the call returns the error, drains both streams and leaves the simulator in the
+ * "no state" condition (CF_E_STATE from every stepping call) until cf_reset or cf_set_full(state, ...) gives it one again. */
 int cf_rollout_host(cf_sim *sim, const float *x0_host, const void *cmds_host, int n_cmds, int cmd_hold, int n_steps,
                     float *state_host, float *min_dist_host, void *staging_dev, size_t staging_bytes, int n_slices);
 

@@ -625,20 +625,36 @@ static int pick_block_rec(long long MN) {
   return 32 * best;
 }
 
+// Option bits of the instantiation that this simulator's configuration dispatches to in record mode rec_mode (-1: none).
+// A request without any fidelity extra still lands on the general OPT_ALL / REC_RUNTIME kernel when no lean instantiation
+// was built for it (e.g. the rotor or position interface of the first-principles model, RK4 on the abstracted model):
+// everything that depends on WHICH kernel runs -- block size, snapshots per store, the pair-written record modes -- is
+// decided from this, not from the request.
+static int dispatched_opt(const cf_sim *sim, int rec_mode) {
+  int opt_used = 0;
+  const bool found = sim->model == CF_MODEL_FIRST_PRINCIPLES
+      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true)
+      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
+  return found ? opt_used : -1;
+}
+static bool dispatches_lean(const cf_sim *sim, int rec_mode) {
+  const int o = dispatched_opt(sim, rec_mode);
+  return o >= 0 && !(o & OPT_EXTRAS);
+}
+
 static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name, int *grid, int *block) {
   LaunchCfg L;
   const int rec_mode = A ? A->rec_mode : sim->last_rec_mode;    // a dry run describes the kernel of the last cf_step
-  if (A) sim->last_rec_mode = A->rec_mode;
-  if (A) sim->last_rec_heavy = (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR || A->rec_mode == REC_TMA_P) && A->record_every <= 4 && !(sim->opt & OPT_EXTRAS);
-  L.block = sim->last_rec_heavy ? pick_block_rec(sim->MN) : pick_block(sim->MN);
-  L.grid = grid_for(A ? A->i_end - A->i_begin : sim->MN, L.block);
   // the kernel stages the parameter rows whenever ITS compile-time options carry OPT_RANDP and N > 1, and the
   // dispatcher may pick a superset instantiation: size the staging area from the instantiation, not from the request
-  int opt_used = 0;
-  bool found = sim->model == CF_MODEL_FIRST_PRINCIPLES
-      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true)
-      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
-  if (!found) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
+  const int opt_used = dispatched_opt(sim, rec_mode);
+  if (opt_used < 0) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
+  const bool general = (opt_used & OPT_EXTRAS) != 0;            // the OPT_ALL kernel: launch bound kMaxBlock
+  if (A) sim->last_rec_mode = A->rec_mode;
+  if (A) sim->last_rec_heavy = (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR || A->rec_mode == REC_TMA_P) && A->record_every <= 4 && !general;
+  L.block = sim->last_rec_heavy ? pick_block_rec(sim->MN) : pick_block(sim->MN);
+  if (general && L.block > kMaxBlock) L.block = kMaxBlock;
+  L.grid = grid_for(A ? A->i_end - A->i_begin : sim->MN, L.block);
   size_t smem_wp = ((opt_used & OPT_RANDP) && sim->N > 1) ? sizeof(float) * sim->P * (size_t)L.block : 0;
   size_t smem_rec = (A && (A->rec_mode == REC_TMA || A->rec_mode == REC_PAIR || A->rec_mode == REC_TMA_P)) ? kRecBufs * A->rec_group * sizeof(float) * sim->D * 32 * (size_t)(L.block / 32) : 0;
   L.smem = smem_wp > smem_rec ? smem_wp : smem_rec;
@@ -679,6 +695,16 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
     if (n_rec > 0 && (!record_dev || record_bytes < (size_t)n_rec * sim->D * (size_t)sim->MN * sizeof(float)))
       return fail(CF_E_BUFFER, "record buffer too small for %lld records", n_rec);
   }
+  // The pair-written kernels (REC_PAIR, REC_*_P) have "attitude tick in the first step of each pair" compiled in, which
+  // holds because THIS call starts at an even step (s0 below, the host mirror).  A launch captured into a CUDA graph is
+  // replayed from whatever the DEVICE counter holds then -- odd, if the graph's total length is odd -- so a call made
+  // during stream capture never takes a pair-written kernel: the run-time-scheduled ones are correct from any step.
+  bool capturing = false;
+  {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(sim->stream, &cs) == cudaSuccess) capturing = cs != cudaStreamCaptureStatusNone;
+    else (void)cudaGetLastError();
+  }
   StepArgs A;
   A.state = sim->state; A.ctrl = sim->ctrl; A.wparam = sim->wparam; A.min_d2 = sim->min_d2;
   A.bcast = sim->pending_bcast ? sim->bcast_buf : nullptr; A.md_drone = sim->md_drone;
@@ -697,7 +723,8 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
     // resident warps can have (two tiles of rec_group * D * 128 bytes per warp; <= 48 KB per block, <= 200 KB per SM with
     // at most 20 resident warps, the lean kernels' launch bound) and by the number of records of this call
     int group = 1;
-    if (record_every <= 4 && !(sim->opt & OPT_EXTRAS)) {
+    const bool lean_tma = dispatches_lean(sim, REC_TMA);        // grouped stores and the large blocks are the lean kernels'
+    if (record_every <= 4 && lean_tma) {
       const int block = pick_block_rec(sim->MN);
       const long long warps = (sim->MN + 31) / 32, bw = block / 32, blocks = (warps + bw - 1) / bw;
       long long resident = ((blocks + 147) / 148) * bw;                      // warps on the busiest SM
@@ -708,8 +735,8 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
     }
     // the pair schedule as a compile-time fact (REC_PAIR): every step recorded, two snapshots per store, attitude tick
     // every second step starting with this call's first, an even number of steps in command runs of even length
-    const bool pair = group >= 2 && record_every == 1 && sim->model == CF_MODEL_FIRST_PRINCIPLES &&
-        sim->p.iface == CF_IF_ATTITUDE && sim->p.integrator == CF_RK4 && !(sim->opt & OPT_EXTRAS) && sim->dp.att_div == 2 &&
+    const bool pair = !capturing && group >= 2 && record_every == 1 && sim->model == CF_MODEL_FIRST_PRINCIPLES &&
+        sim->p.iface == CF_IF_ATTITUDE && sim->p.integrator == CF_RK4 && dispatches_lean(sim, REC_PAIR) && sim->dp.att_div == 2 &&
         s0 % 2 == 0 && n_steps % 2 == 0 && cmd_hold != 1 && (cmd_hold % 2 == 0 || cmd_hold >= n_steps) && n_rec == n_steps;
     if (pair) group = 2;
     if (encode_record_map(&A.rec_map, record_dev, sim->MN, n_rec, sim->D, group) &&
@@ -723,25 +750,38 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
   // pair-written loops for the other record modes (REC_*_P, cf_device.cuh): nominal-plant first-principles kernels with
   // the attitude interface, tick period 2, an even number of steps from an even step in command runs of even length,
   // records never, every step, or with an even period
-  if (A.rec_mode != REC_PAIR && sim->model == CF_MODEL_FIRST_PRINCIPLES && sim->p.iface == CF_IF_ATTITUDE &&
+  if (!capturing && A.rec_mode != REC_PAIR && sim->model == CF_MODEL_FIRST_PRINCIPLES && sim->p.iface == CF_IF_ATTITUDE &&
       (sim->opt & ~OPT_RANDP) == 0 && sim->dp.att_div == 2 && s0 % 2 == 0 && n_steps % 2 == 0 && cmd_hold != 1 &&
-      (cmd_hold % 2 == 0 || cmd_hold >= n_steps) && (record_every <= 1 || record_every % 2 == 0))
-    A.rec_mode += REC_NONE_P;        // REC_NONE / REC_SCALAR / REC_TMA -> their _P forms
+      (cmd_hold % 2 == 0 || cmd_hold >= n_steps) && (record_every <= 1 || record_every % 2 == 0) &&
+      dispatches_lean(sim, A.rec_mode + REC_NONE_P))     // (a parameter-randomised plant has no _P instantiation: it runs
+    A.rec_mode += REC_NONE_P;        // REC_NONE / REC_SCALAR / REC_TMA -> their _P forms   the general kernel, base modes only)
   A.seed_lo = (uint32_t)(sim->seed & 0xFFFFFFFFu); A.seed_hi = (uint32_t)(sim->seed >> 32);
   for (int r = 0; r < 10; ++r) {      // Philox key schedule: k += (0x9E3779B9, 0xBB67AE85) per round
     A.rk[2 * r] = A.seed_lo + (uint32_t)r * 0x9E3779B9u;
     A.rk[2 * r + 1] = A.seed_hi + (uint32_t)r * 0xBB67AE85u;
   }
   if (slice <= 0 || slice >= sim->MN) slice = sim->MN;
+  bool launched = false;
   for (long long i0 = 0, k = 0; i0 < sim->MN; i0 += slice, ++k) {
     A.i_begin = (int)i0;
     A.i_end = (int)(i0 + slice < sim->MN ? i0 + slice : sim->MN);
     A.advance = A.i_end == sim->MN;
     A.ang_bound_ok = sim->wparam_foreign ? 0 : 1;
     int rc = do_launch(sim, &A, false, nullptr, nullptr, nullptr);
-    if (rc != CF_OK) return rc;
-    CF_CUDA(cudaGetLastError());
-    if (after_slice) { rc = after_slice(ctx, (int)k, A.i_begin, A.i_end); if (rc != CF_OK) return rc; }
+    if (rc == CF_OK) {
+      const cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) rc = fail(CF_E_CUDA, "rollout kernel launch: %s", cudaGetErrorString(e));
+    }
+    if (rc == CF_OK) {
+      launched = true;
+      if (after_slice) rc = after_slice(ctx, (int)k, A.i_begin, A.i_end);
+    }
+    if (rc != CF_OK) {
+      // earlier slices have advanced their drones (and consumed a pending broadcast) while the counters have not moved:
+      // the planes are a mixture of two steps.  The simulator refuses to continue from them (cf.h: cf_rollout_host).
+      if (launched) sim->have_state = false;
+      return rc;
+    }
   }
   sim->s_host = s0 + n_steps;
   sim->n_rec_host += n_rec;

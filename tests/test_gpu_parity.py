@@ -448,6 +448,72 @@ def test_general_kernel_fidelity_switches(cf, cfo, W):
         assert np.array_equal(g.counters(), o.counters())
 
 
+def test_general_kernel_at_sizes_where_the_lean_kernels_take_large_blocks(cf, cfo, W):
+    """Requests WITHOUT fidelity extras that have no lean instantiation (position / rotor interface of the first-principles
+    model, a randomised nominal plant, RK4 on the abstracted model) run the general kernel, whose launch bound is 128
+    threads: with every step recorded at >= 32768 drones the launcher must not hand it the 256 / 512-thread blocks, grouped
+    stores or pair-written record modes of the lean record-heavy kernels (decided from the dispatched kernel)."""
+    base = W.cfg2(seed=9, M=64, n_steps=6)
+    rng = np.random.default_rng(3)
+    M = 65536
+    pos = np.zeros((1, M, 4), dtype=np.float32)
+    pos[..., :3] = rng.uniform(-1, 1, (1, M, 3)) + [0, 0, 1]
+    pos[..., 3] = rng.uniform(-0.5, 0.5, (1, M))
+    rot = rng.uniform(12000, 17000, (1, M, 4)).astype(np.float32)
+    att = np.zeros((1, M, 4), dtype=np.float32)
+    att[..., :2] = rng.uniform(-0.2, 0.2, (1, M, 2))
+    att[..., 3] = 0.3
+    lo, hi = [1.0] * 12, [1.0] * 12
+    lo[0], hi[0], lo[4], hi[4] = 0.9, 1.1, 0.95, 1.05
+    cases = [(0, dict(base.params, iface=3), pos), (0, dict(base.params, iface=0, integrator=0), rot),
+             (0, dict(base.params, rnd_lo=lo, rnd_hi=hi), att),                     # OPT_RANDP only: was REC_TMA_P on the general kernel
+             (1, dict(integrator=1, f_phys=500.0, init_mode=1, p0_lo=[-1, -1, 0], p0_hi=[1, 1, 2], tilt0_max=0.4, iface=2), att)]
+    for model, prm, cmds in cases:
+        g = cf.Sim(M, 1, model, prm)
+        o = cfo.OracleSim(M, 1, model, prm)
+        g.reset(9), o.reset(9)
+        rg = g.step(cmds, 6, cmd_hold=6, record_every=1).cpu().numpy()
+        name, grid, block = g.describe_launch()
+        assert "OPT_ALL" in name and block <= 128, (name, block)
+        ro = o.step(cmds, 6, cmd_hold=6, record_every=1)
+        assert rg.shape == ro.shape == (6, g.D, M)
+        for k in (0, 5):
+            assert_state_close(rg[k], ro[k], model, 1e-4, f"{name} rec {k}")
+        assert np.array_equal(g.counters(), o.counters())
+        assert_state_close(g.get_state().cpu().numpy(), o.get_state(), model, 1e-4, name)
+
+
+def test_captured_graph_of_odd_length_never_replays_a_pair_written_kernel(cf, W):
+    """A graph [2 steps, 1 step] replayed 4 times starts its 2-step launch at steps 0, 3, 6, 9: the pair-written kernels
+    assume an even start, so a call made during stream capture must take the run-time-scheduled kernel."""
+    import torch
+    wl = W.cfg2(seed=6, M=256, n_steps=12)
+    a = fresh_gpu(cf, wl)
+    a.step(wl.cmds, 12, cmd_hold=12)
+    b = fresh_gpu(cf, wl)
+    cm = torch.from_numpy(wl.cmds).cuda()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        b.bind_stream(side)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            b.step(cm, 2, cmd_hold=2)
+            assert "_P" not in b.describe_launch()[0] and "REC_PAIR" not in b.describe_launch()[0]
+            b.step(cm, 1, cmd_hold=1)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(4):
+        graph.replay()
+    torch.cuda.synchronize()
+    b.bind_stream()
+    b.sync_counters()
+    assert b.step_counter == 12 and list(b.counters()) == list(a.counters())
+    np.testing.assert_allclose(b.get_state().cpu().numpy(), a.get_state().cpu().numpy(), rtol=1e-6, atol=1e-7)
+    c = fresh_gpu(cf, wl)                                  # outside capture the same call does take the pair-written kernel
+    c.step(cm, 2, cmd_hold=2)
+    assert "_P" in c.describe_launch()[0]
+
+
 # ------------------------------------------------------------------------------------------------ full BASELINE sizes
 def _oracle_slice(cfo, wl, w0, m):
     """The oracle on worlds [w0, w0+m) of the full workload (Philox is keyed by the global world index)."""
