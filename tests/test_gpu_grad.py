@@ -2,9 +2,10 @@
 dynamics and controller stack) against oracle/grad.py, the Richardson-extrapolated central difference of the float64 step.
 
 Tolerance (floating point; north_star states none for gradients, derived in DESIGN.md "Arithmetic and tolerances"): per
-drone |g_gpu - g_oracle| <= 1e-3 * max_k,j |g_oracle| + 1e-9 -- the float32 adjoint carries the 1e-7 rounding of ~10^3
-operations per step and the MUFU approximations of the forward step, the oracle's own rounding floor is 1e-11; measured
-worst 3e-5.  The loss itself is held to the state tolerance 1e-4.
+entry |g_gpu - g_oracle| <= 1e-3 |g_oracle| + 1e-4 * max_k,j |g_oracle of that drone| + 1e-9 -- the float32 adjoint
+carries the 1e-7 rounding of ~10^3 operations per step and the MUFU approximations of the forward step, proportional to
+the drone's dominant entry (measured worst 4.6e-5 of it); the oracle's own rounding floor is 1e-11.  The loss itself is
+held to the state tolerance 1e-4.
 """
 import numpy as np
 import pytest
@@ -49,11 +50,21 @@ def att_cmds(K, M, seed, amp=0.2):
     return c
 
 
-def compare(g_gpu, L_gpu, L_o, g_o, tol=1e-3):
-    scale = np.abs(g_o).max(axis=(0, 2))                          # per drone
-    err = np.abs(g_gpu.astype(np.float64) - g_o).max(axis=(0, 2))
-    worst = (err / (scale + 1e-30)).max()
-    assert (err <= tol * scale + 1e-9).all(), f"worst relative gradient error {worst:.2e}"
+def compare(g_gpu, L_gpu, L_o, g_o, tol=1e-3, floor=1e-4):
+    """Per ENTRY (knot k, drone i, channel j):  |g_gpu - g_o| <= tol |g_o[k,i,j]| + floor max_kj |g_o[.,i,.]| + 1e-9.
+    The relative part holds every entry to 1e-3 of ITSELF; the floor is the float32 rounding of the adjoint, which is
+    proportional to the drone's dominant entry whatever the size of the entry it lands on (measured over all cases of
+    this file and test_gpu_r3.py: <= 4.6e-5 of the dominant entry; a pure per-entry bound with the floor at 1e-3 of the
+    dominant entry reads 3e-2 on three cases for that reason alone).  Until round 3 the bound was tol x the dominant entry
+    for all entries, which let a channel 10^3 x smaller than the dominant one be entirely wrong; now an
+    entry larger than 1e-4 of the dominant one that is 100 % wrong fails."""
+    scale = np.abs(g_o).max(axis=(0, 2))                          # per drone: its dominant entry
+    err_e = np.abs(g_gpu.astype(np.float64) - g_o)
+    bound = tol * np.abs(g_o) + floor * scale[None, :, None] + 1e-9
+    worst = (err_e.max(axis=(0, 2)) / (scale + 1e-30)).max()
+    k, i, j = np.unravel_index(np.argmax(err_e - bound), err_e.shape)
+    assert (err_e <= bound).all(), (f"knot {k} drone {i} channel {j}: gpu {g_gpu[k, i, j]:.6e} oracle {g_o[k, i, j]:.6e} "
+                                    f"(dominant entry of the drone {scale[i]:.3e}); worst error / dominant entry {worst:.2e}")
     assert (np.abs(L_gpu - L_o) <= 1e-4 * np.maximum(L_o, 1.0)).all()
     return worst
 
