@@ -32,7 +32,26 @@ DEFAULT_WORKLOAD = "cfg3"
 ALGO_FLOPS = {"depth": 4096 * 555,      # per frame: 64 x 64 rays x (16 spheres x 14 + 16 boxes x 19 + plane, direction 27)
                "grad": 2120, "mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
 BOUND = {"depth": "alu", "grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
-SM_COUNT, FP32_LANES = 148, 128
+FP32_LANES = 128          # FP32 lanes per SM (sm_100: 4 sub-partitions x 32)
+
+
+def device_units():
+    """(SM count, max SM clock in MHz) of cuda:<LOCAL_RANK> from the driver (NVML through nvidia-smi for the clock, torch
+    for the SM count); None where the query fails -- peaks() then says that it fell back to the B200 data-sheet values."""
+    sms = mhz = None
+    try:
+        import torch
+        if torch.cuda.is_available():
+            sms = int(torch.cuda.get_device_properties(int(os.environ.get("LOCAL_RANK", "0"))).multi_processor_count)
+    except Exception:
+        pass
+    try:
+        out = subprocess.run(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i",
+                              os.environ.get("LOCAL_RANK", "0")], capture_output=True, text=True, timeout=20).stdout
+        mhz = float(out.strip().splitlines()[0])
+    except Exception:
+        pass
+    return sms, mhz
 
 
 def ncu_static():
@@ -47,16 +66,24 @@ def ncu_static():
 
 def peaks():
     """Roofline denominators: measured HBM copy bandwidth from MEASURED_PEAKS.json (else the guide's fallback);
-    FP32 ALU peak derived from unit counts and the max SM clock: 148 SMs x 128 lanes x 2 flop x f_max."""
+    FP32 ALU peak derived from unit counts and the max SM clock: SMs x 128 lanes x 2 flop x f_max, with the SM
+    count and f_max read from the device (f_max: MEASURED_PEAKS.json's if it has one)."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    src, hbm, mhz = "fallback", 6650.0, 1965.0
+    src, hbm, mhz_file = "fallback", 6650.0, None
     if os.path.exists(path):
         try:
             d = json.load(open(path))
-            hbm, mhz, src = float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+            hbm, src = float(d["hbm_gbs"]), "measured"
+            mhz_file = float(d["sm_max_mhz"]) if "sm_max_mhz" in d else None
         except Exception:
             pass
-    return dict(hbm_gbs=hbm, fp32_tflops=SM_COUNT * FP32_LANES * 2 * mhz * 1e6 / 1e12, sm_max_mhz=mhz, source=src)
+    sms_dev, mhz_dev = device_units()
+    sms = sms_dev or 148
+    mhz = mhz_file or mhz_dev or 1965.0
+    units = (f"{sms} SMs ({'device query' if sms_dev else 'B200 data sheet'}) x {FP32_LANES} lanes x 2 x {mhz:.0f} MHz "
+             f"({'MEASURED_PEAKS.json' if mhz_file else 'nvidia-smi clocks.max.sm' if mhz_dev else 'B200 data sheet'})")
+    return dict(hbm_gbs=hbm, fp32_tflops=sms * FP32_LANES * 2 * mhz * 1e6 / 1e12, sm_max_mhz=mhz, source=src, sm_count=sms,
+                alu_peak_source=units)
 
 
 def algo_bytes_per_launch(wl) -> int:
@@ -417,7 +444,7 @@ def oracle_sample(name, target_seconds=12.0, threads=None):
         scale = max(1.0, rate * target_seconds / (small.get("M", 1) * small.get("N", 1) * small["n_steps"]))
         kw["M"] = int(min(small["M"] * scale, {"cfg4": 256}.get(name, 1 << 22)))
     rate, wl = run(kw)
-    sample = f"{wl.M} worlds x {wl.N} drones x {wl.n_steps} steps of {name} (same recipe, reduced M)"
+    sample = f"{wl.M} worlds x {wl.N} drones x {wl.n_steps} steps of {name} (same recipe; a sample of M worlds sized for ~{target_seconds:.0f} s of CPU work)"
     return rate, cfo.num_threads(), sample, wl
 
 
@@ -569,7 +596,11 @@ def main():
         else:
             ach = ALGO_FLOPS[nm] * wl.drone_steps / (k_ms * 1e-3) / 1e12
             roof = dict(bound="alu", achieved=ach, peak=pk["fp32_tflops"], unit="TFLOP/s", frac=ach / pk["fp32_tflops"],
-                        traffic=None, peak_source=f"148 SM x 128 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz")
+                        traffic=None, peak_source=pk["alu_peak_source"])
+        if nm == "depth":       # the count is dense (every ray x every primitive) while the kernel culls per tile: not work done
+            roof["basis"] = ("dense-equivalent: ALGO_FLOPS counts every ray against every primitive; the kernel skips the "
+                             "primitives its tile's cone misses, so frac is a speed-up-inclusive figure -- the executed work "
+                             "is ncu_static.sass_flop_frac of peak")
         st = ncu_static()
         sw = st.get("workloads", {}).get(nm, {})
         roof["traffic"] = sw.get("dram_bytes")                      # static, from the tracked ncu capture (see ncu_static)

@@ -601,9 +601,22 @@ static bool encode_record_map(CUtensorMap *map, float *record_dev, long long MN,
 }
 
 // launch geometry.  One wave always suffices for the paper's sizes up to ~600k drones (64 warps/SM x 148 SMs), so the
-// block size only decides how evenly the warps spread over the 148 SMs: the fewer warps per SM, the smaller the block.
+// block size only decides how evenly the warps spread over the SMs: the fewer warps per SM, the smaller the block.
+// SM count of the current device, asked once (148 on a B200; the same value if the query fails, e.g. without a device)
+static long long sm_count() {
+  static const long long n = []() -> long long {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        sms < 1) {
+      (void)cudaGetLastError();
+      return 148;
+    }
+    return sms;
+  }();
+  return n;
+}
 static int pick_block(long long MN) {
-  const long long sms = 148, warps = (MN + 31) / 32;
+  const long long sms = sm_count(), warps = (MN + 31) / 32;
   if (warps <= sms * 16) return 32;
   if (warps <= sms * 32) return 64;
   return kMaxBlock;
@@ -614,7 +627,7 @@ static int pick_block(long long MN) {
 // measured with a write-only kernel of the same pattern (profiles/r2_record_pattern.md): 4.75 TB/s at 32 threads per
 // block, 5.0 at 128, 5.4 at 256, 6.1 - 6.7 at 512 (a linear fill: 6.9).
 static int pick_block_rec(long long MN) {
-  const long long sms = 148, warps = (MN + 31) / 32;
+  const long long sms = sm_count(), warps = (MN + 31) / 32;
   auto busiest = [&](long long b) {            // warps on the busiest scheduler with blocks of b warps
     const long long blocks = (warps + b - 1) / b, per_sm = (blocks + sms - 1) / sms;
     return (per_sm * b + 3) / 4;
@@ -727,7 +740,7 @@ static int step_launch(cf_sim *sim, const void *cmds_dev, int n_cmds, int cmd_ho
     if (record_every <= 4 && lean_tma) {
       const int block = pick_block_rec(sim->MN);
       const long long warps = (sim->MN + 31) / 32, bw = block / 32, blocks = (warps + bw - 1) / bw;
-      long long resident = ((blocks + 147) / 148) * bw;                      // warps on the busiest SM
+      long long resident = ((blocks + sm_count() - 1) / sm_count()) * bw;    // warps on the busiest SM
       if (resident > 20) resident = 20;
       const size_t tile = sizeof(float) * sim->D * 32;
       for (int g = kRecGroupMax; g > 1 && group == 1; --g)
