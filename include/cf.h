@@ -10,7 +10,8 @@
  *  - Every function returns CF_OK (0) or a negative cf_status; none throws, aborts or prints.  cf_last_error()
  *    returns a thread-local description of the last failure.
  *  - Ownership: the CALLER owns every device byte (workspace, commands, records, outputs).  The library owns only
- *    the host handle and never allocates device memory.  Pointers named *_dev are device pointers, *_host are host
+ *    the host handle and never allocates device memory (one exception to "only the host handle": cf_rollout_host
+ *    creates a second stream and up to 16 events on first use, see there and cf_set_copy_stream).  Pointers named *_dev are device pointers, *_host are host
  *    pointers (pinned memory makes the copies asynchronous to the host but the *_host calls still synchronise the
  *    stream before returning).
  *  - Asynchrony: all *_dev calls enqueue on the bound CUDA stream (cf_set_stream, default stream 0) and return; there
@@ -72,7 +73,10 @@ enum { CF_AUX_COUNTERS = 0,      /* uint32[4]: s, attitude ticks, position ticks
        CF_AUX_COST = 6,          /* float[MN]: rollout cost J (R27): running + terminal + clearance + collision */
        CF_AUX_EPS = 7,           /* float[4][MN]: AR(1) noise state; NaN = nothing drawn since the last re-arm
                                     (kept only when noise_beta != 0) */
-       CF_AUX_COST_RUN = 8 };    /* float[MN]: running part of the cost only */
+       CF_AUX_COST_RUN = 8,      /* float[MN]: running part of the cost only */
+       CF_AUX_NONFINITE = 9 };   /* uint32[2]: number of drones whose state holds a NaN / Inf, index of the first one
+                                    (0xFFFFFFFF if none) -- a debug read-out computed on demand by its own small kernel,
+                                    nothing is added to the rollout kernels */
 #define CF_REC_TABLE_CAP 4096
 #define CF_MAX_OBSTACLES 8
 
@@ -142,6 +146,12 @@ int cf_destroy(cf_sim *sim);
 
 /* Bind the CUDA stream (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) all later calls enqueue on. */
 int cf_set_stream(cf_sim *sim, void *cuda_stream);
+/* The second stream cf_rollout_host queues its device->host result copies on.  By default the handle creates one of its
+ * own on the first cf_rollout_host call; a caller that wants to own it (to give it a priority, or to order other work
+ * against the copies) passes its stream here.  NULL returns to the library-owned stream.  The caller's stream must
+ * outlive the handle or be replaced before it is destroyed; it must differ from the cf_set_stream stream for the copies
+ * to overlap the next slice's kernel. */
+int cf_set_copy_stream(cf_sim *sim, void *cuda_stream);
 
 /* Draw the per-world parameters (Philox PARAM stream) and the initial state (INIT stream) from `seed`, zero the
  * controller integrals, set the held commands to hover, re-arm the minimum distance, s = 0.  (C9) */
@@ -163,6 +173,16 @@ int cf_set_state(cf_sim *sim, const float *state_dev, int broadcast);
  * min_d2 [8][MN] (NULL = keep) and, if step_counter >= 0, the global step counter. */
 int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctrl_dev, const float *wparam_dev,
                 const float *min_d2_dev, int64_t step_counter);
+
+/* Checkpoint restore of the counters cf_set_full leaves alone.  counters_host: the four words of CF_AUX_COUNTERS (step
+ * counter s, attitude ticks, position ticks, records written) on the HOST; rec_table_dev: CF_REC_TABLE_CAP words as read
+ * with CF_AUX_REC_TABLE, on the device, or NULL to keep the table.  Also sets the host mirror of s (cf_step_counter).
+ * A COMPLETE CHECKPOINT of a simulator is: the seed given to cf_reset, cf_get_state, CF_AUX_CTRL, CF_AUX_WORLD_PARAMS,
+ * CF_AUX_MIN_D2 (with obstacles), CF_AUX_EPS / CF_AUX_COST_RUN (planning rollouts), CF_AUX_COUNTERS, CF_AUX_REC_TABLE.
+ * RESTORE into a simulator created with the same (M, N, model, params): cf_reset(seed); cf_set_full(state, ctrl, wparam,
+ * min_d2, -1); cf_set_plan_state(eps, cost_run) where applicable; cf_set_counters(counters, rec_table).  The run then
+ * continues bit for bit as the uninterrupted one would (tests/test_gpu_r3.py). */
+int cf_set_counters(cf_sim *sim, const uint32_t counters_host[4], const uint32_t *rec_table_dev);
 
 /* Teacher forcing / checkpoint restore of the planning-rollout state: eps [4][MN] (needs noise_beta != 0) and the
  * running cost [MN] (needs cost_on); NULL = keep. */

@@ -17,7 +17,7 @@ MODEL_FP, MODEL_AB = 0, 1
 EULER, RK4 = 0, 1
 IF_ROTOR, IF_TORQUE, IF_ATTITUDE, IF_POSITION = 0, 1, 2, 3
 CMD_BUFFER, CMD_NOMINAL_PLUS_NOISE = 0, 1
-AUX_COUNTERS, AUX_MIN_DIST, AUX_CTRL, AUX_WORLD_PARAMS, AUX_REC_TABLE, AUX_MIN_D2, AUX_COST, AUX_EPS, AUX_COST_RUN = range(9)
+AUX_COUNTERS, AUX_MIN_DIST, AUX_CTRL, AUX_WORLD_PARAMS, AUX_REC_TABLE, AUX_MIN_D2, AUX_COST, AUX_EPS, AUX_COST_RUN, AUX_NONFINITE = range(10)
 REC_TABLE_CAP = 4096
 OK, E_ARG, E_SHAPE, E_STATE, E_BUFFER, E_CUDA, E_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
@@ -112,6 +112,8 @@ def lib():
         "cf_set_plan_state": (C.c_int, [vp, vp, vp]),
         "cf_mppi_scratch_bytes": (sz, [vp, C.POINTER(MppiParams)]),
         "cf_mppi_update": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, sz]),
+        "cf_set_counters": (C.c_int, [vp, C.POINTER(C.c_uint32 * 4), vp]),
+        "cf_set_copy_stream": (C.c_int, [vp, vp]),
         "cf_mppi_update_static": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp]),
         "cf_mppi_iterate": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, sz]),
         "cf_mppi_iterate_host": (C.c_int, [vp, C.POINTER(MppiParams), vp, vp, vp, vp, vp, vp, vp, sz]),
@@ -140,7 +142,8 @@ EXPORTS = ["cf_default_params", "cf_state_dim", "cf_world_param_dim", "cf_worksp
            "cf_describe_launch", "cf_last_error", "cf_debug_philox", "cf_debug_philox_dev", "cf_set_plan_state",
            "cf_mppi_scratch_bytes", "cf_mppi_update", "cf_mppi_iterate", "cf_mppi_iterate_host", "cf_grad_scratch_bytes",
            "cf_grad", "cf_depth", "cf_reset_masked", "cf_grad_staging_bytes", "cf_grad_host", "cf_depth_host",
-           "cf_mppi_pack_best", "cf_mppi_select", "cf_rollout_host", "cf_mppi_update_static"]
+           "cf_mppi_pack_best", "cf_mppi_select", "cf_rollout_host", "cf_mppi_update_static",
+           "cf_set_counters", "cf_set_copy_stream"]
 
 
 def _check(rc: int):
@@ -537,6 +540,26 @@ class Sim:
                                           C.c_void_p(plan_host.data_ptr()), C.c_void_p(info_host.data_ptr()),
                                           _dptr(self._mppi_plan), _dptr(self._mppi_info), sp, need))
         return plan_host, info_host
+
+    def nonfinite(self):
+        """(number of drones with a NaN / Inf in their state, index of the first one or None) -- CF_AUX_NONFINITE."""
+        w = self._aux(AUX_NONFINITE, (2,), _torch().int32).cpu().numpy().view(np.uint32)
+        return int(w[0]), (None if w[1] == 0xFFFFFFFF else int(w[1]))
+
+    def set_counters(self, counters, rec_table=None):
+        """cf_set_counters: counters = the 4 words of counters(); rec_table = rec_table() (numpy / tensor) or None."""
+        c = (C.c_uint32 * 4)(*[int(v) for v in counters])
+        t = None
+        if rec_table is not None:
+            t = self._dev(np.asarray(rec_table).view(np.int32) if not isinstance(rec_table, _torch().Tensor) else rec_table,
+                          _torch().int32)
+            assert t.numel() == REC_TABLE_CAP
+        _check(lib().cf_set_counters(self._h, C.byref(c), _dptr(t)))
+
+    def set_copy_stream(self, stream=None):
+        """cf_set_copy_stream: a torch.cuda.Stream the caller owns (kept alive here), or None for the library's own."""
+        self._copy_stream = stream
+        _check(lib().cf_set_copy_stream(self._h, C.c_void_p(stream.cuda_stream) if stream is not None else None))
 
     def rec_table(self):
         return self._aux(AUX_REC_TABLE, (REC_TABLE_CAP,), _torch().int32).cpu().numpy().view(np.uint32)

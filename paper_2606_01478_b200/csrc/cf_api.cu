@@ -325,6 +325,25 @@ __global__ void set_counters_kernel(Counters *c, uint32_t s, int zero_rest) {
   c->blocks_done = 0;
 }
 
+__global__ void set_counters4_kernel(Counters *c, uint32_t s, uint32_t att, uint32_t pos, uint32_t n_rec) {
+  c->s = s; c->att_ticks = att; c->pos_ticks = pos; c->n_rec_total = n_rec;
+  c->blocks_done = 0;
+}
+
+// CF_AUX_NONFINITE: out[0] = number of drones with a NaN / Inf in any state component, out[1] = the first such drone
+__global__ void nonfinite_init_kernel(uint32_t *out) { out[0] = 0u; out[1] = 0xFFFFFFFFu; }
+__global__ void nonfinite_kernel(const float *state, int D, long long MN, uint32_t *out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = false;
+  if (i < MN)
+    for (int d = 0; d < D; ++d) bad |= !isfinite(state[(long long)d * MN + i]);
+  const unsigned m = __ballot_sync(0xffffffffu, bad);
+  if (m && (threadIdx.x & 31) == 0) {
+    atomicAdd(out, (uint32_t)__popc(m));
+    atomicMin(out + 1, (uint32_t)(i + __ffs(m) - 1));
+  }
+}
+
 // C10: per world, min over drones, obstacles (and, through min_d2, steps) of |p - c_j| - r_j.  One warp per world.
 __global__ void min_dist_kernel(const float *min_d2, float *out, long long M, long long N, long long MN,
                                 const __grid_constant__ DevParams P) {
@@ -432,7 +451,7 @@ extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf
 extern "C" int cf_destroy(cf_sim *sim) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
   for (cudaEvent_t e : sim->slice_ev) if (e) cudaEventDestroy(e);
-  if (sim->copy_stream) cudaStreamDestroy(sim->copy_stream);
+  if (sim->copy_stream && sim->copy_stream_owned) cudaStreamDestroy(sim->copy_stream);
   delete sim;
   return CF_OK;
 }
@@ -440,6 +459,14 @@ extern "C" int cf_destroy(cf_sim *sim) {
 extern "C" int cf_set_stream(cf_sim *sim, void *cuda_stream) {
   if (!sim) return fail(CF_E_ARG, "sim is NULL");
   sim->stream = (cudaStream_t)cuda_stream;
+  return CF_OK;
+}
+
+extern "C" int cf_set_copy_stream(cf_sim *sim, void *cuda_stream) {
+  if (!sim) return fail(CF_E_ARG, "sim is NULL");
+  if (sim->copy_stream && sim->copy_stream_owned) CF_CUDA(cudaStreamDestroy(sim->copy_stream));
+  sim->copy_stream = (cudaStream_t)cuda_stream;      // NULL: cf_rollout_host creates its own on the next call
+  sim->copy_stream_owned = false;
   return CF_OK;
 }
 
@@ -567,6 +594,20 @@ extern "C" int cf_set_full(cf_sim *sim, const float *state_dev, const float *ctr
     sim->s_host = step_counter;
   }
   sim->have_state = true;
+  return CF_OK;
+}
+
+// Checkpoint restore of what cf_set_full leaves out: the tick / record counters and the record-slot table.
+extern "C" int cf_set_counters(cf_sim *sim, const uint32_t counters_host[4], const uint32_t *rec_table_dev) {
+  if (!sim || !counters_host) return fail(CF_E_ARG, "NULL argument");
+  if (!sim->have_state) return fail(CF_E_STATE, "cf_set_counters before cf_reset");
+  set_counters4_kernel<<<1, 1, 0, sim->stream>>>(sim->counters, counters_host[0], counters_host[1], counters_host[2],
+                                                 counters_host[3]);
+  CF_CUDA(cudaGetLastError());
+  if (rec_table_dev)
+    CF_CUDA(cudaMemcpyAsync(sim->rec_table, rec_table_dev, sizeof(uint32_t) * kRecTableCap, cudaMemcpyDeviceToDevice, sim->stream));
+  sim->s_host = counters_host[0];
+  sim->n_rec_host = counters_host[3];
   return CF_OK;
 }
 
@@ -877,7 +918,10 @@ extern "C" int cf_rollout_host(cf_sim *sim, const float *x0_host, const void *cm
   if (((uintptr_t)staging_dev & 255) != 0) return fail(CF_E_BUFFER, "staging must be 256-byte aligned");
   const size_t cb = cmd_bytes(sim, n_cmds), xb = align256(sizeof(float) * sim->D);
   if (staging_bytes < cb + xb) return fail(CF_E_BUFFER, "staging too small: %zu < %zu", staging_bytes, cb + xb);
-  if (!sim->copy_stream) CF_CUDA(cudaStreamCreateWithFlags(&sim->copy_stream, cudaStreamNonBlocking));
+  if (!sim->copy_stream) {
+    CF_CUDA(cudaStreamCreateWithFlags(&sim->copy_stream, cudaStreamNonBlocking));
+    sim->copy_stream_owned = true;
+  }
   for (int k = 0; k < n_slices; ++k)
     if (!sim->slice_ev[k]) CF_CUDA(cudaEventCreateWithFlags(&sim->slice_ev[k], cudaEventDisableTiming));
   const size_t per = sim->p.cmd_source == CF_CMD_NOMINAL_PLUS_NOISE ? (size_t)sim->p.n_ctrl : (size_t)sim->MN;
@@ -970,9 +1014,18 @@ static int launch_min_dist(cf_sim *sim, float *out_dev) {
   return CF_OK;
 }
 
+static int launch_nonfinite(cf_sim *sim, uint32_t *out_dev) {
+  { int rc = materialise(sim); if (rc != CF_OK) return rc; }
+  nonfinite_init_kernel<<<1, 1, 0, sim->stream>>>(out_dev);
+  nonfinite_kernel<<<grid_for(sim->MN, 256), 256, 0, sim->stream>>>(sim->state, sim->D, sim->MN, out_dev);
+  CF_CUDA(cudaGetLastError());
+  return CF_OK;
+}
+
 extern "C" int cf_get_aux(cf_sim *sim, int which, void *out_dev) {
   if (!sim || !out_dev) return fail(CF_E_ARG, "NULL argument");
   if (which == CF_AUX_MIN_DIST) return launch_min_dist(sim, (float *)out_dev);
+  if (which == CF_AUX_NONFINITE) return launch_nonfinite(sim, (uint32_t *)out_dev);
   const void *src; size_t bytes;
   int rc = aux_source(sim, which, &src, &bytes);
   if (rc != CF_OK) return rc;
@@ -987,6 +1040,12 @@ extern "C" int cf_get_aux_host(cf_sim *sim, int which, void *out_host, void *scr
     bytes = sizeof(float) * (size_t)sim->M;
     if (!scratch_dev || scratch_bytes < bytes) return fail(CF_E_BUFFER, "scratch_dev must hold M floats");
     int rc = launch_min_dist(sim, (float *)scratch_dev);
+    if (rc != CF_OK) return rc;
+    src = scratch_dev;
+  } else if (which == CF_AUX_NONFINITE) {
+    bytes = 2 * sizeof(uint32_t);
+    if (!scratch_dev || scratch_bytes < bytes || ((uintptr_t)scratch_dev & 3)) return fail(CF_E_BUFFER, "scratch_dev must hold 2 uint32");
+    int rc = launch_nonfinite(sim, (uint32_t *)scratch_dev);
     if (rc != CF_OK) return rc;
     src = scratch_dev;
   } else {

@@ -208,3 +208,82 @@ def test_full_size_cfg4_every_world_every_record(cf, cfo, W):
     print(f"cfg4 full size, every world and record: worst position drift {worst_p:.2e} m, worst relative error {worst:.2e}")
     del rg, g
     torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------------------------------------ checkpoint / resume
+@pytest.mark.parametrize("name,kw,cut", [("cfg5", dict(M=300, n_steps=60), 23), ("cfg4", dict(M=3, N=333, n_steps=60), 31),
+                                         ("cfg3", dict(M=700, n_steps=60), 17)])
+def test_checkpoint_at_an_odd_step_restored_into_a_fresh_simulator_continues_bit_for_bit(cf, W, name, kw, cut):
+    """SURVEY.md section 5 / cf.h "A COMPLETE CHECKPOINT": run `cut` steps, read everything out, restore into a NEW
+    simulator, run the rest; states, records, controller planes, obstacle minima, counters and the record-slot table equal
+    those of the uninterrupted run bit for bit (randomised plant + Philox disturbances; position controller with integrals;
+    planning rollout with its AR(1) noise state, running cost and obstacle minima)."""
+    from util import split_calls
+    wl = W.make(name, seed=12, **kw)
+    rec = 3
+    (cm1, n1, h1), (cm2, n2, h2) = split_calls(wl, [cut, wl.n_steps])      # the same two cf_step calls on both sides
+    assert n1 == cut and n1 + n2 == wl.n_steps
+    a = fresh_gpu(cf, wl)                                          # uninterrupted: the two calls back to back on one simulator
+    ra = np.concatenate([a.step(cm1, n1, cmd_hold=h1, record_every=rec).cpu().numpy(),
+                         a.step(cm2, n2, cmd_hold=h2, record_every=rec).cpu().numpy()])
+    b = fresh_gpu(cf, wl)
+    rb1 = b.step(cm1, n1, cmd_hold=h1, record_every=rec)
+    ck = dict(state=b.get_state().clone(), ctrl=b.ctrl(), wparam=b.world_params(), counters=b.counters(), table=b.rec_table(),
+              min_d2=b.min_d2() if wl.params.get("n_obstacles") else None,
+              eps=b.eps() if wl.params.get("noise_beta") else None, cost_run=b.cost_run() if wl.params.get("cost_on") else None)
+    assert ck["counters"][0] == cut
+    del b
+    c = cf.Sim(wl.M, wl.N, wl.model, wl.params)
+    c.reset(wl.seed)                                               # the seed of the disturbance / noise streams
+    c.set_full(state=ck["state"], ctrl=ck["ctrl"], wparam=ck["wparam"], min_d2=ck["min_d2"])
+    if ck["eps"] is not None or ck["cost_run"] is not None:
+        c.set_plan_state(eps=ck["eps"], cost_run=ck["cost_run"])
+    c.set_counters(ck["counters"], ck["table"])
+    assert c.step_counter == cut and np.array_equal(c.counters(), ck["counters"])
+    rc2 = c.step(cm2, n2, cmd_hold=h2, record_every=rec)
+    assert np.array_equal(np.concatenate([rb1.cpu().numpy(), rc2.cpu().numpy()]).view(np.uint32), ra.view(np.uint32))
+    assert np.array_equal(c.get_state().cpu().numpy().view(np.uint32), a.get_state().cpu().numpy().view(np.uint32))
+    assert np.array_equal(c.ctrl().cpu().numpy().view(np.uint32), a.ctrl().cpu().numpy().view(np.uint32))
+    assert np.array_equal(c.counters(), a.counters()) and np.array_equal(c.rec_table(), a.rec_table())
+    assert c.counters()[3] == wl.n_steps // rec
+    if wl.params.get("n_obstacles"):
+        assert np.array_equal(c.min_d2().cpu().numpy(), a.min_d2().cpu().numpy())
+        assert np.array_equal(c.min_dist().cpu().numpy(), a.min_dist().cpu().numpy())
+    if wl.params.get("cost_on"):
+        assert np.array_equal(c.cost().cpu().numpy(), a.cost().cpu().numpy())
+
+
+def test_nonfinite_debug_counter(cf, W):
+    wl = W.cfg2(seed=3, M=1000, n_steps=10)
+    g = fresh_gpu(cf, wl)
+    g.step(wl.cmds, 10, cmd_hold=wl.cmd_hold)
+    assert g.nonfinite() == (0, None)
+    x = g.get_state().clone()
+    x[9, 713] = float("nan"); x[0, 40] = float("inf"); x[16, 999] = float("-inf"); x[3, 40] = float("nan")
+    g.set_full(state=x)
+    assert g.nonfinite() == (3, 40)
+
+
+def test_rollout_host_on_a_caller_owned_copy_stream(cf, W):
+    """cf_set_copy_stream: the result copies of cf_rollout_host run on the caller's stream; same bits as on the library's."""
+    import torch
+    wl = W.cfg3(seed=9, M=5000, n_steps=20)
+    cm = torch.from_numpy(np.ascontiguousarray(wl.cmds)).pin_memory()
+    x0 = torch.from_numpy(wl.broadcast_state.astype(np.float32)).pin_memory()
+    outs = []
+    mine = torch.cuda.Stream()
+    for stream in (None, mine, None):
+        sim = cf.Sim(wl.M, 1, wl.model, wl.params)
+        sim.reset(wl.seed)
+        if stream is not None:
+            sim.set_copy_stream(stream)
+        st = torch.empty((wl.D, wl.M), dtype=torch.float32).pin_memory()
+        md = torch.empty(wl.M, dtype=torch.float32).pin_memory()
+        sim.rollout_host(cm, 20, st, cmd_hold=wl.cmd_hold, min_dist_host=md, x0_host=x0, n_slices=4)
+        if stream is not None:
+            sim.set_copy_stream(None)                              # back to a library-owned stream: created on the next call
+            st2 = torch.empty_like(st).pin_memory()
+            sim.rollout_host(cm, 20, st2, cmd_hold=wl.cmd_hold, x0_host=x0, n_slices=3)
+        outs.append((st.numpy().copy(), md.numpy().copy()))
+    for s, m in outs[1:]:
+        assert np.array_equal(s, outs[0][0]) and np.array_equal(m, outs[0][1])
