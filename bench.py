@@ -30,9 +30,15 @@ DEFAULT_WORKLOAD = "cfg3"
 # trig / log / min / max / clip of the float64 oracle's formulas counts 1 (an FMA is 2); Philox integer work is not
 # counted.  Controller ticks are amortised over their period.
 ALGO_FLOPS = {"depth": 4096 * 555,      # per frame: 64 x 64 rays x (16 spheres x 14 + 16 boxes x 19 + plane, direction 27)
+               "fp_pos": 720, "fp_rotor": 610, "ab_rk4": 330,      # estimates (cfg2's 689 +- the controller ticks; 4 x Eqs. (7)-(10) + RK4 combine)
                "grad": 2120, "mppi": 161, "cfg1": 214, "cfg2": 689, "cfg3": 182, "cfg3b": 138, "cfg4": 87, "cfg5": 744, "cfg5e": 251}
-BOUND = {"depth": "alu", "grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
+BOUND = {"fp_pos": "alu", "fp_rotor": "alu", "ab_rk4": "alu", "depth": "alu", "grad": "alu", "mppi": "alu", "cfg1": "alu", "cfg2": "alu", "cfg3": "alu", "cfg3b": "alu", "cfg4": "alu", "cfg5": "alu", "cfg5e": "hbm"}
 FP32_LANES = 128          # FP32 lanes per SM (sm_100: 4 sub-partitions x 32)
+
+
+def under_torchrun() -> bool:
+    """Launched by torch.distributed.run (also with a single rank): rendezvous variables are in the environment."""
+    return all(k in os.environ for k in ("RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT"))
 
 
 def device_units():
@@ -249,7 +255,7 @@ class Runner:
             return
         if self.planner:
             out = sim.mppi_iterate(self.mpar, self.bstate, self.cmds)
-            if self.world > 1:      # the planner's one exchange step: all ranks agree on the best controller's plan
+            if self.world > 1 or under_torchrun():      # the planner's one exchange step: all ranks agree on the best controller's plan
                 from paper_2606_01478_b200 import planner
                 self.global_plan = planner.select_global_plan(sim, self.mpar, out, self.rank)
             return
@@ -571,7 +577,8 @@ def main():
     torch.cuda.set_device(local)
     device = f"cuda:{local}"
     barrier = None
-    if world > 1:
+    distributed = world > 1 or under_torchrun()      # torchrun with one rank still runs the NCCL init / barrier / reduce path
+    if distributed:
         dist.init_process_group("nccl", device_id=torch.device(device))
         barrier = dist.barrier
     pk = peaks()
@@ -584,7 +591,7 @@ def main():
             ms = time_steps(R.step, torch, steps, warmup, flush, barrier)
         kms = time_steps(R.rollout_only, torch, max(3, min(steps, 10)), 1, flush)     # dominant kernel alone
         t = torch.tensor([sum(ms)], dtype=torch.float64, device=device)
-        if world > 1:
+        if distributed:
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
         value = world * wl.drone_steps * steps / (total_ms * 1e-3)
@@ -615,7 +622,7 @@ def main():
         if want_e2e and R.e2e_ok:
             ems = time_host_steps(R.step_e2e, torch, max(3, min(steps, 10)), 2)
             et = torch.tensor([sum(ems) / len(ems)], dtype=torch.float64, device=device)
-            if world > 1:
+            if distributed:
                 dist.all_reduce(et, op=dist.ReduceOp.MAX)
             out["e2e"] = dict(value=world * wl.drone_steps / (float(et.item()) * 1e-3), unit=UNIT,
                               h2d_bytes_per_step=R.h2d, d2h_bytes_per_step=R.d2h, ms_per_step=float(et.item()))
@@ -707,7 +714,7 @@ def main():
         if name == "mppi":      # plans per second (the paper's requirement: 50 Hz)
             line["config"]["plans_per_sec"] = 1e3 / main_res["ms_per_step"]
         print(json.dumps(line))
-    if world > 1:
+    if distributed:
         dist.destroy_process_group()
     return 0
 

@@ -140,6 +140,8 @@ size_t cf_workspace_bytes(int64_t M, int64_t N, int model, const cf_params *p);
 /* Create a simulator of M worlds x N drones.  workspace_dev: device memory of >= cf_workspace_bytes() bytes, 256-byte
  * aligned, owned by the caller and kept alive until cf_destroy.  Validates p (CF_E_ARG / CF_E_SHAPE /
  * CF_E_UNSUPPORTED), never touches the device. */
+/* (Measurement switch: with CF_FORCE_GENERAL=1 in the environment at cf_create, cf_step always dispatches the general
+ * run-time-gated kernel, also where a lean compile-time-selected one exists; results agree to rounding.) */
 int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf_params *p,
               void *workspace_dev, size_t workspace_bytes);
 int cf_destroy(cf_sim *sim);

@@ -4,6 +4,8 @@
 #include "cf_device.cuh"
 #include "cf_internal.h"
 
+#include <cstdlib>
+
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -444,6 +446,7 @@ extern "C" int cf_create(cf_sim **out, int64_t M, int64_t N, int model, const cf
       ? launch_fp(p->integrator, p->iface, s->opt, REC_NONE, nullptr, nullptr, nullptr, &name, nullptr, true)
       : launch_ab(p->integrator, p->iface, s->opt, REC_NONE, nullptr, nullptr, nullptr, &name, nullptr, true);
   if (!ok) { delete s; return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration"); }
+  { const char *fg = getenv("CF_FORCE_GENERAL"); s->force_general = fg && fg[0] == '1'; }
   *out = s;
   return CF_OK;
 }
@@ -684,11 +687,15 @@ static int pick_block_rec(long long MN) {
 // was built for it (e.g. the rotor or position interface of the first-principles model, RK4 on the abstracted model):
 // everything that depends on WHICH kernel runs -- block size, snapshots per store, the pair-written record modes -- is
 // decided from this, not from the request.
+// Measurement switch: with CF_FORCE_GENERAL=1 in the environment when the simulator is created, every cf_step runs the
+// general OPT_ALL kernel (which gates each feature at run time from the same parameters) even where a lean instantiation
+// exists -- for like-for-like lean / general timings (bench.py).  Results agree to rounding.
+static int dispatch_opt_bits(const cf_sim *sim) { return sim->opt | (sim->force_general ? OPT_EXTRAS : 0); }
 static int dispatched_opt(const cf_sim *sim, int rec_mode) {
   int opt_used = 0;
   const bool found = sim->model == CF_MODEL_FIRST_PRINCIPLES
-      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true)
-      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
+      ? launch_fp(sim->p.integrator, sim->p.iface, dispatch_opt_bits(sim), rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true)
+      : launch_ab(sim->p.integrator, sim->p.iface, dispatch_opt_bits(sim), rec_mode, nullptr, nullptr, nullptr, nullptr, &opt_used, true);
   return found ? opt_used : -1;
 }
 static bool dispatches_lean(const cf_sim *sim, int rec_mode) {
@@ -716,8 +723,8 @@ static int do_launch(cf_sim *sim, const StepArgs *A, bool dry, const char **name
   if (grid) *grid = L.grid;
   if (block) *block = L.block;
   bool ok = sim->model == CF_MODEL_FIRST_PRINCIPLES
-      ? launch_fp(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, A, &sim->dp, &L, name, nullptr, dry)
-      : launch_ab(sim->p.integrator, sim->p.iface, sim->opt, rec_mode, A, &sim->dp, &L, name, nullptr, dry);
+      ? launch_fp(sim->p.integrator, sim->p.iface, dispatch_opt_bits(sim), rec_mode, A, &sim->dp, &L, name, nullptr, dry)
+      : launch_ab(sim->p.integrator, sim->p.iface, dispatch_opt_bits(sim), rec_mode, A, &sim->dp, &L, name, nullptr, dry);
   if (!ok) return fail(CF_E_UNSUPPORTED, "no kernel instantiation for this configuration");
   return CF_OK;
 }

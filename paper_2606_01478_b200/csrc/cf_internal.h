@@ -38,6 +38,7 @@ struct cf_sim {
   // cf_rollout_host: a second stream for the result copies and one event per slice (created on first use)
   bool wparam_foreign = false;   // cf_set_full replaced the parameter planes (cf_reset re-draws them and clears this)
   cudaStream_t copy_stream = nullptr;
+  bool force_general = false;     // CF_FORCE_GENERAL=1 at cf_create: dispatch the general kernel everywhere (measurement)
   bool copy_stream_owned = false; // created by cf_rollout_host (destroyed with the handle) vs given by cf_set_copy_stream
   cudaEvent_t slice_ev[16] = {};
 };

@@ -23,6 +23,11 @@ static const RolloutEntry kTableFP[] = {
   // the pair-written loop for the other record modes (REC_*_P): configs[0], configs[1], the world-count sweep
   CF_FP1(INTEG_RK4, IF_ATTITUDE, 0, REC_NONE_P), CF_FP1(INTEG_RK4, IF_ATTITUDE, 0, REC_SCALAR_P), CF_FP1(INTEG_RK4, IF_ATTITUDE, 0, REC_TMA_P),
   CF_FP1(INTEG_EULER, IF_ATTITUDE, 0, REC_NONE_P), CF_FP1(INTEG_EULER, IF_ATTITUDE, 0, REC_SCALAR_P), CF_FP1(INTEG_EULER, IF_ATTITUDE, 0, REC_TMA_P),
+  // round 3 ("dynamically select only the required functions", L282 "direct rotor velocity" control, L330 the
+  // full Mellinger stack): the nominal plant behind the rotor interface (motor-level control) and behind the position
+  // interface (position controller -> attitude controller -> mixer), which until now fell to the general kernel
+  CF_FP(INTEG_RK4, IF_ROTOR, 0), CF_FP(INTEG_EULER, IF_ROTOR, 0),
+  CF_FP(INTEG_RK4, IF_POSITION, 0), CF_FP(INTEG_EULER, IF_POSITION, 0),
   // general kernels
   CF_FP_GEN(INTEG_EULER, IF_ROTOR),    CF_FP_GEN(INTEG_RK4, IF_ROTOR),
   CF_FP_GEN(INTEG_EULER, IF_TORQUE),   CF_FP_GEN(INTEG_RK4, IF_TORQUE),

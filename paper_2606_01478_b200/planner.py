@@ -18,9 +18,9 @@ def gather_rows(row, group=None):
     """All ranks' rows, stacked in rank order: [world][2 + 4 H] on the device of `row`.  The planner's one collective."""
     import torch
     import torch.distributed as dist
-    world = dist.get_world_size(group) if dist.is_initialized() else 1
-    if world == 1:
+    if not dist.is_initialized():
         return row[None].contiguous()
+    world = dist.get_world_size(group)      # (a group of one rank still goes through the collective)
     parts = [torch.empty_like(row) for _ in range(world)]
     dist.all_gather(parts, row.contiguous(), group=group)
     return torch.stack(parts)

@@ -239,7 +239,45 @@ def depth(seed=REPORT_SEED, M=1024, model=MODEL_FP, width=64, height=64) -> Work
                     seed, 1, 1, 0, None, notes=dict(scene=scene))
 
 
-REGISTRY = {"depth": depth, "grad": grad, "mppi": mppi, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
+# ---- round 3: configurations of the paper's tasks that are NOT BASELINE.json benchmark rows ----
+def fp_pos(seed=REPORT_SEED, M=1 << 16, n_steps=500) -> Workload:
+    """The full onboard stack on the first-principles model: position targets -> geometric position controller (100 Hz)
+    -> attitude controller + mixer (500 Hz) -> Eqs. (1)-(6), RK4 1000 Hz; nominal plant, nothing recorded."""
+    rng = _rng(seed, 11)
+    cmds = np.zeros((1, M, 4), dtype=np.float32)
+    cmds[0, :, :3] = rng.uniform([-1, -1, 0.5], [1, 1, 1.5], (M, 3))
+    cmds[0, :, 3] = rng.uniform(-0.5, 0.5, M)
+    return Workload("fp_pos", M, 1, MODEL_FP,
+                    dict(integrator=RK4, iface=IF_POSITION, f_phys=1000.0, f_att=500.0, f_pos=100.0, init_mode=1,
+                         p0_lo=[-1, -1, 0.5], p0_hi=[1, 1, 1.5], tilt0_max=0.3),
+                    seed, n_steps, n_steps, 0, cmds)
+
+
+def fp_rotor(seed=REPORT_SEED, M=1 << 20, n_steps=100) -> Workload:
+    """Motor-level control ("direct rotor velocity"): four rotor speed commands per drone, redrawn every 50
+    steps; first-principles model, RK4 1000 Hz, nominal plant, nothing recorded."""
+    rng = _rng(seed, 12)
+    hold = 50
+    cmds = rng.uniform(12000.0, 17000.0, (-(-n_steps // hold), M, 4)).astype(np.float32)
+    return Workload("fp_rotor", M, 1, MODEL_FP,
+                    dict(integrator=RK4, iface=IF_ROTOR, f_phys=1000.0, f_att=500.0, init_mode=1, p0_lo=[-1, -1, 0],
+                         p0_hi=[1, 1, 2], tilt0_max=0.5),
+                    seed, n_steps, hold, 0, cmds)
+
+
+def ab_rk4(seed=REPORT_SEED, M=1 << 20, n_steps=100) -> Workload:
+    """The abstracted model integrated with RK4 (the paper's benchmark rows use Euler for it): attitude commands redrawn
+    every 50 steps, 500 Hz, nothing recorded.  Runs the general kernel (no lean instantiation)."""
+    rng = _rng(seed, 13)
+    hold = 50
+    cmds = _attitude_cmds(rng, -(-n_steps // hold), M, 0.3, 0.2, 0.33)
+    return Workload("ab_rk4", M, 1, MODEL_AB,
+                    dict(integrator=RK4, iface=IF_ATTITUDE, f_phys=500.0, f_att=500.0, init_mode=1, p0_lo=[-1, -1, 0],
+                         p0_hi=[1, 1, 2], tilt0_max=0.4),
+                    seed, n_steps, hold, 0, cmds)
+
+
+REGISTRY = {"fp_pos": fp_pos, "fp_rotor": fp_rotor, "ab_rk4": ab_rk4, "depth": depth, "grad": grad, "mppi": mppi, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg3b": cfg3b, "cfg4": cfg4, "cfg5": cfg5, "cfg5e": cfg5e}
 
 
 def make(name: str, **kw) -> Workload:

@@ -465,7 +465,10 @@ def test_general_kernel_at_sizes_where_the_lean_kernels_take_large_blocks(cf, cf
     att[..., 3] = 0.3
     lo, hi = [1.0] * 12, [1.0] * 12
     lo[0], hi[0], lo[4], hi[4] = 0.9, 1.1, 0.95, 1.05
-    cases = [(0, dict(base.params, iface=3), pos), (0, dict(base.params, iface=0, integrator=0), rot),
+    tq = np.zeros((1, M, 4), dtype=np.float32)
+    tq[..., :3] = rng.uniform(-2e-4, 2e-4, (1, M, 3))
+    tq[..., 3] = 0.3
+    cases = [(0, dict(base.params, iface=3, rnd_lo=lo, rnd_hi=hi), pos), (0, dict(base.params, iface=1, integrator=0), tq),
              (0, dict(base.params, rnd_lo=lo, rnd_hi=hi), att),                     # OPT_RANDP only: was REC_TMA_P on the general kernel
              (1, dict(integrator=1, f_phys=500.0, init_mode=1, p0_lo=[-1, -1, 0], p0_hi=[1, 1, 2], tilt0_max=0.4, iface=2), att)]
     for model, prm, cmds in cases:
@@ -481,6 +484,46 @@ def test_general_kernel_at_sizes_where_the_lean_kernels_take_large_blocks(cf, cf
             assert_state_close(rg[k], ro[k], model, 1e-4, f"{name} rec {k}")
         assert np.array_equal(g.counters(), o.counters())
         assert_state_close(g.get_state().cpu().numpy(), o.get_state(), model, 1e-4, name)
+
+
+@pytest.mark.parametrize("iface,integ", [(0, 0), (0, 1), (3, 0), (3, 1)])
+def test_lean_rotor_and_position_interface_kernels_of_the_first_principles_model(cf, cfo, W, iface, integ, monkeypatch):
+    """Round 3: compile-time-selected kernels for motor-level control and for the full onboard stack
+     on the nominal plant.  Free-running vs the oracle with records in every mode (none / scalar / TMA,
+    ragged and aligned sizes, large blocks), and against the general kernel forced by CF_FORCE_GENERAL=1."""
+    base = W.cfg2(seed=10, M=64, n_steps=6)
+    rng = np.random.default_rng(5)
+    for M, n, rec in ((32768, 12, 1), (257, 60, 7), (1024, 40, 0)):
+        if iface == 0:
+            cmds = rng.uniform(12000, 17000, (2, M, 4)).astype(np.float32)
+        else:
+            cmds = np.zeros((2, M, 4), dtype=np.float32)
+            cmds[..., :3] = rng.uniform(-1, 1, (2, M, 3)) + [0, 0, 1]
+            cmds[..., 3] = rng.uniform(-0.5, 0.5, (2, M))
+        prm = dict(base.params, iface=iface, integrator=integ, f_pos=100.0)
+        hold = -(-n // 2)
+        g, o = cf.Sim(M, 1, 0, prm), cfo.OracleSim(M, 1, 0, prm)
+        g.reset(10), o.reset(10)
+        rg = g.step(cmds, n, cmd_hold=hold, record_every=rec)
+        name, _, block = g.describe_launch()
+        assert "OPT_ALL" not in name, name
+        ro = o.step(cmds, n, cmd_hold=hold, record_every=rec)
+        if rec:
+            rgn = rg.cpu().numpy()
+            assert rgn.shape == ro.shape
+            for k in range(ro.shape[0]):
+                assert_state_close(rgn[k], ro[k], 0, 2e-4, f"{name} M {M} record {k}")
+        assert_state_close(g.get_state().cpu().numpy(), o.get_state(), 0, 2e-4, f"{name} M {M}")
+        assert np.array_equal(g.counters(), o.counters()) and np.array_equal(g.rec_table(), o.rec_table())
+        co = o.ctrl()
+        assert (np.abs(g.ctrl().cpu().numpy() - co) / (np.abs(co).max(axis=1, keepdims=True) + 1e-3)).max() <= 5e-4
+        monkeypatch.setenv("CF_FORCE_GENERAL", "1")
+        gg = cf.Sim(M, 1, 0, prm)
+        monkeypatch.delenv("CF_FORCE_GENERAL")
+        gg.reset(10)
+        gg.step(cmds, n, cmd_hold=hold, record_every=rec)
+        assert "OPT_ALL" in gg.describe_launch()[0]
+        assert_state_close(gg.get_state().cpu().numpy(), g.get_state().cpu().numpy().astype(np.float64), 0, 2e-5, "lean vs general")
 
 
 def test_captured_graph_of_odd_length_never_replays_a_pair_written_kernel(cf, W):
